@@ -1,0 +1,158 @@
+/*
+ * pinmpc.h — C ABI of libpinmpc.so: batched, construction-free ADMM-MPC solves on one B200 (sm_100a).
+ *
+ * One handle solves B independent linear time-varying MPC QPs, one per RL environment
+ * (eq. (16)-(17), with C = I and X_k = R^nx):
+ *
+ *     min  sum_{k=0}^{N-1} 1/2 |x_{k+1} - xbar_{k+1}|^2_Q + 1/2 |u_k - ubar_k|^2_R
+ *     s.t. x_{k+1} = A_k x_k + B_k u_k + c_k,   x_0 given,   u_k in U_k
+ *
+ * by a fixed number of scaled-form ADMM iterations in the block order of PAPER.md:L186 eq. (21a)
+ * -> (21b) -> (21c): equality-constrained step (exact time-varying LQR, solved with on-chip
+ * factors), projection onto U_k, dual update, residuals (the readings of the
+ * paper are listed there).  State x = [Theta(3) p(3) omega(3) v(3) g] (nx = 13, BASELINE.json
+ * config 0), control u = [f_0..f_{nw-1} | m_0..m_{nw-1} | fh_0..fh_{nf-1}], 3 floats per block.
+ *
+ * Conventions for every entry point
+ *   - plain C types; all array arguments are DEVICE pointers unless the name starts with h_ (host);
+ *   - arrays are float32 (contact flags uint8, iteration counts int32), contiguous, env-major,
+ *     row-major: [B,N,...] means index ((b*N + k)*... );
+ *   - the caller owns all device memory including the workspace; the library owns only the host
+ *     context.  Pointers given to pinmpc_set_problem / pinmpc_set_dynamics are BORROWED until the
+ *     next set call or pinmpc_destroy;
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  solve/get
+ *     enqueue work and return; nothing synchronises the host except pinmpc_create;
+ *   - every call returns a pinmpc_status; no exceptions, no abort.  CUDA errors are sticky in the
+ *     handle; pinmpc_last_error() describes the last failure;
+ *   - a handle is not thread-safe; different handles are independent;
+ *   - there is no CPU fallback: a device that is not compute capability 10.x gives
+ *     PINMPC_EUNSUPPORTED.
+ */
+#ifndef PINMPC_H
+#define PINMPC_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PINMPC_NX 13
+#define PINMPC_N_MAX 512
+
+typedef struct pinmpc_ctx *pinmpc_t;
+
+typedef enum {
+    PINMPC_OK = 0,
+    PINMPC_EINVAL = 1,       /* bad argument (NULL, non-positive size, negative weight ...)         */
+    PINMPC_EALLOC = 2,       /* workspace too small or host allocation failed                       */
+    PINMPC_ECUDA = 3,        /* a CUDA call or launch failed (sticky)                               */
+    PINMPC_ESTATE = 4,       /* call order violated (solve before set_problem, get before solve)    */
+    PINMPC_EUNSUPPORTED = 5  /* nx != 13, nu not in {12,18}, N > PINMPC_N_MAX, not an sm_100 device */
+} pinmpc_status;
+
+/* Constraint layout: which contacts u holds and the constants of U_k (eq. (7c);
+ * BASELINE.json configs 0 and 3).  A foot (6-D wrench contact) in stance is constrained to
+ *   |f_x|,|f_y| <= mu f_z,  |m_x| <= mx_coef f_z,  |m_y| <= my_coef f_z,  |m_z| <= mz_coef f_z,
+ *   0 <= f_z <= fz_max   — one set, projected jointly; a hand (3-D force contact) in contact to the
+ * box |f| <= hand_fmax componentwise; any contact whose flag is 0 to {0}.
+ * nu must equal 6*n_wrench + 3*n_force; supported: (2,0) and (2,2). */
+typedef struct {
+    int n_wrench;
+    int n_force;
+    float mu, fz_max;
+    float mx_coef, my_coef, mz_coef;
+    float hand_fmax;
+} pinmpc_layout;
+
+/* Solver variants, chosen by measurement.  AUTO picks the structured
+ * on-chip solver for problems given by pinmpc_set_problem and the dense one after
+ * pinmpc_set_dynamics. */
+typedef enum {
+    PINMPC_METHOD_AUTO = 0,
+    PINMPC_METHOD_DENSE = 1,     /* materialise A_k,B_k,c_k; dense Riccati factors streamed from HBM/L2 */
+    PINMPC_METHOD_SRB = 2        /* construction-free structured solver, factors resident on chip       */
+} pinmpc_method;
+
+/* Bytes of device workspace pinmpc_create needs for these sizes (0 on invalid arguments). */
+size_t pinmpc_workspace_bytes(int nx, int nu, int N, int B, const pinmpc_layout *layout);
+
+/* Same for a specific variant: PINMPC_METHOD_DENSE additionally holds A_k,B_k,c_k and the dense
+ * Riccati factors (about 2.7 KB per stage); a workspace of this size enables both variants. */
+size_t pinmpc_workspace_bytes_method(int nx, int nu, int N, int B, const pinmpc_layout *layout, pinmpc_method m);
+
+/* Create a handle.  rho > 0 is the ADMM penalty, iters >= 1 the (maximum) iteration count.
+ * d_workspace: device memory of at least pinmpc_workspace_bytes(...) bytes, 256-byte aligned,
+ * owned by the caller and kept alive until pinmpc_destroy.  Default weights are BASELINE.json's
+ * Q = diag(500,500,100,50,50,200,1,1,1,20,20,10,0), R = 1e-5 I and dt = 0.03; change them with
+ * pinmpc_set_weights.  Synchronises the device once (to read its properties). */
+pinmpc_status pinmpc_create(pinmpc_t *out, int nx, int nu, int N, int B, const pinmpc_layout *layout,
+                            float rho, int iters, void *d_workspace, size_t workspace_bytes);
+
+/* Diagonal cost weights (HOST pointers, copied) and the discretisation step of eq. (2)-(4). */
+pinmpc_status pinmpc_set_weights(pinmpc_t h, const float *h_Qdiag /*[nx]*/, const float *h_Rdiag /*[nu]*/, float dt);
+
+/* Early exit (north_star (4)).  eps_abs = eps_rel = 0 (default) => exactly `iters` iterations.
+ * Otherwise every check_every-th iteration an env stops once
+ *   r_prim <= eps_abs + eps_rel max(|u|_inf,|z|_inf)  and  r_dual <= eps_abs + eps_rel rho |y|_inf. */
+pinmpc_status pinmpc_set_tolerance(pinmpc_t h, float eps_abs, float eps_rel, int check_every);
+
+/* Force a solver variant (default PINMPC_METHOD_AUTO). */
+pinmpc_status pinmpc_set_method(pinmpc_t h, pinmpc_method m);
+
+/* Per-env problem data, all DEVICE pointers ("{A_k,B_k,e_k} are obtained along the
+ * input periodic contact sequence" — here from these raw inputs, on the device, every solve). */
+typedef struct {
+    const float *x0;           /* [B,nx]      initial state xi_0                                    */
+    const float *x_ref;        /* [B,N,nx]    reference xbar_1..xbar_N                              */
+    const float *u_ref;        /* [B,N,nu]    reference ubar_0..ubar_{N-1}; NULL => zeros           */
+    const uint8_t *contact;    /* [B,N,nc]    1 = contact i active at stage k, nc = n_wrench+n_force */
+    const float *foot_r;       /* [B,N,nc,3]  contact position minus CoM, world-aligned axes        */
+    const float *yaw;          /* [B,N]       linearisation yaw psi_k                               */
+    const float *mass;         /* [B]                                                               */
+    const float *inertia;      /* [B,3,3]     body-frame inertia, symmetric positive definite       */
+    const float *ext_wrench;   /* [B,N,6]     (F_ext, tau_ext) entering c_k; NULL => c_k = 0        */
+} pinmpc_problem;
+
+/* Record the problem (pointers are borrowed, nothing is copied or launched). */
+pinmpc_status pinmpc_set_problem(pinmpc_t h, const pinmpc_problem *p);
+
+/* Bypass the dynamics assembly with generic dense LTV matrices (DEVICE pointers, borrowed):
+ * A [B,N,nx,nx], Bm [B,N,nx,nu], c [B,N,nx] (NULL => 0).  x0, x_ref, u_ref and contact are still
+ * taken from pinmpc_set_problem.  Pass A = NULL to return to on-device assembly.  Solves then use
+ * the dense variant. */
+pinmpc_status pinmpc_set_dynamics(pinmpc_t h, const float *A, const float *Bm, const float *c);
+
+/* One batched solve: assembly (S1) + factorisation (S2) + iters x (equality step S3, projection
+ * S4, dual update S5, residuals / early exit S6), cold start z = y = 0.  Asynchronous on `stream`. */
+pinmpc_status pinmpc_solve(pinmpc_t h, void *stream);
+
+/* Copy results of the last solve into caller DEVICE buffers (any may be NULL), asynchronously on
+ * `stream` (use the solve's stream, or order the streams yourself):
+ *   x [B,N,nx] = x_1..x_N and u [B,N,nu] = u_0..u_{N-1} of the last equality step (they satisfy
+ *   the dynamics exactly), r_prim [B] = max_k |u_k - z_k|_inf, r_dual [B] = rho max_k |z_k -
+ *   z_k^prev|_inf, iters_done [B] (int32). */
+pinmpc_status pinmpc_get(pinmpc_t h, float *x, float *u, float *r_prim, float *r_dual, int *iters_done, void *stream);
+
+/* The splitting variables after the last solve: z [B,N,nu] (feasible copy), y [B,N,nu] (scaled dual). */
+pinmpc_status pinmpc_get_aux(pinmpc_t h, float *z, float *y, void *stream);
+
+/* Materialise the assembled dynamics of the current problem into caller DEVICE buffers
+ * A [B,N,nx,nx], Bm [B,N,nx,nu], c [B,N,nx] (any may be NULL); runs the assembly kernel on `stream`. */
+pinmpc_status pinmpc_get_dynamics(pinmpc_t h, float *A, float *Bm, float *c, void *stream);
+
+/* Number of kernel launches the last pinmpc_solve enqueued (for bench.py's gpu_launches). */
+int pinmpc_last_launch_count(pinmpc_t h);
+
+/* Human-readable description of the last error on this handle (owned by the handle; "" if none).
+ * With h = NULL: the last pinmpc_create failure in this thread. */
+const char *pinmpc_last_error(pinmpc_t h);
+
+/* Free the host context.  The workspace and all problem buffers stay with the caller. */
+void pinmpc_destroy(pinmpc_t h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PINMPC_H */

@@ -1,0 +1,285 @@
+"""Thin ctypes binding of libpinmpc.so (include/pinmpc.h): argument marshalling only.
+
+Every step of the path (assembly, factorisation, ADMM iterations, projection, residuals) runs in
+the CUDA kernels behind the C ABI.  PyTorch is used here for device memory and streams only.
+There is no CPU fallback: if the shared library is missing or cannot be loaded this module raises.
+The function names mirror the C entry points one to one; `Solver` is a convenience holder that
+keeps the borrowed tensors alive.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from ctypes import POINTER, c_char_p, c_float, c_int, c_size_t, c_void_p
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libpinmpc.so")
+NX = 13
+
+OK, EINVAL, EALLOC, ECUDA, ESTATE, EUNSUPPORTED = range(6)
+METHOD_AUTO, METHOD_DENSE, METHOD_SRB = 0, 1, 2
+_STATUS = {0: "PINMPC_OK", 1: "PINMPC_EINVAL", 2: "PINMPC_EALLOC", 3: "PINMPC_ECUDA", 4: "PINMPC_ESTATE",
+           5: "PINMPC_EUNSUPPORTED"}
+
+EXPORTS = ("pinmpc_workspace_bytes", "pinmpc_workspace_bytes_method", "pinmpc_create", "pinmpc_set_weights",
+           "pinmpc_set_tolerance", "pinmpc_set_method", "pinmpc_set_problem", "pinmpc_set_dynamics", "pinmpc_solve",
+           "pinmpc_get", "pinmpc_get_aux", "pinmpc_get_dynamics", "pinmpc_last_launch_count", "pinmpc_last_error",
+           "pinmpc_destroy")
+
+
+class PinmpcError(RuntimeError):
+    def __init__(self, status, msg):
+        super().__init__(f"{_STATUS.get(status, status)}: {msg}")
+        self.status = status
+
+
+class Layout(ctypes.Structure):
+    _fields_ = [("n_wrench", c_int), ("n_force", c_int), ("mu", c_float), ("fz_max", c_float),
+                ("mx_coef", c_float), ("my_coef", c_float), ("mz_coef", c_float), ("hand_fmax", c_float)]
+
+
+class Problem(ctypes.Structure):
+    _fields_ = [(n, c_void_p) for n in ("x0", "x_ref", "u_ref", "contact", "foot_r", "yaw", "mass", "inertia",
+                                        "ext_wrench")]
+
+
+_lib = None
+
+
+def load():
+    """Load libpinmpc.so (built in-tree by paper_2606_05687_b200.build / __graft_entry__.build)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_2606_05687_b200.build` (needs nvcc). "
+                          "There is no CPU fallback.")
+    lib = ctypes.CDLL(LIB_PATH)
+    lib.pinmpc_workspace_bytes.restype = c_size_t
+    lib.pinmpc_workspace_bytes.argtypes = [c_int, c_int, c_int, c_int, POINTER(Layout)]
+    lib.pinmpc_workspace_bytes_method.restype = c_size_t
+    lib.pinmpc_workspace_bytes_method.argtypes = [c_int, c_int, c_int, c_int, POINTER(Layout), c_int]
+    lib.pinmpc_create.restype = c_int
+    lib.pinmpc_create.argtypes = [POINTER(c_void_p), c_int, c_int, c_int, c_int, POINTER(Layout), c_float, c_int,
+                                  c_void_p, c_size_t]
+    lib.pinmpc_set_weights.restype = c_int
+    lib.pinmpc_set_weights.argtypes = [c_void_p, POINTER(c_float), POINTER(c_float), c_float]
+    lib.pinmpc_set_tolerance.restype = c_int
+    lib.pinmpc_set_tolerance.argtypes = [c_void_p, c_float, c_float, c_int]
+    lib.pinmpc_set_method.restype = c_int
+    lib.pinmpc_set_method.argtypes = [c_void_p, c_int]
+    lib.pinmpc_set_problem.restype = c_int
+    lib.pinmpc_set_problem.argtypes = [c_void_p, POINTER(Problem)]
+    lib.pinmpc_set_dynamics.restype = c_int
+    lib.pinmpc_set_dynamics.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p]
+    lib.pinmpc_solve.restype = c_int
+    lib.pinmpc_solve.argtypes = [c_void_p, c_void_p]
+    lib.pinmpc_get.restype = c_int
+    lib.pinmpc_get.argtypes = [c_void_p] + [c_void_p] * 6
+    lib.pinmpc_get_aux.restype = c_int
+    lib.pinmpc_get_aux.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p]
+    lib.pinmpc_get_dynamics.restype = c_int
+    lib.pinmpc_get_dynamics.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]
+    lib.pinmpc_last_launch_count.restype = c_int
+    lib.pinmpc_last_launch_count.argtypes = [c_void_p]
+    lib.pinmpc_last_error.restype = c_char_p
+    lib.pinmpc_last_error.argtypes = [c_void_p]
+    lib.pinmpc_destroy.restype = None
+    lib.pinmpc_destroy.argtypes = [c_void_p]
+    _lib = lib
+    return lib
+
+
+def _check(status, h=None):
+    if status != OK:
+        raise PinmpcError(status, load().pinmpc_last_error(h).decode())
+
+
+def _ptr(t):
+    return None if t is None else c_void_p(t.data_ptr())
+
+
+def make_layout(n_wrench=2, n_force=0, mu=0.5, fz_max=600.0, mx_coef=0.02, my_coef=0.02, mz_coef=0.01,
+                hand_fmax=150.0) -> Layout:
+    return Layout(n_wrench, n_force, mu, fz_max, mx_coef, my_coef, mz_coef, hand_fmax)
+
+
+# ---- one-to-one wrappers -------------------------------------------------------------------------
+def pinmpc_workspace_bytes(nx, nu, N, B, layout, method=None) -> int:
+    lib = load()
+    if method is None:
+        return int(lib.pinmpc_workspace_bytes(nx, nu, N, B, ctypes.byref(layout)))
+    return int(lib.pinmpc_workspace_bytes_method(nx, nu, N, B, ctypes.byref(layout), method))
+
+
+def pinmpc_create(nx, nu, N, B, layout, rho, iters, workspace_ptr, workspace_bytes):
+    h = c_void_p()
+    st = load().pinmpc_create(ctypes.byref(h), nx, nu, N, B, ctypes.byref(layout), rho, iters,
+                              c_void_p(workspace_ptr), workspace_bytes)
+    _check(st, None)
+    return h
+
+
+def pinmpc_set_weights(h, Qdiag, Rdiag, dt):
+    q = (c_float * len(Qdiag))(*[float(v) for v in Qdiag])
+    r = (c_float * len(Rdiag))(*[float(v) for v in Rdiag])
+    _check(load().pinmpc_set_weights(h, q, r, float(dt)), h)
+
+
+def pinmpc_set_tolerance(h, eps_abs, eps_rel, check_every):
+    _check(load().pinmpc_set_tolerance(h, float(eps_abs), float(eps_rel), int(check_every)), h)
+
+
+def pinmpc_set_method(h, method):
+    _check(load().pinmpc_set_method(h, int(method)), h)
+
+
+def pinmpc_set_problem(h, x0, x_ref, u_ref, contact, foot_r, yaw, mass, inertia, ext_wrench=None):
+    p = Problem(*[(None if t is None else t.data_ptr()) for t in
+                  (x0, x_ref, u_ref, contact, foot_r, yaw, mass, inertia, ext_wrench)])
+    _check(load().pinmpc_set_problem(h, ctypes.byref(p)), h)
+
+
+def pinmpc_set_dynamics(h, A, Bm, c=None):
+    _check(load().pinmpc_set_dynamics(h, _ptr(A), _ptr(Bm), _ptr(c)), h)
+
+
+def pinmpc_solve(h, stream=0):
+    _check(load().pinmpc_solve(h, c_void_p(stream)), h)
+
+
+def pinmpc_get(h, x=None, u=None, r_prim=None, r_dual=None, iters_done=None, stream=0):
+    _check(load().pinmpc_get(h, _ptr(x), _ptr(u), _ptr(r_prim), _ptr(r_dual), _ptr(iters_done), c_void_p(stream)), h)
+
+
+def pinmpc_get_aux(h, z=None, y=None, stream=0):
+    _check(load().pinmpc_get_aux(h, _ptr(z), _ptr(y), c_void_p(stream)), h)
+
+
+def pinmpc_get_dynamics(h, A=None, Bm=None, c=None, stream=0):
+    _check(load().pinmpc_get_dynamics(h, _ptr(A), _ptr(Bm), _ptr(c), c_void_p(stream)), h)
+
+
+def pinmpc_last_launch_count(h) -> int:
+    return int(load().pinmpc_last_launch_count(h))
+
+
+def pinmpc_destroy(h):
+    load().pinmpc_destroy(h)
+
+
+# ---- convenience holder ---------------------------------------------------------------------------
+class Solver:
+    """Owns the workspace (a torch uint8 tensor) and keeps borrowed problem tensors alive."""
+
+    def __init__(self, nu, N, B, layout=None, rho=1.0, iters=100, Qdiag=None, Rdiag=None, dt=0.03,
+                 method=METHOD_AUTO, device="cuda:0", dense_workspace=None):
+        import torch
+        load()
+        self.torch = torch
+        self.device = torch.device(device)
+        self.nu, self.N, self.B = int(nu), int(N), int(B)
+        self.layout = layout or make_layout(2, 2 if nu == 18 else 0)
+        if dense_workspace is None:
+            dense_workspace = method == METHOD_DENSE
+        wm = METHOD_DENSE if dense_workspace else METHOD_SRB
+        self.workspace_bytes = pinmpc_workspace_bytes(NX, nu, N, B, self.layout, wm)
+        if self.workspace_bytes == 0:
+            raise PinmpcError(EUNSUPPORTED, "unsupported sizes")
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(self.workspace_bytes, dtype=torch.uint8, device=self.device)
+            self.h = pinmpc_create(NX, nu, N, B, self.layout, float(rho), int(iters), self.workspace.data_ptr(),
+                                   self.workspace_bytes)
+        if Qdiag is not None or Rdiag is not None or dt is not None:
+            Qd = [500, 500, 100, 50, 50, 200, 1, 1, 1, 20, 20, 10, 0] if Qdiag is None else list(Qdiag)
+            Rd = [1e-5] * nu if Rdiag is None else list(Rdiag)
+            pinmpc_set_weights(self.h, Qd, Rd, dt)
+        if method != METHOD_AUTO:
+            pinmpc_set_method(self.h, method)
+        self._keep = {}
+
+    def _dev(self, a, dtype):
+        torch = self.torch
+        if a is None:
+            return None
+        if not isinstance(a, torch.Tensor):
+            a = torch.from_numpy(a)
+        return a.to(device=self.device, dtype=dtype).contiguous()
+
+    def set_problem(self, x0, x_ref, u_ref, contact, foot_r, yaw, mass, inertia, ext_wrench=None):
+        t = self.torch
+        f = t.float32
+        k = dict(x0=self._dev(x0, f), x_ref=self._dev(x_ref, f), u_ref=self._dev(u_ref, f),
+                 contact=self._dev(contact, t.uint8), foot_r=self._dev(foot_r, f), yaw=self._dev(yaw, f),
+                 mass=self._dev(mass, f), inertia=self._dev(inertia, f), ext_wrench=self._dev(ext_wrench, f))
+        B, N, nu = self.B, self.N, self.nu
+        nc = self.layout.n_wrench + self.layout.n_force
+        shapes = dict(x0=(B, NX), x_ref=(B, N, NX), u_ref=(B, N, nu), contact=(B, N, nc), foot_r=(B, N, nc, 3),
+                      yaw=(B, N), mass=(B,), inertia=(B, 3, 3), ext_wrench=(B, N, 6))
+        for name, v in k.items():
+            if v is not None and tuple(v.shape) != shapes[name]:
+                raise ValueError(f"{name}: shape {tuple(v.shape)} != {shapes[name]}")
+        self._keep.update(k)
+        pinmpc_set_problem(self.h, **k)
+
+    def set_workload(self, w):
+        self.set_problem(w.x0, w.x_ref, w.u_ref, w.contact, w.foot_r, w.yaw, w.mass, w.inertia, w.ext_wrench)
+
+    def set_dynamics(self, A, Bm, c=None):
+        f = self.torch.float32
+        k = dict(A=self._dev(A, f), Bm=self._dev(Bm, f), c=self._dev(c, f))
+        self._keep.update(k)
+        pinmpc_set_dynamics(self.h, k["A"], k["Bm"], k["c"])
+
+    def set_tolerance(self, eps_abs, eps_rel, check_every=1):
+        pinmpc_set_tolerance(self.h, eps_abs, eps_rel, check_every)
+
+    def set_method(self, method):
+        pinmpc_set_method(self.h, method)
+
+    def _stream(self, stream):
+        if stream is None:
+            stream = self.torch.cuda.current_stream(self.device)
+        return stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream)
+
+    def solve(self, stream=None):
+        pinmpc_solve(self.h, self._stream(stream))
+
+    def launch_count(self):
+        return pinmpc_last_launch_count(self.h)
+
+    def get(self, stream=None, aux=False):
+        t = self.torch
+        B, N, nu = self.B, self.N, self.nu
+        o = dict(x=t.empty((B, N, NX), dtype=t.float32, device=self.device),
+                 u=t.empty((B, N, nu), dtype=t.float32, device=self.device),
+                 r_prim=t.empty(B, dtype=t.float32, device=self.device),
+                 r_dual=t.empty(B, dtype=t.float32, device=self.device),
+                 iters_done=t.empty(B, dtype=t.int32, device=self.device))
+        s = self._stream(stream)
+        pinmpc_get(self.h, o["x"], o["u"], o["r_prim"], o["r_dual"], o["iters_done"], s)
+        if aux:
+            o["z"] = t.empty((B, N, nu), dtype=t.float32, device=self.device)
+            o["y"] = t.empty((B, N, nu), dtype=t.float32, device=self.device)
+            pinmpc_get_aux(self.h, o["z"], o["y"], s)
+        return o
+
+    def get_dynamics(self, stream=None):
+        t = self.torch
+        B, N, nu = self.B, self.N, self.nu
+        A = t.empty((B, N, NX, NX), dtype=t.float32, device=self.device)
+        Bm = t.empty((B, N, NX, nu), dtype=t.float32, device=self.device)
+        c = t.empty((B, N, NX), dtype=t.float32, device=self.device)
+        pinmpc_get_dynamics(self.h, A, Bm, c, self._stream(stream))
+        return A, Bm, c
+
+    def close(self):
+        if getattr(self, "h", None) is not None:
+            pinmpc_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,173 @@
+// pinmpc_common.cuh — host context and small device helpers shared by the kernels of libpinmpc.so.
+// CUDA path only: nothing here is shared with oracle/ (which is plain C and never includes this).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+
+#include "../../include/pinmpc.h"
+
+#define NX 13
+#define NU_MAX 18
+
+// Kernel-side copy of the constraint layout and weights (passed by value as a kernel argument).
+struct SolveParams {
+    int B, N, nu, nw, nf, iters, check_every;
+    float rho, dt, eps_abs, eps_rel;
+    float mu, fz_max, cx, cy, cz, hand_fmax;
+    float Qd[NX];
+    float Rd[NU_MAX];
+};
+
+struct ProblemPtrs {
+    const float *x0, *x_ref, *u_ref;
+    const uint8_t *contact;
+    const float *foot_r, *yaw, *mass, *inertia, *ext;
+};
+
+struct OutPtrs {
+    float *x, *u, *z, *y, *r_prim, *r_dual;
+    int *iters_done;
+};
+
+struct DensePtrs {       // dense variant: materialised dynamics and Riccati factors in HBM
+    const float *A, *Bm, *c;          // [B,N,13,13], [B,N,13,nu], [B,N,13] (c may be NULL)
+    float *K, *Minv, *s, *kappa;      // [B,N,nu,13], [B,N,nu,nu], [B,N,13], [B,N,nu]
+};
+
+struct pinmpc_ctx {
+    int nx, nu, N, B;
+    pinmpc_layout layout;
+    float rho;
+    int iters;
+    float eps_abs, eps_rel;
+    int check_every;
+    float Qd[NX], Rd[NU_MAX], dt;
+    pinmpc_method method;
+    bool have_problem, have_dynamics, solved;
+    pinmpc_problem prob;
+    const float *userA, *userB, *userC;
+    char *ws;
+    size_t ws_bytes;
+    // carved from the workspace
+    OutPtrs out;
+    float *dA, *dB, *dC, *dK, *dMinv, *dS, *dKappa;   // dense-only (NULL when the workspace is the small one)
+    int sm_count, smem_optin;
+    int launch_count;
+    cudaError_t sticky;
+    char err[256];
+};
+
+size_t pinmpc_ws_base_bytes(int nu, int N, int B);
+size_t pinmpc_ws_dense_bytes(int nu, int N, int B);
+
+// launchers (each returns the number of kernels it enqueued, or -1 with h->err set)
+int pinmpc_launch_assemble_dense(pinmpc_ctx *h, float *A, float *Bm, float *c, cudaStream_t st);
+int pinmpc_launch_solve_dense(pinmpc_ctx *h, cudaStream_t st);
+int pinmpc_launch_solve_srb(pinmpc_ctx *h, cudaStream_t st);
+size_t pinmpc_srb_smem_bytes(int nu, int N);
+
+static inline SolveParams make_params(const pinmpc_ctx *h)
+{
+    SolveParams p;
+    memset(&p, 0, sizeof p);
+    p.B = h->B; p.N = h->N; p.nu = h->nu; p.nw = h->layout.n_wrench; p.nf = h->layout.n_force;
+    p.iters = h->iters; p.check_every = h->check_every;
+    p.rho = h->rho; p.dt = h->dt; p.eps_abs = h->eps_abs; p.eps_rel = h->eps_rel;
+    p.mu = h->layout.mu; p.fz_max = h->layout.fz_max; p.cx = h->layout.mx_coef; p.cy = h->layout.my_coef;
+    p.cz = h->layout.mz_coef; p.hand_fmax = h->layout.hand_fmax;
+    for (int i = 0; i < NX; i++) p.Qd[i] = h->Qd[i];
+    for (int i = 0; i < NU_MAX; i++) p.Rd[i] = h->Rd[i];
+    return p;
+}
+
+static inline ProblemPtrs make_problem_ptrs(const pinmpc_ctx *h)
+{
+    ProblemPtrs q;
+    q.x0 = h->prob.x0; q.x_ref = h->prob.x_ref; q.u_ref = h->prob.u_ref; q.contact = h->prob.contact;
+    q.foot_r = h->prob.foot_r; q.yaw = h->prob.yaw; q.mass = h->prob.mass; q.inertia = h->prob.inertia;
+    q.ext = h->prob.ext_wrench;
+    return q;
+}
+
+#ifdef __CUDACC__
+// ---------------------------------------------------------------------------------------------
+// device helpers
+// ---------------------------------------------------------------------------------------------
+// Inverse of a 3x3 matrix (adjugate / determinant), row-major.
+__device__ __forceinline__ void inv3f(const float *M, float *Mi)
+{
+    float c00 = M[4] * M[8] - M[5] * M[7], c01 = M[5] * M[6] - M[3] * M[8], c02 = M[3] * M[7] - M[4] * M[6];
+    float id = 1.0f / (M[0] * c00 + M[1] * c01 + M[2] * c02);
+    Mi[0] = c00 * id; Mi[1] = (M[2] * M[7] - M[1] * M[8]) * id; Mi[2] = (M[1] * M[5] - M[2] * M[4]) * id;
+    Mi[3] = c01 * id; Mi[4] = (M[0] * M[8] - M[2] * M[6]) * id; Mi[5] = (M[2] * M[3] - M[0] * M[5]) * id;
+    Mi[6] = c02 * id; Mi[7] = (M[1] * M[6] - M[0] * M[7]) * id; Mi[8] = (M[0] * M[4] - M[1] * M[3]) * id;
+}
+
+// I_w^{-1} = R_z(yaw) I_b^{-1} R_z(yaw)^T  (BASELINE.json config 0), row-major 3x3.
+__device__ __forceinline__ void world_inertia_inv(const float *Ibinv, float cs, float sn, float *W)
+{
+    // T = R_z Ibinv
+    float T[9];
+#pragma unroll
+    for (int j = 0; j < 3; j++) {
+        T[0 * 3 + j] = cs * Ibinv[0 * 3 + j] - sn * Ibinv[1 * 3 + j];
+        T[1 * 3 + j] = sn * Ibinv[0 * 3 + j] + cs * Ibinv[1 * 3 + j];
+        T[2 * 3 + j] = Ibinv[2 * 3 + j];
+    }
+    // W = T R_z^T : W[i][0] = T[i][0] c - T[i][1] s ; W[i][1] = T[i][0] s + T[i][1] c ; W[i][2] = T[i][2]
+#pragma unroll
+    for (int i = 0; i < 3; i++) {
+        W[i * 3 + 0] = T[i * 3 + 0] * cs - T[i * 3 + 1] * sn;
+        W[i * 3 + 1] = T[i * 3 + 0] * sn + T[i * 3 + 1] * cs;
+        W[i * 3 + 2] = T[i * 3 + 2];
+    }
+}
+
+// Free minimiser t* of  1/2 (t-t0)^2 + 1/2 sum_i (a_i - w_i t)_+^2  (a_i = |y_i| >= 0): the height
+// of the exact Euclidean projection onto the foot wrench set before clamping to [0, f_max]
+// (z-update).  The derivative g(t) is increasing, concave and
+// piecewise linear with kinks b_i = a_i / w_i, so coordinate i is clipped at the optimum
+// (a_i > w_i t*) exactly when g(b_i) > 0.  Five kink evaluations decide the clipped set, one
+// division gives t*.  Branch-free; w_i > 0 required (iw_i = 1 / w_i).
+__device__ __forceinline__ float wrench_height(float t0, const float a[5], const float w[5], const float iw[5])
+{
+    float num = t0, den = 1.0f;
+#pragma unroll
+    for (int i = 0; i < 5; i++) {
+        float bi = a[i] * iw[i];
+        float g = bi - t0;
+#pragma unroll
+        for (int j = 0; j < 5; j++)
+            if (j != i) g -= w[j] * fmaxf(a[j] - w[j] * bi, 0.0f);
+        if (g > 0.0f) { num = fmaf(w[i], a[i], num); den = fmaf(w[i], w[i], den); }
+    }
+    return num / den;
+}
+
+// Exact projection of one foot wrench (f, m) onto W; writes the projected 6 values.
+__device__ __forceinline__ void project_wrench(const SolveParams &P, float fx, float fy, float fz, float mx, float my,
+                                               float mz, float &ofx, float &ofy, float &ofz, float &omx, float &omy,
+                                               float &omz)
+{
+    const float w[5] = { P.mu, P.mu, P.cx, P.cy, P.cz };
+    const float iw[5] = { 1.0f / P.mu, 1.0f / P.mu, 1.0f / P.cx, 1.0f / P.cy, 1.0f / P.cz };
+    const float a[5] = { fabsf(fx), fabsf(fy), fabsf(mx), fabsf(my), fabsf(mz) };
+    float t = wrench_height(fz, a, w, iw);
+    t = fminf(fmaxf(t, 0.0f), P.fz_max);
+    ofx = copysignf(fminf(a[0], w[0] * t), fx);
+    ofy = copysignf(fminf(a[1], w[1] * t), fy);
+    ofz = t;
+    omx = copysignf(fminf(a[2], w[2] * t), mx);
+    omy = copysignf(fminf(a[3], w[3] * t), my);
+    omz = copysignf(fminf(a[4], w[4] * t), mz);
+}
+
+__device__ __forceinline__ float warp_max(float v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+#endif  // __CUDACC__
