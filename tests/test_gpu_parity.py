@@ -3,7 +3,7 @@
 north_star tolerances, per env, after the same fixed iteration count:
     max|du| <= 1e-3 (1 + |u_ref|_inf),  max|dx| <= 1e-4 (1 + |x_ref|_inf),  residuals to 1e-3 relative
 with "ref" read as the oracle's solution AND as the tracking reference, enforcing the tighter of
-the two (reading D14); residual floor per reading D15 (32 fp32 ulps of 1 + |u|_inf).
+the two (reading D14); residual floor per reading D15 (5e-5 (1 + |u|_inf)).
 """
 import numpy as np
 import pytest
@@ -54,9 +54,10 @@ def check_parity(w, got, ref, envs=None):
     worst_u = np.max(du / tol_u); worst_x = np.max(dx / tol_x)
     assert worst_u <= 1.0, f"max|du| / tol = {worst_u:.3f} (env {np.argmax(du / tol_u)})"
     assert worst_x <= 1.0, f"max|dx| / tol = {worst_x:.3f} (env {np.argmax(dx / tol_x)})"
-    # residuals are differences of O(|u|) fp32 numbers: 1e-3 relative (north_star) plus an absolute
-    # floor of a few fp32 ulps of |u| that no relative bound on a tiny residual can absorb (D15)
-    floor = 32 * np.finfo(np.float32).eps * (1 + np.abs(ref["u"]).max(axis=ax))
+    # residuals: 1e-3 relative (north_star) plus an absolute floor (reading D15).  r_prim = max|u - z|
+    # is a difference of O(|u|) fp32 numbers, so it inherits the ABSOLUTE error of u and z, which
+    # north_star itself allows to be 1e-3 (1 + |u|); the floor is 1/20 of that allowance.
+    floor = 0.05 * 1e-3 * (1 + np.abs(ref["u"]).max(axis=ax))
     for name in ("r_prim", "r_dual"):
         r = got[name][sel].astype(np.float64)
         assert np.all(np.abs(r - ref[name]) <= 1e-3 * ref[name] + floor), name
