@@ -1,0 +1,303 @@
+#!/usr/bin/env python
+"""bench.py — batched ADMM-MPC solves/s at B=4096, N=50, 100 fixed iterations (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 2]
+                    [--method auto|srb|dense] [--B ..] [--N ..]
+
+A "step" is one pinmpc_solve of the whole batch: assembly + factorisation + all ADMM iterations
+ on synthetic inputs (gen/) that are resident in HBM when the timed region
+starts.  Timing: CUDA events on the launching stream around every step, an L2 flush (256 MiB write)
+between steps, max over ranks.  `e2e` repeats the measurement through the public API with HOST
+(pinned) buffers: H2D copies of every input and D2H reads of x,u,residuals inside the timed region.
+`--gpus N` (under torchrun) runs N independent replicas: the path does not shard across GPUs
+(replicas only, no collective on the data path).
+`--impl reference` times the fp64 CPU oracle (oracle/) on the host cores, a bounded sample per step.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "batched ADMM-MPC solves/s at B=4096,N=50 (fixed iters); % of roofline"
+
+# Algorithmic FLOPs of the formulation shipped (structured 6-D-input LQR):
+FLOP_PER_STAGE_ITER = {12: 995.0, 18: 1245.0}     # one stage of one ADMM iteration
+FLOP_PER_STAGE_ONCE = {12: 3900.0, 18: 4700.0}    # assembly + factorisation, once per solve
+# dense-generic count of SURVEY.md 8(d), used when --method dense is timed
+FLOP_DENSE_ITER = {12: 2700.0, 18: 3700.0}
+FLOP_DENSE_ONCE = {12: 33000.0, 18: 60000.0}
+FMA_LANES_PER_SM = 128
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2)
+    ap.add_argument("--method", default="auto", choices=["auto", "srb", "dense"])
+    ap.add_argument("--B", type=int, default=None)
+    ap.add_argument("--N", type=int, default=None)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons sampled while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([t.strip() for t in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        self.th.join(timeout=2)
+        sm, mx, reasons = [], None, set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx = float(r[1])
+            except (ValueError, IndexError):
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def flops_per_solve(w, method):
+    st = w.B * w.N
+    if method == "dense":
+        return st * (FLOP_DENSE_ONCE[w.nu] + w.iters * FLOP_DENSE_ITER[w.nu])
+    return st * (FLOP_PER_STAGE_ONCE[w.nu] + w.iters * FLOP_PER_STAGE_ITER[w.nu])
+
+
+def time_oracle(w, n_envs, threads=0):
+    import numpy as np
+    import gen
+    import oracle
+    sub = gen.subset(w, np.arange(min(n_envs, w.B)))
+    t0 = time.perf_counter()
+    oracle.solve(sub, nthreads=threads)
+    return sub.B, time.perf_counter() - t0
+
+
+def run_reference(args):
+    """The oracle, as it stands, on the host cores: each step solves a bounded sample of the workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import gen
+    import oracle
+    oracle.build()
+    w = gen.make_config(args.config, B=args.B, N=args.N)
+    n = min(w.B, 128)
+    for _ in range(args.warmup):
+        time_oracle(w, n)
+    t = 0.0
+    for _ in range(args.steps):
+        t += time_oracle(w, n)[1]
+    ms = 1e3 * t / args.steps
+    val = n / (ms * 1e-3)
+    sample = f"first {n} of {w.B} envs of {w.name} per step, all {w.iters} iterations, fp64"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": "solves/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "B": w.B, "N": w.N, "iters": w.iters, "nu": w.nu, "sample_envs_per_step": n},
+        "cpu_baseline": {"value": val, "unit": "solves/s", "cores": oracle.max_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": "solves/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import numpy as np
+    import torch
+    import gen
+    from paper_2606_05687_b200 import METHOD_AUTO, METHOD_DENSE, METHOD_SRB, Solver, binding, make_layout
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback); use --impl reference for the oracle")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    w = gen.make_config(args.config, B=args.B, N=args.N)
+    method = {"auto": METHOD_AUTO, "srb": METHOD_SRB, "dense": METHOD_DENSE}[args.method]
+    mname = "dense" if args.method == "dense" else "srb"
+    lay = make_layout(w.n_wrench, w.n_force, w.mu, w.fz_max, w.mx_coef, w.my_coef, w.mz_coef, w.hand_fmax)
+    s = Solver(w.nu, w.N, w.B, layout=lay, rho=w.rho, iters=w.iters, Qdiag=w.Qdiag, Rdiag=w.Rdiag, dt=w.dt,
+               method=method, device=dev)
+    s.set_workload(w)
+    stream = torch.cuda.current_stream(dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    def timed(fn, steps):
+        evs = []
+        for _ in range(steps):
+            flush.zero_()                                   # L2 flush, outside the per-step events
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream); fn(); b.record(stream)
+            evs.append((a, b))
+        torch.cuda.synchronize(dev)
+        return [a.elapsed_time(b) for a, b in evs]
+
+    # ---- device-resident timing ------------------------------------------------------------------
+    for _ in range(max(args.warmup, 3)):
+        s.solve()
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    if sampler:
+        sampler.start()
+    ms_steps = timed(s.solve, args.steps)
+    barrier()
+    clocks = sampler.stop() if sampler else None
+    launches = s.launch_count() * args.steps
+    ms = float(np.mean(ms_steps))
+
+    # ---- end to end through the public API with host buffers ----------------------------------------
+    e2e = None
+    if not args.no_e2e:
+        names = [n for n in gen.Workload.ARRAYS if getattr(w, n) is not None]
+        host = {n: torch.from_numpy(getattr(w, n)).pin_memory() for n in names}
+        devbuf = {n: torch.empty_like(host[n], device=dev) for n in names}
+        s.set_problem(**{n: devbuf.get(n) for n in gen.Workload.ARRAYS})
+        for n in names:
+            devbuf[n].copy_(host[n], non_blocking=True)
+        s.solve()
+        out_dev = s.get()
+        out_host = {k: torch.empty_like(v, device="cpu").pin_memory() for k, v in out_dev.items()}
+        h2d = sum(host[n].numel() * host[n].element_size() for n in names)
+        d2h = sum(v.numel() * v.element_size() for v in out_host.values())
+
+        def step_e2e():
+            for n in names:
+                devbuf[n].copy_(host[n], non_blocking=True)
+            s.solve()
+            binding.pinmpc_get(s.h, out_dev["x"], out_dev["u"], out_dev["r_prim"], out_dev["r_dual"],
+                               out_dev["iters_done"], stream.cuda_stream)
+            for k in out_host:
+                out_host[k].copy_(out_dev[k], non_blocking=True)
+
+        for _ in range(3):
+            step_e2e()
+        barrier()
+        ms_e2e = float(np.mean(timed(step_e2e, args.steps)))
+        barrier()
+        e2e = (ms_e2e, h2d, d2h)
+
+    # ---- max over ranks ---------------------------------------------------------------------------
+    if dist is not None:
+        t = torch.tensor([ms, e2e[0] if e2e else 0.0], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t[0]); e2e = (float(t[1]), e2e[1], e2e[2]) if e2e else None
+
+    if rank == 0:
+        total_solves = w.B * world
+        value = total_solves / (ms * 1e-3)
+        fl = flops_per_solve(w, mname)
+        achieved = fl / (ms * 1e-3) / 1e12                     # TFLOP/s of this rank's kernel(s)
+        props = torch.cuda.get_device_properties(dev)
+        peaks = {}
+        try:
+            peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+        except OSError:
+            pass
+        sm_max_mhz = (clocks or {}).get("sm_max_mhz") or peaks.get("sm_max_mhz") or 1965.0
+        peak = props.multi_processor_count * FMA_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
+        # measured FMA-pipe peak on this device (register-resident loop), for context
+        scratch = torch.zeros(1, device=dev)
+        binding.pinmpc_probe_fma(props.multi_processor_count * 8, 2000, scratch, stream.cuda_stream)
+        torch.cuda.synchronize(dev)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        pf = binding.pinmpc_probe_fma(props.multi_processor_count * 8, 20000, scratch, stream.cuda_stream)
+        b.record(stream); torch.cuda.synchronize(dev)
+        fma_meas = pf / (a.elapsed_time(b) * 1e-3) / 1e12
+
+        io_bytes = sum(getattr(w, n).nbytes for n in gen.Workload.ARRAYS if getattr(w, n) is not None) + \
+            w.B * w.N * (13 + 3 * w.nu) * 4 + w.B * 12
+        line = {
+            "metric": METRIC, "value": value, "unit": "solves/s", "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": w.name, "B": w.B, "N": w.N, "iters": w.iters, "nu": w.nu, "rho": w.rho,
+                       "method": mname, "l2": "flushed (256 MiB write) between timed steps; per-step CUDA events",
+                       "multi_gpu": "replicas only (no collective on the data path)"},
+            "stage_iters_per_s": total_solves * w.N * w.iters / (ms * 1e-3),
+            "ms_min": float(np.min(ms_steps)), "ms_median": float(np.median(ms_steps)),
+            "gpu_launches": launches,
+            "clocks": clocks,
+            "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+                         "traffic": None,
+                         "peak_source": f"{props.multi_processor_count} SMs x {FMA_LANES_PER_SM} FP32 lanes x 2 x "
+                                        f"{sm_max_mhz:.0f} MHz (guide unit counts, max SM clock)",
+                         "peak_measured_fma_tflops": fma_meas,
+                         "flops_per_launch": fl,
+                         "hbm_algorithmic_bytes": io_bytes,
+                         "hbm_gbs_achieved": io_bytes / (ms * 1e-3) / 1e9,
+                         "hbm_peak_gbs": peaks.get("hbm_gbs")},
+        }
+        if e2e:
+            line["e2e"] = {"value": total_solves / (e2e[0] * 1e-3), "unit": "solves/s", "ms_per_step": e2e[0],
+                           "h2d_bytes_per_step": e2e[1], "d2h_bytes_per_step": e2e[2]}
+        if not args.no_cpu_baseline and world == 1:
+            import oracle
+            oracle.build()
+            n0, t0 = time_oracle(w, 32)
+            n = int(min(w.B, max(32, 12.0 * n0 / max(t0, 1e-3))))        # about 12 s of CPU work
+            n, t = time_oracle(w, n)
+            line["cpu_baseline"] = {"value": n / t, "unit": "solves/s", "cores": oracle.max_threads(), "kind": "oracle",
+                                    "sample": f"first {n} of {w.B} envs of {w.name}, all {w.iters} iterations, fp64, {t:.1f} s"}
+        print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

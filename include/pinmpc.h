@@ -142,6 +142,12 @@ pinmpc_status pinmpc_get_aux(pinmpc_t h, float *z, float *y, void *stream);
  * A [B,N,nx,nx], Bm [B,N,nx,nu], c [B,N,nx] (any may be NULL); runs the assembly kernel on `stream`. */
 pinmpc_status pinmpc_get_dynamics(pinmpc_t h, float *A, float *Bm, float *c, void *stream);
 
+/* Measurement aid, not part of the solve path: enqueue a register-resident FP32 FMA loop
+ * (`blocks` CTAs x 256 threads x 128*iters FMAs) on `stream` and return the FLOPs it performs
+ * (0 on a launch error).  bench.py times it with CUDA events to report the measured FMA-pipe peak
+ * next to the roofline.  d_out: one float of device scratch. */
+double pinmpc_probe_fma(int blocks, int iters, float *d_out, void *stream);
+
 /* Number of kernel launches the last pinmpc_solve enqueued (for bench.py's gpu_launches). */
 int pinmpc_last_launch_count(pinmpc_t h);
 

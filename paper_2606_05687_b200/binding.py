@@ -24,7 +24,7 @@ _STATUS = {0: "PINMPC_OK", 1: "PINMPC_EINVAL", 2: "PINMPC_EALLOC", 3: "PINMPC_EC
 EXPORTS = ("pinmpc_workspace_bytes", "pinmpc_workspace_bytes_method", "pinmpc_create", "pinmpc_set_weights",
            "pinmpc_set_tolerance", "pinmpc_set_method", "pinmpc_set_problem", "pinmpc_set_dynamics", "pinmpc_solve",
            "pinmpc_get", "pinmpc_get_aux", "pinmpc_get_dynamics", "pinmpc_last_launch_count", "pinmpc_last_error",
-           "pinmpc_destroy")
+           "pinmpc_destroy", "pinmpc_probe_fma")
 
 
 class PinmpcError(RuntimeError):
@@ -84,6 +84,8 @@ def load():
     lib.pinmpc_last_launch_count.argtypes = [c_void_p]
     lib.pinmpc_last_error.restype = c_char_p
     lib.pinmpc_last_error.argtypes = [c_void_p]
+    lib.pinmpc_probe_fma.restype = ctypes.c_double
+    lib.pinmpc_probe_fma.argtypes = [c_int, c_int, c_void_p, c_void_p]
     lib.pinmpc_destroy.restype = None
     lib.pinmpc_destroy.argtypes = [c_void_p]
     _lib = lib
@@ -162,6 +164,10 @@ def pinmpc_get_dynamics(h, A=None, Bm=None, c=None, stream=0):
 
 def pinmpc_last_launch_count(h) -> int:
     return int(load().pinmpc_last_launch_count(h))
+
+
+def pinmpc_probe_fma(blocks, iters, d_out, stream=0) -> float:
+    return float(load().pinmpc_probe_fma(int(blocks), int(iters), _ptr(d_out), c_void_p(stream)))
 
 
 def pinmpc_destroy(h):
