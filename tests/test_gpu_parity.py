@@ -62,9 +62,11 @@ def check_parity(w, got, ref, envs=None):
         r = got[name][sel].astype(np.float64)
         assert np.all(np.abs(r - ref[name]) <= 1e-3 * ref[name] + floor), name
     assert np.array_equal(got["iters_done"][sel], ref["iters_done"])
-    # z and y are not part of north_star's bar but must track at the same level as u
+    # z and y are not part of north_star's bar.  Both live in the units of u (y accumulates u - z every
+    # iteration, so it inherits u's absolute rounding error), hence both get u's allowance.
     dz = np.abs(got["z"][sel] - ref["z"]).max(axis=ax); dy = np.abs(got["y"][sel] - ref["y"]).max(axis=ax)
-    assert np.all(dz <= 2 * tol_u) and np.all(dy <= 2e-3 * (1 + np.abs(ref["y"]).max(axis=ax)))
+    assert np.all(dz <= 2 * tol_u), f"max|dz| / tol = {np.max(dz / tol_u):.3f}"
+    assert np.all(dy <= tol_u), f"max|dy| / tol = {np.max(dy / tol_u):.3f}"
     return worst_u, worst_x
 
 
