@@ -39,7 +39,7 @@ extern "C" {
 #endif
 
 #define PINMPC_NX 13
-#define PINMPC_N_MAX 512
+#define PINMPC_N_MAX 256
 
 typedef struct pinmpc_ctx *pinmpc_t;
 
@@ -100,6 +100,10 @@ pinmpc_status pinmpc_set_tolerance(pinmpc_t h, float eps_abs, float eps_rel, int
 
 /* Force a solver variant (default PINMPC_METHOD_AUTO). */
 pinmpc_status pinmpc_set_method(pinmpc_t h, pinmpc_method m);
+
+/* Tuning knob of the structured solver: envs solved per thread block (1..4; 0 = choose by the
+ * occupancy heuristic of DESIGN.md "Kernels").  Results do not depend on it. */
+pinmpc_status pinmpc_set_tuning(pinmpc_t h, int envs_per_cta);
 
 /* Per-env problem data, all DEVICE pointers ("{A_k,B_k,e_k} are obtained along the
  * input periodic contact sequence" — here from these raw inputs, on the device, every solve). */

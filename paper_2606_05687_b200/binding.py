@@ -22,7 +22,7 @@ _STATUS = {0: "PINMPC_OK", 1: "PINMPC_EINVAL", 2: "PINMPC_EALLOC", 3: "PINMPC_EC
            5: "PINMPC_EUNSUPPORTED"}
 
 EXPORTS = ("pinmpc_workspace_bytes", "pinmpc_workspace_bytes_method", "pinmpc_create", "pinmpc_set_weights",
-           "pinmpc_set_tolerance", "pinmpc_set_method", "pinmpc_set_problem", "pinmpc_set_dynamics", "pinmpc_solve",
+           "pinmpc_set_tolerance", "pinmpc_set_method", "pinmpc_set_tuning", "pinmpc_set_problem", "pinmpc_set_dynamics", "pinmpc_solve",
            "pinmpc_get", "pinmpc_get_aux", "pinmpc_get_dynamics", "pinmpc_last_launch_count", "pinmpc_last_error",
            "pinmpc_destroy", "pinmpc_probe_fma")
 
@@ -68,6 +68,8 @@ def load():
     lib.pinmpc_set_tolerance.argtypes = [c_void_p, c_float, c_float, c_int]
     lib.pinmpc_set_method.restype = c_int
     lib.pinmpc_set_method.argtypes = [c_void_p, c_int]
+    lib.pinmpc_set_tuning.restype = c_int
+    lib.pinmpc_set_tuning.argtypes = [c_void_p, c_int]
     lib.pinmpc_set_problem.restype = c_int
     lib.pinmpc_set_problem.argtypes = [c_void_p, POINTER(Problem)]
     lib.pinmpc_set_dynamics.restype = c_int
@@ -134,6 +136,10 @@ def pinmpc_set_tolerance(h, eps_abs, eps_rel, check_every):
 
 def pinmpc_set_method(h, method):
     _check(load().pinmpc_set_method(h, int(method)), h)
+
+
+def pinmpc_set_tuning(h, envs_per_cta):
+    _check(load().pinmpc_set_tuning(h, int(envs_per_cta)), h)
 
 
 def pinmpc_set_problem(h, x0, x_ref, u_ref, contact, foot_r, yaw, mass, inertia, ext_wrench=None):
@@ -242,6 +248,9 @@ class Solver:
 
     def set_method(self, method):
         pinmpc_set_method(self.h, method)
+
+    def set_tuning(self, envs_per_cta):
+        pinmpc_set_tuning(self.h, envs_per_cta)
 
     def _stream(self, stream):
         if stream is None:

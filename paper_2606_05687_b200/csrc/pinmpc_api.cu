@@ -16,11 +16,29 @@ size_t pinmpc_ws_base_bytes(int nu, int N, int B)
     return align_up(st * NX * 4) + 3 * align_up(st * nu * 4) + 3 * align_up((size_t)B * 4);
 }
 
+// structured-solver factors (SrbWs)
+static const int SRB_NARR = 12;
+static void srb_sizes(int nu, int N, int B, size_t *f)
+{
+    size_t st = (size_t)B * N;
+    int nc = 2 + (nu - 12) / 3;
+    f[0] = st * 72; f[1] = (size_t)B * (N + 1) * 12; f[2] = st * 6; f[3] = st * 12; f[4] = st * 2; f[5] = st * 21;
+    f[6] = st * 6; f[7] = st * 21; f[8] = st * 6; f[9] = st * 3 * nc; f[10] = st * nu; f[11] = st;
+}
+
+size_t pinmpc_ws_srb_bytes(int nu, int N, int B)
+{
+    size_t f[SRB_NARR], t = 0;
+    srb_sizes(nu, N, B, f);
+    for (int i = 0; i < SRB_NARR; i++) t += align_up(f[i] * 4);
+    return t;
+}
+
 // dense extras: A, Bm, c, K, Minv, s, kappa
 size_t pinmpc_ws_dense_bytes(int nu, int N, int B)
 {
     size_t st = (size_t)B * N;
-    return pinmpc_ws_base_bytes(nu, N, B) + align_up(st * NX * NX * 4) + align_up(st * NX * nu * 4) +
+    return pinmpc_ws_base_bytes(nu, N, B) + pinmpc_ws_srb_bytes(nu, N, B) + align_up(st * NX * NX * 4) + align_up(st * NX * nu * 4) +
            align_up(st * NX * 4) + align_up(st * nu * NX * 4) + align_up(st * nu * nu * 4) + align_up(st * NX * 4) +
            align_up(st * nu * 4);
 }
@@ -39,14 +57,15 @@ extern "C" size_t pinmpc_workspace_bytes(int nx, int nu, int N, int B, const pin
 {
     pinmpc_status why;
     if (!sizes_ok(nx, nu, N, B, layout, &why)) return 0;
-    return pinmpc_ws_base_bytes(nu, N, B);
+    return pinmpc_ws_base_bytes(nu, N, B) + pinmpc_ws_srb_bytes(nu, N, B);
 }
 
 extern "C" size_t pinmpc_workspace_bytes_method(int nx, int nu, int N, int B, const pinmpc_layout *layout, pinmpc_method m)
 {
     pinmpc_status why;
     if (!sizes_ok(nx, nu, N, B, layout, &why)) return 0;
-    return m == PINMPC_METHOD_DENSE ? pinmpc_ws_dense_bytes(nu, N, B) : pinmpc_ws_base_bytes(nu, N, B);
+    return m == PINMPC_METHOD_DENSE ? pinmpc_ws_dense_bytes(nu, N, B)
+                                    : pinmpc_ws_base_bytes(nu, N, B) + pinmpc_ws_srb_bytes(nu, N, B);
 }
 
 static pinmpc_status set_err(pinmpc_t h, pinmpc_status s, const char *msg)
@@ -63,13 +82,13 @@ extern "C" pinmpc_status pinmpc_create(pinmpc_t *out, int nx, int nu, int N, int
     *out = nullptr;
     pinmpc_status why = PINMPC_OK;
     if (!sizes_ok(nx, nu, N, B, layout, &why))
-        return set_err(nullptr, why, "pinmpc_create: unsupported or invalid sizes (nx=13, nu in {12,18}, 1<=N<=512, B>=1)");
+        return set_err(nullptr, why, "pinmpc_create: unsupported or invalid sizes (nx=13, nu in {12,18}, 1<=N<=256, B>=1)");
     if (!(rho > 0.0f) || iters < 1) return set_err(nullptr, PINMPC_EINVAL, "pinmpc_create: rho must be > 0 and iters >= 1");
     if (!(layout->mu > 0.0f) || !(layout->fz_max > 0.0f) || !(layout->mx_coef > 0.0f) || !(layout->my_coef > 0.0f) ||
         !(layout->mz_coef > 0.0f) || (layout->n_force > 0 && !(layout->hand_fmax >= 0.0f)))
         return set_err(nullptr, PINMPC_EINVAL, "pinmpc_create: layout constants must be positive");
     if (!d_workspace || ((uintptr_t)d_workspace & 255)) return set_err(nullptr, PINMPC_EINVAL, "pinmpc_create: workspace NULL or not 256-byte aligned");
-    size_t base = pinmpc_ws_base_bytes(nu, N, B);
+    size_t base = pinmpc_ws_base_bytes(nu, N, B) + pinmpc_ws_srb_bytes(nu, N, B);
     if (workspace_bytes < base) return set_err(nullptr, PINMPC_EALLOC, "pinmpc_create: workspace smaller than pinmpc_workspace_bytes()");
 
     int dev = 0, major = 0, sms = 0, optin = 0;
@@ -104,6 +123,14 @@ extern "C" pinmpc_status pinmpc_create(pinmpc_t *out, int nx, int nu, int N, int
     h->out.r_prim = (float *)take((size_t)B * 4);
     h->out.r_dual = (float *)take((size_t)B * 4);
     h->out.iters_done = (int *)take((size_t)B * 4);
+    {
+        size_t f[SRB_NARR];
+        srb_sizes(nu, N, B, f);
+        h->srb.Kh = (float *)take(f[0] * 4); h->srb.qv = (float *)take(f[1] * 4); h->srb.c6 = (float *)take(f[2] * 4);
+        h->srb.sv = (float *)take(f[3] * 4); h->srb.cs = (float *)take(f[4] * 4); h->srb.MI = (float *)take(f[5] * 4);
+        h->srb.KG = (float *)take(f[6] * 4); h->srb.LI = (float *)take(f[7] * 4); h->srb.IW = (float *)take(f[8] * 4);
+        h->srb.RR = (float *)take(f[9] * 4); h->srb.RU = (float *)take(f[10] * 4); h->srb.bits = (int *)take(f[11] * 4);
+    }
     if (workspace_bytes >= pinmpc_ws_dense_bytes(nu, N, B)) {
         h->dA = (float *)take(st * NX * NX * 4);
         h->dB = (float *)take(st * NX * nu * 4);
@@ -144,6 +171,14 @@ extern "C" pinmpc_status pinmpc_set_method(pinmpc_t h, pinmpc_method m)
     if (m != PINMPC_METHOD_AUTO && m != PINMPC_METHOD_DENSE && m != PINMPC_METHOD_SRB)
         return set_err(h, PINMPC_EINVAL, "pinmpc_set_method: unknown method");
     h->method = m;
+    return PINMPC_OK;
+}
+
+extern "C" pinmpc_status pinmpc_set_tuning(pinmpc_t h, int envs_per_cta)
+{
+    if (!h) return PINMPC_EINVAL;
+    if (envs_per_cta < 0 || envs_per_cta > 4) return set_err(h, PINMPC_EINVAL, "pinmpc_set_tuning: envs_per_cta must be 0 (auto) .. 4");
+    h->envs_per_cta = envs_per_cta;
     return PINMPC_OK;
 }
 

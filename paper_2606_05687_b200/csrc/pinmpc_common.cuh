@@ -36,6 +36,25 @@ struct DensePtrs {       // dense variant: materialised dynamics and Riccati fac
     float *K, *Minv, *s, *kappa;      // [B,N,nu,13], [B,N,nu,nu], [B,N,13], [B,N,nu]
 };
 
+// Structured (SRB) variant: per-stage factors kept in the workspace between the assembly,
+// factorisation and iteration kernels (st = B*N stages).  "Pass" arrays are env-major and copied
+// verbatim into shared memory; "stage" arrays are component-major [comp][st] so that threads
+// mapped lane = stage read and write them coalesced.
+struct SrbWs {
+    float *Kh;     // [st][6][12]    gain of the 6-D-input LQR, columns 0..11
+    float *qv;     // [B][N+1][12]   q_k = Q xbar_k (k = 1..N), q_0 = 0
+    float *c6;     // [st][6]        ch = (dt I_w^-1 tau_ext ; dt/m F_ext)   (zeros without ext_wrench)
+    float *sv;     // [st][12]       s_k = P_{k+1} E ch                      (zeros without ext_wrench)
+    float *cs;     // [st][2]        cos, sin of the linearisation yaw
+    float *MI;     // [21][st]       S_k after assembly, Mh_k^-1 after factorisation (packed symmetric)
+    float *KG;     // [6][st]        Kh[:,12] * x_12  (the constant gravity state's share of w)
+    float *LI;     // [21][st]       Lam_k^-1 (packed symmetric)
+    float *IW;     // [6][st]        I_w (packed symmetric 3x3)
+    float *RR;     // [3*nc][st]     contact offsets
+    float *RU;     // [nu][st]       R ubar
+    int *bits;     // [st]           contact flags
+};
+
 struct pinmpc_ctx {
     int nx, nu, N, B;
     pinmpc_layout layout;
@@ -53,6 +72,8 @@ struct pinmpc_ctx {
     // carved from the workspace
     OutPtrs out;
     float *dA, *dB, *dC, *dK, *dMinv, *dS, *dKappa;   // dense-only (NULL when the workspace is the small one)
+    SrbWs srb;
+    int envs_per_cta;        // tuning knob of the structured solver (0 = auto)
     int sm_count, smem_optin;
     int launch_count;
     cudaError_t sticky;
@@ -66,7 +87,7 @@ size_t pinmpc_ws_dense_bytes(int nu, int N, int B);
 int pinmpc_launch_assemble_dense(pinmpc_ctx *h, float *A, float *Bm, float *c, cudaStream_t st);
 int pinmpc_launch_solve_dense(pinmpc_ctx *h, cudaStream_t st);
 int pinmpc_launch_solve_srb(pinmpc_ctx *h, cudaStream_t st);
-size_t pinmpc_srb_smem_bytes(int nu, int N);
+size_t pinmpc_ws_srb_bytes(int nu, int N, int B);
 
 static inline SolveParams make_params(const pinmpc_ctx *h)
 {

@@ -1,54 +1,44 @@
 // pinmpc_srb.cu — the STRUCTURED on-chip solver (PINMPC_METHOD_SRB), the product path.
 //
-// One fused kernel per solve: dynamics assembly (S1), Riccati factorisation (S2) and all ADMM
-// iterations (S3-S6) of one env run inside one warp with every iteration-invariant factor resident
-// in shared memory.  A_k and B_k are never formed ("construction-free"):
-// the single-rigid-body structure of BASELINE.json config 0 (SRB form of PAPER.md eq. (2)-(4))
+// A_k and B_k are never formed ("construction-free"): the single-rigid-body
+// structure of BASELINE.json config 0 (SRB form of PAPER.md eq. (2)-(4))
 //     A_k = I + dt [Theta <- R_z^T omega, p <- v, v_z <- g],     B_k = E Bh_k,
 //     E = rows 6..11 (omega, v),   Bh_k = D_k Gh_k,   D_k = blkdiag(dt I_w^-1, dt/m I),
 //     Gh_k u = (sum_i r_i x f_i + sum_i m_i ;  sum_i f_i)          (net wrench about the CoM)
 // lets the equality-constrained step (21a) be solved EXACTLY as an LQR in the 6-D input
 // w = Bh_k u (the momentum increment) instead of the nu-D input u:
-//   for given w the best u is  u = u0 + Rt^-1 Bh^T S (w - Bh u0),  u0 = Rt^-1 r,  S = (Bh Rt^-1 Bh^T)^-1
-//   and its cost is 1/2 (w - w0)^T S (w - w0) + const, so with P_N = Q, for k = N-1..0
+//   for given w the best u is  u = u0 + Rt^-1 Gh^T Lam^-1 (D^-1 w - Gh u0),  u0 = Rt^-1 r,
+//   Lam = Gh Rt^-1 Gh^T, and its cost is 1/2 (w - w0)^T S (w - w0) + const, S = D^-1 Lam^-1 D^-1,
+//   so with P_N = Q, for k = N-1..0
 //     Mh = S_k + E^T P E,  Kh = Mh^-1 E^T P A_k (6x13),  P <- [k>=1] Q + A^T P A - G^T Kh,  G = E^T P A
-//   backward  g = p - s;  hh = S w0 + E^T g;  kap = Mh^-1 hh;  p <- q + A^T g - Kh^T hh
-//   forward   w = -Kh x + kap;  x+ = A x + E (w + ch);  u = u0 + Rt^-1 Gh^T Lam^-1 (D^-1 w - Gh u0)
-// with Lam = Gh Rt^-1 Gh^T (well conditioned; S = D^-1 Lam^-1 D^-1).  The value function P_k and
-// the iterates (x,u) equal those of the dense recursion of SURVEY.md 8(c)-O2/O3 (the oracle) up to
-// rounding; only 6x13 + 2 symmetric 6x6 blocks per stage are dense.
+//   backward  g = p - s;  hh = S w0 + E^T g;  p <- q + A^T g - Kh^T hh;   kappa = Mh^-1 hh
+//   forward   w = kappa - Kh x;  x+ = A x + E (w + ch)
+// The value function P_k and the iterates (x,u) equal those of the dense recursion of SURVEY.md
+// 8(c)-O2/O3 (the oracle) up to rounding.
 //
-// Mapping (v1): CTA = one warp = one env.  Sequential passes: lane j owns row j of x / p.
-// Stage-parallel phases (projection S4, dual update S5, residuals S6, u reconstruction): lane = stage.
+// Three kernels per solve:
+//   k_assemble_srb  S1   one thread per (env, stage): geometry, Lam^-1, S, R ubar, Q xbar, ch
+//   k_factor_srb    S2   one warp per env: the 13-state Riccati recursion in the 6-D input
+//   k_iterate_srb   S3-6 one CTA per G envs, all ADMM iterations with every factor on chip:
+//                        Kh and the exchange vectors in shared memory, the per-stage symmetric blocks,
+//                        z and y in the registers of the thread that owns the stage (lane = stage);
+//                        the two sequential passes run in warp 0, 8 lanes per env.
 #include "pinmpc_common.cuh"
 
 namespace {
 
 constexpr int NW = 2;   // 6-D wrench contacts (feet)
+constexpr unsigned FULL = 0xffffffffu;
 
 __host__ __device__ constexpr int sidx(int i, int j)   // packed upper triangle of a symmetric 6x6
 {
     return i <= j ? (i * 6 - i * (i - 1) / 2 + (j - i)) : (j * 6 - j * (j - 1) / 2 + (i - j));
 }
 
-template <int NU>
-struct Lay {
-    static constexpr int NF = (NU - 12) / 3;
-    static constexpr int NC = NW + NF;
-    // per-stage strides in floats (odd where lanes index by stage, to stay bank-conflict free)
-    static constexpr int KB = 104;        // [13][8]: Kh[0..5][j], q_j, s_j
-    static constexpr int MI = 21;         // S_k during factorisation, then Mh_k^-1 (packed)
-    static constexpr int LI = 21;         // Lam_k^-1 (packed)
-    static constexpr int IW = 9;          // I_w packed (6), cos, sin, contact bits
-    static constexpr int RR = 3 * NC + 1; // contact offsets r_i (7 / 13)
-    static constexpr int RU = NU + 1;     // R ubar
-    static constexpr int ZY = NU + 1;     // z, y (each)
-    static constexpr int V6 = 7;          // 6-vectors: sigma0, hh/kappa, w, ch
-    static constexpr int PER_STAGE = KB + MI + LI + IW + RR + RU + 2 * ZY + 4 * V6;
-    static constexpr int FIXED = 3 * 172 + 80 + 80 + 40;   // P, X, Y (13x13), G, Kh (6x13), Mh (6x6)
-};
+__device__ __forceinline__ int fcol(int i) { return i < NW ? 3 * i : 6 * NW + 3 * (i - NW); }
+__device__ __forceinline__ int mcol(int i) { return 3 * NW + 3 * i; }
 
-// y = M x for packed symmetric 6x6
+// y = M x for packed symmetric 6x6 held in registers
 __device__ __forceinline__ void symv6(const float *M, const float *x, float *y)
 {
 #pragma unroll
@@ -60,7 +50,7 @@ __device__ __forceinline__ void symv6(const float *M, const float *x, float *y)
     }
 }
 
-// In-place inverse of a packed symmetric positive definite 6x6 (Cholesky, registers only).
+// In-place inverse of a packed symmetric positive definite 6x6 (Cholesky, registers of one thread).
 __device__ __forceinline__ void spd_inv6(float *Mp)
 {
     float L[6][6], Li[6][6];
@@ -79,7 +69,6 @@ __device__ __forceinline__ void spd_inv6(float *Mp)
             L[i][j] = a * idj;
         }
     }
-    // Li = L^-1 (lower triangular)
 #pragma unroll
     for (int c = 0; c < 6; c++) {
         Li[c][c] = 1.0f / L[c][c];
@@ -91,7 +80,6 @@ __device__ __forceinline__ void spd_inv6(float *Mp)
             Li[i][c] = a / L[i][i];
         }
     }
-    // M^-1 = Li^T Li
 #pragma unroll
     for (int i = 0; i < 6; i++)
 #pragma unroll
@@ -103,38 +91,21 @@ __device__ __forceinline__ void spd_inv6(float *Mp)
         }
 }
 
-template <int NU>
-struct StageView {      // pointers into one env's shared-memory arena
-    float *KB, *MI, *LI, *IW, *RR, *RU, *ZZ, *YY, *S0, *KP, *WV, *CE, *P, *X, *Y, *G, *Kh, *Mh;
-    __device__ StageView(float *base, int N)
-    {
-        using L = Lay<NU>;
-        float *p = base;
-        KB = p; p += (size_t)N * L::KB;
-        MI = p; p += (size_t)N * L::MI;
-        LI = p; p += (size_t)N * L::LI;
-        IW = p; p += (size_t)N * L::IW;
-        RR = p; p += (size_t)N * L::RR;
-        RU = p; p += (size_t)N * L::RU;
-        ZZ = p; p += (size_t)N * L::ZY;
-        YY = p; p += (size_t)N * L::ZY;
-        S0 = p; p += (size_t)N * L::V6;
-        KP = p; p += (size_t)N * L::V6;
-        WV = p; p += (size_t)N * L::V6;
-        CE = p; p += (size_t)N * L::V6;
-        P = p; p += 172; X = p; p += 172; Y = p; p += 172; G = p; p += 80; Kh = p; p += 80; Mh = p;
-    }
-};
+// D^-1 v = (I_w v_tau / dt ; m v_F / dt) with I_w packed symmetric 3x3 (xx,xy,xz,yy,yz,zz)
+__device__ __forceinline__ void dinv_apply(const float *Iw, float idt, float m_dt, const float *v, float *o)
+{
+    o[0] = (Iw[0] * v[0] + Iw[1] * v[1] + Iw[2] * v[2]) * idt;
+    o[1] = (Iw[1] * v[0] + Iw[3] * v[1] + Iw[4] * v[2]) * idt;
+    o[2] = (Iw[2] * v[0] + Iw[4] * v[1] + Iw[5] * v[2]) * idt;
+    o[3] = v[3] * m_dt; o[4] = v[4] * m_dt; o[5] = v[5] * m_dt;
+}
 
-__device__ __forceinline__ int fcol(int i) { return i < NW ? 3 * i : 6 * NW + 3 * (i - NW); }
-__device__ __forceinline__ int mcol(int i) { return 3 * NW + 3 * i; }
-
-// u0 = Rt^-1 (R ubar + rho (z - y)) and its net wrench G0 = Gh u0 for one stage (lane-local)
+// u0 = Rt^-1 (R ubar + rho (z - y)) and its net wrench G0 = Gh u0 for one stage (thread-local)
 template <int NU>
 __device__ __forceinline__ void stage_u0(const SolveParams &P, const float *ru, const float *z, const float *y,
                                          const float *r, float *u0, float *G0)
 {
-    constexpr int NC = Lay<NU>::NC;
+    constexpr int NC = NW + (NU - 12) / 3;
 #pragma unroll
     for (int j = 0; j < NU; j++) u0[j] = (ru[j] + P.rho * (z[j] - y[j])) / (P.Rd[j] + P.rho);
 #pragma unroll
@@ -154,340 +125,493 @@ __device__ __forceinline__ void stage_u0(const SolveParams &P, const float *ru, 
     }
 }
 
-// D^-1 v = (I_w v_tau / dt ; m v_F / dt) with I_w packed symmetric 3x3 (xx,xy,xz,yy,yz,zz)
-__device__ __forceinline__ void dinv_apply(const float *Iw, float idt, float m_dt, const float *v, float *o)
+// ---------------------------------------------------------------------------------------------
+// S1  construction-free assembly: one thread per (env, stage)
+// ---------------------------------------------------------------------------------------------
+template <int NU>
+__global__ void __launch_bounds__(128) k_assemble_srb(SolveParams P, ProblemPtrs q, SrbWs W)
 {
-    o[0] = (Iw[0] * v[0] + Iw[1] * v[1] + Iw[2] * v[2]) * idt;
-    o[1] = (Iw[1] * v[0] + Iw[3] * v[1] + Iw[4] * v[2]) * idt;
-    o[2] = (Iw[2] * v[0] + Iw[4] * v[1] + Iw[5] * v[2]) * idt;
-    o[3] = v[3] * m_dt; o[4] = v[4] * m_dt; o[5] = v[5] * m_dt;
+    constexpr int NC = NW + (NU - 12) / 3;
+    const long st = (long)P.B * P.N;
+    const long s = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= st) return;
+    const int N = P.N;
+    const int b = (int)(s / N), k = (int)(s - (long)b * N);
+    const float dt = P.dt, idt = 1.0f / P.dt;
+    const float mass = q.mass[b], dtm = dt / mass, m_dt = mass / dt;
+
+    float Ib[9];
+#pragma unroll
+    for (int i = 0; i < 9; i++) Ib[i] = q.inertia[(long)b * 9 + i];
+    float sn, cs;
+    sincosf(q.yaw[s], &sn, &cs);
+    W.cs[s * 2] = cs; W.cs[s * 2 + 1] = sn;
+    // I_w = R_z I_b R_z^T (same congruence as world_inertia_inv, applied to I_b)
+    float Iwf[9];
+    world_inertia_inv(Ib, cs, sn, Iwf);
+    const float iw[6] = { Iwf[0], Iwf[1], Iwf[2], Iwf[4], Iwf[5], Iwf[8] };
+#pragma unroll
+    for (int i = 0; i < 6; i++) W.IW[i * st + s] = iw[i];
+
+    int bits = 0;
+    float r[3 * NC];
+#pragma unroll
+    for (int i = 0; i < NC; i++) {
+        bits |= (q.contact[s * NC + i] != 0) << i;
+#pragma unroll
+        for (int a = 0; a < 3; a++) {
+            r[3 * i + a] = q.foot_r[(s * NC + i) * 3 + a];
+            W.RR[(3 * i + a) * st + s] = r[3 * i + a];
+        }
+    }
+    W.bits[s] = bits;
+#pragma unroll
+    for (int j = 0; j < NU; j++) W.RU[j * st + s] = q.u_ref ? P.Rd[j] * q.u_ref[s * NU + j] : 0.0f;
+    // q_{k+1} = Q xbar_{k+1}  (x_ref[b,k] holds xbar_{k+1});  q_0 = 0
+    {
+        float *qv = W.qv + ((long)b * (N + 1) + k + 1) * 12;
+#pragma unroll
+        for (int j = 0; j < 12; j++) qv[j] = P.Qd[j] * q.x_ref[s * NX + j];
+        if (k == 0) {
+            float *q0 = W.qv + (long)b * (N + 1) * 12;
+#pragma unroll
+            for (int j = 0; j < 12; j++) q0[j] = 0.0f;
+        }
+    }
+    // Lam = Gh Rt^-1 Gh^T, accumulated column by column of Gh
+    float Lam[21];
+#pragma unroll
+    for (int i = 0; i < 21; i++) Lam[i] = 0.0f;
+#pragma unroll
+    for (int i = 0; i < NC; i++) {
+        float rx = r[3 * i], ry = r[3 * i + 1], rz = r[3 * i + 2];
+        const float col[3][3] = { { 0.0f, rz, -ry }, { -rz, 0.0f, rx }, { ry, -rx, 0.0f } };   // r x e_a
+#pragma unroll
+        for (int a = 0; a < 3; a++) {
+            float w = 1.0f / (P.Rd[fcol(i) + a] + P.rho);
+            float g6[6] = { col[a][0], col[a][1], col[a][2], a == 0 ? 1.0f : 0.0f, a == 1 ? 1.0f : 0.0f, a == 2 ? 1.0f : 0.0f };
+#pragma unroll
+            for (int x = 0; x < 6; x++)
+#pragma unroll
+                for (int y = x; y < 6; y++) Lam[sidx(x, y)] = fmaf(w * g6[x], g6[y], Lam[sidx(x, y)]);
+            if (i < NW) Lam[sidx(a, a)] += 1.0f / (P.Rd[mcol(i) + a] + P.rho);
+        }
+    }
+    spd_inv6(Lam);                                   // Lam^-1
+#pragma unroll
+    for (int i = 0; i < 21; i++) W.LI[i * st + s] = Lam[i];
+    // S = D^-1 Lam^-1 D^-1,  D^-1 = blkdiag(I_w / dt, m/dt I)
+    {
+        const float Iw3[3][3] = { { iw[0], iw[1], iw[2] }, { iw[1], iw[3], iw[4] }, { iw[2], iw[4], iw[5] } };
+        float T[3][3], S[21];
+#pragma unroll
+        for (int x = 0; x < 3; x++)
+#pragma unroll
+            for (int y = 0; y < 3; y++) {
+                float a = 0.0f;
+#pragma unroll
+                for (int l = 0; l < 3; l++) a = fmaf(Iw3[x][l], Lam[sidx(l, y)], a);
+                T[x][y] = a;
+            }
+#pragma unroll
+        for (int x = 0; x < 3; x++)
+#pragma unroll
+            for (int y = x; y < 3; y++) {
+                float a = 0.0f;
+#pragma unroll
+                for (int l = 0; l < 3; l++) a = fmaf(T[x][l], Iw3[l][y], a);
+                S[sidx(x, y)] = a * idt * idt;
+            }
+#pragma unroll
+        for (int x = 0; x < 3; x++)
+#pragma unroll
+            for (int y = 0; y < 3; y++) {
+                float a = 0.0f;
+#pragma unroll
+                for (int l = 0; l < 3; l++) a = fmaf(Iw3[x][l], Lam[sidx(l, 3 + y)], a);
+                S[sidx(x, 3 + y)] = a * idt * m_dt;
+            }
+#pragma unroll
+        for (int x = 0; x < 3; x++)
+#pragma unroll
+            for (int y = x; y < 3; y++) S[sidx(3 + x, 3 + y)] = Lam[sidx(3 + x, 3 + y)] * m_dt * m_dt;
+#pragma unroll
+        for (int i = 0; i < 21; i++) W.MI[i * st + s] = S[i];
+    }
+    // ch = (dt I_w^-1 tau_ext ; dt/m F_ext): the part of c_k in rows 6..11
+    if (q.ext != nullptr) {
+        float Ibi[9], Wi[9];
+        inv3f(Ib, Ibi);
+        world_inertia_inv(Ibi, cs, sn, Wi);
+        const float *e = q.ext + s * 6;
+#pragma unroll
+        for (int a = 0; a < 3; a++) {
+            W.c6[s * 6 + a] = dt * (Wi[a * 3] * e[3] + Wi[a * 3 + 1] * e[4] + Wi[a * 3 + 2] * e[5]);
+            W.c6[s * 6 + 3 + a] = dtm * e[a];
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// S2  factorisation: one warp per env, sequential over stages, P (13x13) in shared memory
+// ---------------------------------------------------------------------------------------------
+constexpr int FAC_WARPS = 4;                     // warps (envs) per CTA
+constexpr int FAC_SMEM = 172 + 172 + 80 + 24;    // floats per warp: P, X, Kh, Mh^-1
+
+// element (i,j) of A^T X for the structured A (rows 6..12 of A^T pick up dt * rows of X)
+__device__ __forceinline__ float atx(const float *X, int i, int j, float dt, float cs, float sn)
+{
+    float a = X[i * NX + j];
+    if (i == 6) a += dt * (cs * X[0 * NX + j] - sn * X[1 * NX + j]);
+    else if (i == 7) a += dt * (sn * X[0 * NX + j] + cs * X[1 * NX + j]);
+    else if (i == 8) a += dt * X[2 * NX + j];
+    else if (i >= 9 && i <= 11) a += dt * X[(i - 6) * NX + j];
+    else if (i == 12) a += dt * X[11 * NX + j];
+    return a;
+}
+
+__global__ void __launch_bounds__(FAC_WARPS * 32) k_factor_srb(SolveParams P, const float *__restrict__ x0, SrbWs W, int has_ext)
+{
+    __shared__ __align__(16) float sm_all[FAC_WARPS * FAC_SMEM];
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    const int b = blockIdx.x * FAC_WARPS + wib;
+    if (b >= P.B) return;
+    float *sP = sm_all + wib * FAC_SMEM, *sX = sP + 172, *sK = sX + 172, *sM = sK + 80;
+    const int N = P.N;
+    const long st = (long)P.B * N;
+    const float dt = P.dt;
+    const float x12 = x0[(long)b * NX + 12];
+
+    // lane <-> (i,j) of the packed symmetric 6x6 (lanes >= 21 shadow element (0,0))
+    int mi = 0, mj = 0;
+    {
+        int l = lane < 21 ? lane : 0, row = 0;
+        while (l >= 6 - row) { l -= 6 - row; row++; }
+        mi = row; mj = row + l;
+    }
+    int la[6], lb[6];
+#pragma unroll
+    for (int p = 0; p < 6; p++) { la[p] = sidx(mi, p); lb[p] = sidx(p, mj); }
+    // upper triangle of the 13x13: element t = lane + 32 r  ->  (ti, tj), ti <= tj
+    int ti[3], tj[3];
+#pragma unroll
+    for (int r = 0; r < 3; r++) {
+        int t = lane + 32 * r, row = 0;
+        if (t > 90) t = 90;
+        while (t >= NX - row) { t -= NX - row; row++; }
+        ti[r] = row; tj[r] = row + t;
+    }
+
+    for (int i = lane; i < 169; i += 32) sP[i] = ((i * 79) >> 10) * 14 == i ? P.Qd[(i * 79) >> 10] : 0.0f;
+    __syncwarp();
+
+    // prefetch stage N-1
+    long s = (long)b * N + N - 1;
+    float cs_n = W.cs[s * 2], sn_n = W.cs[s * 2 + 1];
+    float S_n = W.MI[(long)(lane < 21 ? lane : 0) * st + s];
+    float ch_n = (has_ext && lane < 6) ? W.c6[s * 6 + lane] : 0.0f;
+    for (int k = N - 1; k >= 0; k--) {
+        s = (long)b * N + k;
+        const float cs = cs_n, sn = sn_n, Sl = S_n, chl = ch_n;
+        if (k > 0) {
+            cs_n = W.cs[(s - 1) * 2]; sn_n = W.cs[(s - 1) * 2 + 1];
+            S_n = W.MI[(long)(lane < 21 ? lane : 0) * st + s - 1];
+            ch_n = (has_ext && lane < 6) ? W.c6[(s - 1) * 6 + lane] : 0.0f;
+        }
+        // X = P A
+#pragma unroll
+        for (int r = 0; r < 6; r++) {
+            int e = lane + 32 * r;
+            if (e < 169) {
+                int i = (e * 79) >> 10, j = e - i * NX;
+                const float *Pi = sP + i * NX;
+                float a = Pi[j];
+                if (j == 6) a += dt * (cs * Pi[0] - sn * Pi[1]);
+                else if (j == 7) a += dt * (sn * Pi[0] + cs * Pi[1]);
+                else if (j == 8) a += dt * Pi[2];
+                else if (j >= 9 && j <= 11) a += dt * Pi[j - 6];
+                else if (j == 12) a += dt * Pi[11];
+                sX[e] = a;
+            }
+        }
+        // Mh = S + P[6:12,6:12] (one packed element per lane) ; s_k = P (E ch)
+        float M = Sl + sP[(6 + mi) * NX + 6 + mj];
+        float sk = 0.0f;
+        if (has_ext) {
+            const int rl = lane < NX ? lane : 0;
+#pragma unroll
+            for (int a = 0; a < 6; a++) sk = fmaf(sP[rl * NX + 6 + a], __shfl_sync(FULL, chl, a), sk);
+        }
+        // Mh^-1 by symmetric sweeps (-Mh^-1 after six pivots), all in registers
+#pragma unroll
+        for (int p = 0; p < 6; p++) {
+            float d = __shfl_sync(FULL, M, sidx(p, p));
+            float a = __shfl_sync(FULL, M, la[p]);
+            float c = __shfl_sync(FULL, M, lb[p]);
+            float id = 1.0f / d;
+            if (mi == p && mj == p) M = -id;
+            else if (mi == p || mj == p) M = M * id;
+            else M = fmaf(-a * id, c, M);
+        }
+        M = -M;
+        if (lane < 21) { sM[lane] = M; W.MI[(long)lane * st + s] = M; }
+        __syncwarp();
+        // Kh = Mh^-1 X[6:12,:]
+#pragma unroll
+        for (int r = 0; r < 3; r++) {
+            int e = lane + 32 * r;
+            if (e < 78) {
+                int i = (e * 79) >> 10, j = e - i * NX;
+                float a = 0.0f;
+#pragma unroll
+                for (int l = 0; l < 6; l++) a = fmaf(sM[sidx(i, l)], sX[(6 + l) * NX + j], a);
+                sK[e] = a;
+                if (j < 12) W.Kh[s * 72 + i * 12 + j] = a;
+                else W.KG[(long)i * st + s] = a * x12;
+            }
+        }
+        if (has_ext && lane < 12) W.sv[s * 12 + lane] = sk;
+        __syncwarp();
+        // P <- [k>=1] Q + A^T X - G^T Kh   (upper triangle, mirrored: both terms are symmetric)
+#pragma unroll
+        for (int r = 0; r < 3; r++) {
+            if (lane + 32 * r < 91) {
+                int i = ti[r], j = tj[r];
+                float a = atx(sX, i, j, dt, cs, sn);
+#pragma unroll
+                for (int l = 0; l < 6; l++) a = fmaf(-sX[(6 + l) * NX + i], sK[l * NX + j], a);
+                if (k >= 1 && i == j) a += P.Qd[i];
+                sP[i * NX + j] = a;
+                sP[j * NX + i] = a;
+            }
+        }
+        __syncwarp();
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// S3-S6  ADMM iterations: one CTA per G envs, every factor on chip
+// ---------------------------------------------------------------------------------------------
+// Shared-memory arena of one env (offsets in floats).  The arena stride is 8 mod 32 so that the
+// 8-lane groups of up to four envs in the pass warp hit disjoint banks.
+struct ArenaLay { int oQ, oX, oCS, oM, oC, oS, oF, stride; };
+
+__host__ __device__ inline ArenaLay arena_layout(int N, int ext)
+{
+    ArenaLay L;
+    L.oQ = 72 * N;                    // Kh [N][6][12] at 0 ; q [N+1][12]
+    L.oX = L.oQ + 12 * (N + 1);       // exchange vector [N][8]: sigma0 -> hh -> kappa -> w
+    L.oCS = L.oX + 8 * N;             // cos, sin [N][2]
+    L.oM = L.oCS + 2 * N;             // Mh^-1 (21) and kg (6) per stage, stride 27 (lane = stage)
+    L.oC = L.oM + 27 * N;             // ch [N][6]      (ext only)
+    L.oS = L.oC + (ext ? 6 * N : 0);  // s  [N][12]     (ext only)
+    L.oF = (L.oS + (ext ? 12 * N : 0) + 3) & ~3;   // forward-pass exchange scratch [2][8]
+    int size = L.oF + 16;
+    L.stride = size + ((8 - (size & 31)) & 31);
+    return L;
+}
+
+constexpr int CTL_INTS = 32;          // done[4] | ndone | pad[3] | red[4][5]
+
+// Backward vector pass of all envs of the CTA (warp 0; lane = 8 e + i, lanes i < 6 own the
+// columns i (Theta/p part) and 6 + i (omega/v part) of p).
+__device__ __forceinline__ void backward_pass(const ArenaLay &L, float *smem, int N, int Gv, float dt, int has_ext, int lane)
+{
+    const int e = lane >> 3, i0 = lane & 7, i = i0 < 6 ? i0 : 5;
+    const bool act = i0 < 6 && e < Gv;
+    float *ar = smem + (e < Gv ? e : 0) * L.stride;
+    const float *aQ = ar + L.oQ, *aCS = ar + L.oCS, *aS = ar + L.oS;
+    float *aX = ar + L.oX;
+    float pq = aQ[N * 12 + i], pv = aQ[N * 12 + 6 + i];
+    for (int k = N - 1; k >= 0; k--) {
+        const float *Kk = ar + k * 72;
+        float kq[6], kv[6];
+#pragma unroll
+        for (int r = 0; r < 6; r++) { kq[r] = Kk[r * 12 + i]; kv[r] = Kk[r * 12 + 6 + i]; }
+        const float qq = aQ[k * 12 + i], qn = aQ[k * 12 + 6 + i];
+        const float s0 = aX[k * 8 + i];
+        const float csk = aCS[2 * k], snk = aCS[2 * k + 1];
+        float sq = 0.0f, sn6 = 0.0f;
+        if (has_ext) { sq = aS[k * 12 + i]; sn6 = aS[k * 12 + 6 + i]; }
+        const float gq = pq - sq, gv = pv - sn6;
+        const float hh = s0 + gv;
+        if (act) aX[k * 8 + i] = hh;
+        const float oth = __shfl_xor_sync(FULL, gq, 1);
+        __syncwarp();
+        const float4 h0 = *reinterpret_cast<const float4 *>(aX + k * 8);
+        const float2 h1 = *reinterpret_cast<const float2 *>(aX + k * 8 + 4);
+        float a0 = kq[0] * h0.x, a1 = kq[3] * h0.w, b0 = kv[0] * h0.x, b1 = kv[3] * h0.w;
+        a0 = fmaf(kq[1], h0.y, a0); a1 = fmaf(kq[4], h1.x, a1); b0 = fmaf(kv[1], h0.y, b0); b1 = fmaf(kv[4], h1.x, b1);
+        a0 = fmaf(kq[2], h0.z, a0); a1 = fmaf(kq[5], h1.y, a1); b0 = fmaf(kv[2], h0.z, b0); b1 = fmaf(kv[5], h1.y, b1);
+        // (A^T g)_nu = g_nu + dt (R_z g_Theta ; g_p)
+        const float ca = i < 2 ? csk : 1.0f, cb = i == 0 ? -snk : (i == 1 ? snk : 0.0f);
+        const float rot = fmaf(cb, oth, ca * gq);
+        pq = (qq + gq) - (a0 + a1);
+        pv = fmaf(dt, rot, qn + gv) - (b0 + b1);
+    }
+}
+
+// Forward rollout of all envs of the CTA (warp 0; every active lane holds the whole state, lane i
+// owns row i of Kh and the new omega/v component i).  Writes w_k over kappa_k; optionally emits x.
+__device__ __forceinline__ void forward_pass(const ArenaLay &L, float *smem, int N, int Gv, float dt, int has_ext, int lane,
+                                             const float *__restrict__ x0g, int b0, bool emit, const int *done, float *ox)
+{
+    const int e = lane >> 3, i0 = lane & 7, i = i0 < 6 ? i0 : 5;
+    const bool act = i0 < 6 && e < Gv;
+    const int ee = e < Gv ? e : 0;
+    float *ar = smem + ee * L.stride;
+    const float *aCS = ar + L.oCS, *aC = ar + L.oC;
+    float *aX = ar + L.oX, *aF = ar + L.oF;
+    const float *xg = x0g + (long)(b0 + ee) * NX;
+    float x0 = xg[0], x1 = xg[1], x2 = xg[2], x3 = xg[3], x4 = xg[4], x5 = xg[5];
+    float x6 = xg[6], x7 = xg[7], x8 = xg[8], x9 = xg[9], x10 = xg[10], x11 = xg[11];
+    const float x12 = xg[12];
+    float own = xg[6 + i];
+    const float gdt = i == 5 ? dt * x12 : 0.0f;
+    const bool wr = emit && act && !done[ee];
+    float *oxe = ox + (long)(b0 + ee) * N * NX;
+    int par = 0;
+    for (int k = 0; k < N; k++) {
+        const float4 *Kr = reinterpret_cast<const float4 *>(ar + k * 72 + i * 12);
+        const float4 r0 = Kr[0], r1 = Kr[1], r2 = Kr[2];
+        const float kap = aX[k * 8 + i];
+        const float csk = aCS[2 * k], snk = aCS[2 * k + 1];
+        const float c = (has_ext ? aC[k * 6 + i] : 0.0f) + gdt;
+        float a0 = r0.x * x0, a1 = r0.w * x3, a2 = r1.z * x6, a3 = r2.y * x9;
+        a0 = fmaf(r0.y, x1, a0); a1 = fmaf(r1.x, x4, a1); a2 = fmaf(r1.w, x7, a2); a3 = fmaf(r2.z, x10, a3);
+        a0 = fmaf(r0.z, x2, a0); a1 = fmaf(r1.y, x5, a1); a2 = fmaf(r2.x, x8, a2); a3 = fmaf(r2.w, x11, a3);
+        const float w = kap - ((a0 + a1) + (a2 + a3));
+        const float nun = own + (w + c);
+        if (act) { aX[k * 8 + i] = w; aF[par * 8 + i] = nun; }
+        // Theta+ = Theta + dt R_z^T omega ; p+ = p + dt v   (old omega, v)
+        x0 = fmaf(dt, fmaf(csk, x6, snk * x7), x0);
+        x1 = fmaf(dt, fmaf(csk, x7, -snk * x6), x1);
+        x2 = fmaf(dt, x8, x2); x3 = fmaf(dt, x9, x3); x4 = fmaf(dt, x10, x4); x5 = fmaf(dt, x11, x5);
+        __syncwarp();
+        const float4 n0 = *reinterpret_cast<const float4 *>(aF + par * 8);
+        const float2 n1 = *reinterpret_cast<const float2 *>(aF + par * 8 + 4);
+        x6 = n0.x; x7 = n0.y; x8 = n0.z; x9 = n0.w; x10 = n1.x; x11 = n1.y;
+        own = nun;
+        if (wr) {
+            const float xs = i == 0 ? x0 : i == 1 ? x1 : i == 2 ? x2 : i == 3 ? x3 : i == 4 ? x4 : x5;
+            oxe[k * NX + i] = xs;
+            oxe[k * NX + 6 + i] = nun;
+            if (i == 0) oxe[k * NX + 12] = x12;
+        }
+        par ^= 1;
+    }
 }
 
 template <int NU>
-__global__ void __launch_bounds__(32) k_solve_srb(SolveParams P, ProblemPtrs q, OutPtrs o)
+__global__ void __launch_bounds__(256) k_iterate_srb(SolveParams P, SrbWs W, const float *__restrict__ x0g,
+                                                     const float *__restrict__ massg, OutPtrs o, int G, int has_ext)
 {
-    using L = Lay<NU>;
-    constexpr int NC = L::NC;
-    constexpr unsigned FULL = 0xffffffffu;
+    constexpr int NC = NW + (NU - 12) / 3;
     extern __shared__ __align__(16) float smem[];
-    const int lane = threadIdx.x;
-    const int b = blockIdx.x;
-    const int N = P.N;
-    StageView<NU> V(smem, N);
+    const int N = P.N, tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, warp = tid >> 5;
+    const long st = (long)P.B * N;
+    const ArenaLay L = arena_layout(N, has_ext);
+    const int b0 = blockIdx.x * G;
+    const int Gv = min(G, P.B - b0);
+    int *ctl = reinterpret_cast<int *>(smem + G * L.stride);
+    int *done = ctl, *ndone = ctl + 4;
+    unsigned *red = reinterpret_cast<unsigned *>(ctl + 8);
     const float dt = P.dt, idt = 1.0f / P.dt;
-    const float mass = q.mass[b], dtm = dt / mass, m_dt = mass / dt;
-    const bool has_ext = q.ext != nullptr;
 
-    // ------------------------------------------------------------------------------------------
-    // S1  construction-free assembly: per-stage geometry, Lam^-1, S   (lane = stage)
-    // ------------------------------------------------------------------------------------------
-    float Ib[9], Ibi[9];
-#pragma unroll
-    for (int i = 0; i < 9; i++) Ib[i] = q.inertia[(long)b * 9 + i];
-    inv3f(Ib, Ibi);
-    for (int k = lane; k < N; k += 32) {
-        const long s = (long)b * N + k;
-        float sn, cs;
-        sincosf(q.yaw[s], &sn, &cs);
-        // I_w = R_z I_b R_z^T : same congruence as world_inertia_inv, applied to I_b
-        float Iwf[9];
-        world_inertia_inv(Ib, cs, sn, Iwf);
-        float *iw = V.IW + k * L::IW;
-        iw[0] = Iwf[0]; iw[1] = Iwf[1]; iw[2] = Iwf[2]; iw[3] = Iwf[4]; iw[4] = Iwf[5]; iw[5] = Iwf[8];
-        iw[6] = cs; iw[7] = sn;
-        int bits = 0;
-        float r[3 * NC];
-#pragma unroll
-        for (int i = 0; i < NC; i++) {
-            bits |= (q.contact[s * NC + i] != 0) << i;
-#pragma unroll
-            for (int a = 0; a < 3; a++) {
-                r[3 * i + a] = q.foot_r[(s * NC + i) * 3 + a];
-                V.RR[k * L::RR + 3 * i + a] = r[3 * i + a];
-            }
-        }
-        iw[8] = __int_as_float(bits);
-#pragma unroll
-        for (int j = 0; j < NU; j++) {
-            V.RU[k * L::RU + j] = q.u_ref ? P.Rd[j] * q.u_ref[s * NU + j] : 0.0f;
-            V.ZZ[k * L::ZY + j] = 0.0f;
-            V.YY[k * L::ZY + j] = 0.0f;
-        }
-        // Lam = Gh Rt^-1 Gh^T, accumulated column by column of Gh
-        float Lam[21];
-#pragma unroll
-        for (int i = 0; i < 21; i++) Lam[i] = 0.0f;
-#pragma unroll
-        for (int i = 0; i < NC; i++) {
-            float rx = r[3 * i], ry = r[3 * i + 1], rz = r[3 * i + 2];
-            const float col[3][3] = { { 0.0f, rz, -ry }, { -rz, 0.0f, rx }, { ry, -rx, 0.0f } };   // r x e_a
-#pragma unroll
-            for (int a = 0; a < 3; a++) {
-                float w = 1.0f / (P.Rd[fcol(i) + a] + P.rho);
-                float g6[6] = { col[a][0], col[a][1], col[a][2], a == 0 ? 1.0f : 0.0f, a == 1 ? 1.0f : 0.0f, a == 2 ? 1.0f : 0.0f };
-#pragma unroll
-                for (int x = 0; x < 6; x++)
-#pragma unroll
-                    for (int y = x; y < 6; y++) Lam[sidx(x, y)] = fmaf(w * g6[x], g6[y], Lam[sidx(x, y)]);
-                if (i < NW) Lam[sidx(a, a)] += 1.0f / (P.Rd[mcol(i) + a] + P.rho);
-            }
-        }
-        spd_inv6(Lam);                                   // Lam^-1
-#pragma unroll
-        for (int i = 0; i < 21; i++) V.LI[k * L::LI + i] = Lam[i];
-        // S = D^-1 Lam^-1 D^-1,  D^-1 = blkdiag(I_w / dt, m/dt I)
-        {
-            const float Iw3[3][3] = { { iw[0], iw[1], iw[2] }, { iw[1], iw[3], iw[4] }, { iw[2], iw[4], iw[5] } };
-            float T[3][3], S[21];
-            // tau-tau block: I_w V_tt I_w / dt^2
-#pragma unroll
-            for (int x = 0; x < 3; x++)
-#pragma unroll
-                for (int y = 0; y < 3; y++) {
-                    float a = 0.0f;
-#pragma unroll
-                    for (int l = 0; l < 3; l++) a = fmaf(Iw3[x][l], Lam[sidx(l, y)], a);
-                    T[x][y] = a;
-                }
-#pragma unroll
-            for (int x = 0; x < 3; x++)
-#pragma unroll
-                for (int y = x; y < 3; y++) {
-                    float a = 0.0f;
-#pragma unroll
-                    for (int l = 0; l < 3; l++) a = fmaf(T[x][l], Iw3[l][y], a);
-                    S[sidx(x, y)] = a * idt * idt;
-                }
-            // tau-F block: I_w V_tF m / dt^2 ; F-F block: V_FF m^2 / dt^2
-#pragma unroll
-            for (int x = 0; x < 3; x++)
-#pragma unroll
-                for (int y = 0; y < 3; y++) {
-                    float a = 0.0f;
-#pragma unroll
-                    for (int l = 0; l < 3; l++) a = fmaf(Iw3[x][l], Lam[sidx(l, 3 + y)], a);
-                    S[sidx(x, 3 + y)] = a * idt * m_dt;
-                }
-#pragma unroll
-            for (int x = 0; x < 3; x++)
-#pragma unroll
-                for (int y = x; y < 3; y++) S[sidx(3 + x, 3 + y)] = Lam[sidx(3 + x, 3 + y)] * m_dt * m_dt;
-#pragma unroll
-            for (int i = 0; i < 21; i++) V.MI[k * L::MI + i] = S[i];
-        }
-        // ch = (dt I_w^-1 tau_ext ; dt/m F_ext): the part of c_k in rows 6..11
-        float ch[6] = { 0, 0, 0, 0, 0, 0 };
+    // this thread's stage task: env te of the CTA, stage tk
+    const int te = tid / N, tk = tid - te * N;
+    const bool tact = te < Gv;
+    const int bb = b0 + (tact ? te : 0);
+    const long ts = (long)bb * N + tk;
+    float *ar = smem + (tact ? te : 0) * L.stride;
+    float *myX = ar + L.oX + tk * 8, *myM = ar + L.oM + tk * 27;
+
+    // ---- load the pass arrays of the CTA's envs into shared memory ------------------------------
+    for (int e = 0; e < Gv; e++) {
+        float *a = smem + e * L.stride;
+        const long s0 = (long)(b0 + e) * N;
+        const float4 *src = reinterpret_cast<const float4 *>(W.Kh + s0 * 72);
+        float4 *dst = reinterpret_cast<float4 *>(a);
+        for (int i = tid; i < N * 18; i += nthr) dst[i] = src[i];
+        src = reinterpret_cast<const float4 *>(W.qv + (long)(b0 + e) * (N + 1) * 12);
+        dst = reinterpret_cast<float4 *>(a + L.oQ);
+        for (int i = tid; i < (N + 1) * 3; i += nthr) dst[i] = src[i];
+        for (int i = tid; i < N * 2; i += nthr) a[L.oCS + i] = W.cs[s0 * 2 + i];
         if (has_ext) {
-            float Wi[9];
-            world_inertia_inv(Ibi, cs, sn, Wi);
-            const float *e = q.ext + s * 6;
-#pragma unroll
-            for (int a = 0; a < 3; a++) {
-                ch[a] = dt * (Wi[a * 3] * e[3] + Wi[a * 3 + 1] * e[4] + Wi[a * 3 + 2] * e[5]);
-                ch[3 + a] = dtm * e[a];
-            }
+            for (int i = tid; i < N * 6; i += nthr) a[L.oC + i] = W.c6[s0 * 6 + i];
+            for (int i = tid; i < N * 12; i += nthr) a[L.oS + i] = W.sv[s0 * 12 + i];
         }
-#pragma unroll
-        for (int a = 0; a < 6; a++) V.CE[k * L::V6 + a] = ch[a];
     }
-    __syncwarp();
+    if (tid < CTL_INTS) ctl[tid] = 0;
 
-    // ------------------------------------------------------------------------------------------
-    // S2  factorisation: P recursion in the 6-D input, warp-cooperative, sequential over stages
-    // ------------------------------------------------------------------------------------------
-    for (int i = lane; i < 169; i += 32) V.P[i] = (i / NX == i % NX) ? P.Qd[i / NX] : 0.0f;
-    __syncwarp();
-    for (int k = N - 1; k >= 0; k--) {
-        const float cs = V.IW[k * L::IW + 6], sn = V.IW[k * L::IW + 7];
-        // X = P A
-        for (int e = lane; e < 169; e += 32) {
-            int i = e / NX, j = e % NX;
-            const float *Pi = V.P + i * NX;
-            float a = Pi[j];
-            if (j == 6) a += dt * (cs * Pi[0] - sn * Pi[1]);
-            else if (j == 7) a += dt * (sn * Pi[0] + cs * Pi[1]);
-            else if (j == 8) a += dt * Pi[2];
-            else if (j >= 9 && j <= 11) a += dt * Pi[j - 6];
-            else if (j == 12) a += dt * Pi[11];
-            V.X[e] = a;
-        }
-        // Mh = S + P[6:12,6:12] ; s_k = P (E ch)
-        for (int e = lane; e < 36; e += 32) {
-            int i = e / 6, j = e % 6;
-            V.Mh[e] = V.MI[k * L::MI + sidx(i, j)] + V.P[(6 + i) * NX + 6 + j];
-        }
-        float sk = 0.0f;
-        if (lane < NX) {
+    // ---- stage-stationary registers (lane = stage) ---------------------------------------------
+    float LI[21], Iw[6], r[3 * NC], ru[NU], z[NU], y[NU];
+    int bits = 0;
+    float m_dt = 0.0f;
+    if (tact) {
 #pragma unroll
-            for (int a = 0; a < 6; a++) sk = fmaf(V.P[lane * NX + 6 + a], V.CE[k * L::V6 + a], sk);
-        }
-        __syncwarp();
-        // Mh^-1 (lane 0, registers) ; Y = A^T X ; G = X[6:12,:]
-        if (lane == 0) {
-            float M[21];
+        for (int c = 0; c < 21; c++) { LI[c] = W.LI[c * st + ts]; myM[c] = W.MI[c * st + ts]; }
 #pragma unroll
-            for (int i = 0; i < 6; i++)
+        for (int c = 0; c < 6; c++) { Iw[c] = W.IW[c * st + ts]; myM[21 + c] = W.KG[c * st + ts]; }
 #pragma unroll
-                for (int j = i; j < 6; j++) M[sidx(i, j)] = 0.5f * (V.Mh[i * 6 + j] + V.Mh[j * 6 + i]);
-            spd_inv6(M);
+        for (int c = 0; c < 3 * NC; c++) r[c] = W.RR[c * st + ts];
 #pragma unroll
-            for (int i = 0; i < 21; i++) V.MI[k * L::MI + i] = M[i];
-        }
-        for (int e = lane; e < 169; e += 32) {
-            int i = e / NX, j = e % NX;
-            float a = V.X[e];
-            if (i == 6) a += dt * (cs * V.X[0 * NX + j] - sn * V.X[1 * NX + j]);
-            else if (i == 7) a += dt * (sn * V.X[0 * NX + j] + cs * V.X[1 * NX + j]);
-            else if (i == 8) a += dt * V.X[2 * NX + j];
-            else if (i >= 9 && i <= 11) a += dt * V.X[(i - 6) * NX + j];
-            else if (i == 12) a += dt * V.X[11 * NX + j];
-            V.Y[e] = a;
-        }
-        __syncwarp();
-        // Kh = Mh^-1 G
-        for (int e = lane; e < 78; e += 32) {
-            int i = e / NX, j = e % NX;
-            float a = 0.0f;
-#pragma unroll
-            for (int l = 0; l < 6; l++) a = fmaf(V.MI[k * L::MI + sidx(i, l)], V.X[(6 + l) * NX + j], a);
-            V.Kh[e] = a;
-        }
-        __syncwarp();
-        // store the sequential block: Kh^T, q_k, s_k
-        if (lane < NX) {
-            float *kb = V.KB + k * L::KB + lane * 8;
-#pragma unroll
-            for (int i = 0; i < 6; i++) kb[i] = V.Kh[i * NX + lane];
-            kb[6] = (k >= 1) ? P.Qd[lane] * q.x_ref[((long)b * N + k - 1) * NX + lane] : 0.0f;
-            kb[7] = sk;
-        }
-        // Z = Y - G^T Kh  (into X's storage is unsafe: G lives there) -> into P after symmetrisation
-        float zloc[6];
-        int cnt = 0;
-        for (int e = lane; e < 169; e += 32, cnt++) {
-            int i = e / NX, j = e % NX;
-            float a = V.Y[e];
-#pragma unroll
-            for (int l = 0; l < 6; l++) a = fmaf(-V.X[(6 + l) * NX + i], V.Kh[l * NX + j], a);
-            zloc[cnt] = a;
-        }
-        __syncwarp();
-        cnt = 0;
-        for (int e = lane; e < 169; e += 32, cnt++) V.Y[e] = zloc[cnt];
-        __syncwarp();
-        for (int e = lane; e < 169; e += 32) {
-            int i = e / NX, j = e % NX;
-            V.P[e] = 0.5f * (V.Y[i * NX + j] + V.Y[j * NX + i]) + ((k >= 1 && i == j) ? P.Qd[i] : 0.0f);
-        }
-        __syncwarp();
+        for (int c = 0; c < NU; c++) { ru[c] = W.RU[c * st + ts]; z[c] = 0.0f; y[c] = 0.0f; }
+        bits = W.bits[ts];
+        m_dt = massg[bb] / dt;
     }
 
-    // ------------------------------------------------------------------------------------------
-    // S3-S6  ADMM iterations
-    // ------------------------------------------------------------------------------------------
-    // per-lane constants of the structured A: (A^T g)_j = g_j + ca g[sa] + cb g[sb], same for A x
-    int bsa = 0, bsb = 0, fsa = 0, fsb = 0;
-    float b_c1 = 0, b_cc = 0, b_cs = 0, b_dc = 0, b_ds = 0;      // backward: ca = b_c1 + b_cc cs + b_cs sn ; cb = b_dc cs + b_ds sn
-    float f_c1 = 0, f_cc = 0, f_cs = 0, f_dc = 0, f_ds = 0;
-    if (lane == 6) { bsa = 0; bsb = 1; b_cc = dt; b_ds = -dt; }
-    else if (lane == 7) { bsa = 0; bsb = 1; b_cs = dt; b_dc = dt; }
-    else if (lane >= 8 && lane <= 11) { bsa = lane - 6; b_c1 = dt; }
-    else if (lane == 12) { bsa = 11; b_c1 = dt; }
-    if (lane == 0) { fsa = 6; fsb = 7; f_cc = dt; f_ds = dt; }
-    else if (lane == 1) { fsa = 6; fsb = 7; f_cs = -dt; f_dc = dt; }
-    else if (lane >= 2 && lane <= 5) { fsa = lane + 6; f_c1 = dt; }
-    else if (lane == 11) { fsa = 12; f_c1 = dt; }
-    const int wsrc = (lane >= 6 && lane < 12) ? lane - 6 : 0;
-    const float Qd_l = lane < NX ? P.Qd[lane] : 0.0f;
-    const float x0_l = lane < NX ? q.x0[(long)b * NX + lane] : 0.0f;
-    const float pN_l = lane < NX ? Qd_l * q.x_ref[((long)b * N + N - 1) * NX + lane] : 0.0f;
-    const bool tol_mode = (P.eps_abs > 0.0f || P.eps_rel > 0.0f) && P.check_every > 0;
-
-    // sigma0 for the first iteration (z = y = 0)
-    auto stage_sigma0 = [&](int k) {
+    // sigma0 = D^-1 Lam^-1 Gh u0 of the coming iteration from the current z, y  (phase P1)
+    auto stage_sigma0 = [&]() {
         float u0[NU], G0[6], l0[6], s0[6];
-        stage_u0<NU>(P, V.RU + k * L::RU, V.ZZ + k * L::ZY, V.YY + k * L::ZY, V.RR + k * L::RR, u0, G0);
-        symv6(V.LI + k * L::LI, G0, l0);
-        dinv_apply(V.IW + k * L::IW, idt, m_dt, l0, s0);
-#pragma unroll
-        for (int a = 0; a < 6; a++) V.S0[k * L::V6 + a] = s0[a];
+        stage_u0<NU>(P, ru, z, y, r, u0, G0);
+        symv6(LI, G0, l0);
+        dinv_apply(Iw, idt, m_dt, l0, s0);
+        *reinterpret_cast<float4 *>(myX) = make_float4(s0[0], s0[1], s0[2], s0[3]);
+        *reinterpret_cast<float2 *>(myX + 4) = make_float2(s0[4], s0[5]);
     };
-    for (int k = lane; k < N; k += 32) stage_sigma0(k);
-    __syncwarp();
+    if (tact) stage_sigma0();
 
-    float rp = 0.0f, rd = 0.0f;
-    int done = 0;
+    const bool tol_mode = (P.eps_abs > 0.0f || P.eps_rel > 0.0f) && P.check_every > 0;
+    bool frozen = false;          // this thread's env has met the tolerances (tolerance mode only)
+
     for (int it = 0; it < P.iters; it++) {
         const bool is_check = tol_mode && ((it + 1) % P.check_every == 0);
         const bool emit = (it == P.iters - 1) || is_check;
-        // ---- backward vector pass (sequential over stages; lane j = row j) ----------------------
-        float p = pN_l;
-        for (int k = N - 1; k >= 0; k--) {
-            const float4 *kb4 = reinterpret_cast<const float4 *>(V.KB + k * L::KB + (lane < NX ? lane : 0) * 8);
-            float4 k0 = kb4[0], k1 = kb4[1];            // Kh[0..3][j] | Kh[4][j], Kh[5][j], q_j, s_j
-            const float cs = V.IW[k * L::IW + 6], sn = V.IW[k * L::IW + 7];
-            float g = p - k1.w;
-            float hh = g + ((lane >= 6 && lane < 12) ? V.S0[k * L::V6 + lane - 6] : 0.0f);   // lanes 6..11
-            if (lane >= 6 && lane < 12) V.KP[k * L::V6 + lane - 6] = hh;
-            float h0 = __shfl_sync(FULL, hh, 6), h1 = __shfl_sync(FULL, hh, 7), h2 = __shfl_sync(FULL, hh, 8);
-            float h3 = __shfl_sync(FULL, hh, 9), h4 = __shfl_sync(FULL, hh, 10), h5 = __shfl_sync(FULL, hh, 11);
-            float ga = __shfl_sync(FULL, g, bsa), gb = __shfl_sync(FULL, g, bsb);
-            float ca = fmaf(b_cc, cs, fmaf(b_cs, sn, b_c1)), cb = fmaf(b_dc, cs, b_ds * sn);
-            float acc = k1.z + g;
-            acc = fmaf(ca, ga, acc); acc = fmaf(cb, gb, acc);
-            float t0 = fmaf(k0.x, h0, fmaf(k0.y, h1, k0.z * h2));
-            float t1 = fmaf(k0.w, h3, fmaf(k1.x, h4, k1.y * h5));
-            p = acc - (t0 + t1);
+        __syncthreads();                                   // sigma0 of every stage is in place
+        if (warp == 0) backward_pass(L, smem, N, Gv, dt, has_ext, lane);
+        __syncthreads();
+        // ---- P2: kappa = Mh^-1 hh - Kh[:,12] x_12  (lane = stage) ----------------------------------
+        if (tact) {
+            const float4 h0 = *reinterpret_cast<const float4 *>(myX);
+            const float2 h1 = *reinterpret_cast<const float2 *>(myX + 4);
+            const float h[6] = { h0.x, h0.y, h0.z, h0.w, h1.x, h1.y };
+            float Mi[21], kp[6];
+#pragma unroll
+            for (int c = 0; c < 21; c++) Mi[c] = myM[c];
+            symv6(Mi, h, kp);
+#pragma unroll
+            for (int a = 0; a < 6; a++) kp[a] -= myM[21 + a];
+            *reinterpret_cast<float4 *>(myX) = make_float4(kp[0], kp[1], kp[2], kp[3]);
+            *reinterpret_cast<float2 *>(myX + 4) = make_float2(kp[4], kp[5]);
         }
-        __syncwarp();
-        // ---- kappa = Mh^-1 hh (lane = stage) ------------------------------------------------------
-        for (int k = lane; k < N; k += 32) {
-            float h[6], kp[6];
-#pragma unroll
-            for (int a = 0; a < 6; a++) h[a] = V.KP[k * L::V6 + a];
-            symv6(V.MI + k * L::MI, h, kp);
-#pragma unroll
-            for (int a = 0; a < 6; a++) V.KP[k * L::V6 + a] = kp[a];
-        }
-        __syncwarp();
-        // ---- forward rollout (sequential; lane j = row j of x, lanes 0..5 also own w_i) -----------
-        float x = x0_l;
-        for (int k = 0; k < N; k++) {
-            const float *kb = V.KB + k * L::KB;
-            const float cs = V.IW[k * L::IW + 6], sn = V.IW[k * L::IW + 7];
-            float w = (lane < 6) ? V.KP[k * L::V6 + lane] : 0.0f;
-            const int li = lane < 6 ? lane : 0;
-#pragma unroll
-            for (int j = 0; j < NX; j++) {
-                float xj = __shfl_sync(FULL, x, j);
-                w = fmaf(-kb[j * 8 + li], xj, w);
+        if (emit && tid < 20) red[tid] = 0u;
+        __syncthreads();
+        if (warp == 0) forward_pass(L, smem, N, Gv, dt, has_ext, lane, x0g, b0, emit, done, o.x);
+        __syncthreads();
+        // ---- P3: u from w, projection (S4), dual update (S5), residuals (S6)  (lane = stage) --------
+        if (tact && !frozen) {
+            float u0[NU], G0[6], wv[6], dl[6], lam[6];
+            stage_u0<NU>(P, ru, z, y, r, u0, G0);
+            {
+                const float4 w0 = *reinterpret_cast<const float4 *>(myX);
+                const float2 w1 = *reinterpret_cast<const float2 *>(myX + 4);
+                wv[0] = w0.x; wv[1] = w0.y; wv[2] = w0.z; wv[3] = w0.w; wv[4] = w1.x; wv[5] = w1.y;
             }
-            if (lane < 6) V.WV[k * L::V6 + lane] = w;
-            float wc = w + ((lane < 6) ? V.CE[k * L::V6 + lane] : 0.0f);
-            float wj = __shfl_sync(FULL, wc, wsrc);
-            float xa = __shfl_sync(FULL, x, fsa), xb = __shfl_sync(FULL, x, fsb);
-            float ca = fmaf(f_cc, cs, fmaf(f_cs, sn, f_c1)), cb = fmaf(f_dc, cs, f_ds * sn);
-            float xn = fmaf(ca, xa, fmaf(cb, xb, x));
-            if (lane >= 6 && lane < 12) xn += wj;
-            x = xn;
-            if (emit && lane < NX) o.x[((long)b * N + k) * NX + lane] = x;
-        }
-        __syncwarp();
-        // ---- u reconstruction, projection, dual update, residuals (lane = stage) -------------------
-        float rp_l = 0.0f, rd_l = 0.0f, un_l = 0.0f, zn_l = 0.0f, yn_l = 0.0f;
-        for (int k = lane; k < N; k += 32) {
-            float u0[NU], G0[6], wv[6], dl[6], lam[6], z[NU], y[NU], r[3 * NC];
-#pragma unroll
-            for (int j = 0; j < NU; j++) { z[j] = V.ZZ[k * L::ZY + j]; y[j] = V.YY[k * L::ZY + j]; }
-#pragma unroll
-            for (int j = 0; j < 3 * NC; j++) r[j] = V.RR[k * L::RR + j];
-            stage_u0<NU>(P, V.RU + k * L::RU, z, y, r, u0, G0);
-#pragma unroll
-            for (int a = 0; a < 6; a++) wv[a] = V.WV[k * L::V6 + a];
-            dinv_apply(V.IW + k * L::IW, idt, m_dt, wv, dl);
+            dinv_apply(Iw, idt, m_dt, wv, dl);
 #pragma unroll
             for (int a = 0; a < 6; a++) dl[a] -= G0[a];
-            symv6(V.LI + k * L::LI, dl, lam);
+            symv6(LI, dl, lam);
             // u = u0 + Rt^-1 Gh^T lam :  f_i += lam_tau x r_i + lam_F ;  m_i += lam_tau
             float u[NU];
 #pragma unroll
@@ -496,25 +620,23 @@ __global__ void __launch_bounds__(32) k_solve_srb(SolveParams P, ProblemPtrs q, 
                 float c0 = lam[1] * rz - lam[2] * ry + lam[3];
                 float c1 = lam[2] * rx - lam[0] * rz + lam[4];
                 float c2 = lam[0] * ry - lam[1] * rx + lam[5];
-                int fc = fcol(i);
+                const int fc = fcol(i);
                 u[fc] = u0[fc] + c0 / (P.Rd[fc] + P.rho);
                 u[fc + 1] = u0[fc + 1] + c1 / (P.Rd[fc + 1] + P.rho);
                 u[fc + 2] = u0[fc + 2] + c2 / (P.Rd[fc + 2] + P.rho);
                 if (i < NW) {
-                    int mc = mcol(i);
+                    const int mc = mcol(i);
 #pragma unroll
                     for (int a = 0; a < 3; a++) u[mc + a] = u0[mc + a] + lam[a] / (P.Rd[mc + a] + P.rho);
                 }
             }
-            // projection (S4), dual update (S5), residuals (S6)
-            const int bits = __float_as_int(V.IW[k * L::IW + 8]);
             float zn[NU];
 #pragma unroll
             for (int i = 0; i < NC; i++) {
                 const bool on = (bits >> i) & 1;
-                int fc = fcol(i);
+                const int fc = fcol(i);
                 if (i < NW) {
-                    int mc = mcol(i);
+                    const int mc = mcol(i);
                     float a0, a1, a2, a3, a4, a5;
                     project_wrench(P, u[fc] + y[fc], u[fc + 1] + y[fc + 1], u[fc + 2] + y[fc + 2], u[mc] + y[mc],
                                    u[mc + 1] + y[mc + 1], u[mc + 2] + y[mc + 2], a0, a1, a2, a3, a4, a5);
@@ -526,63 +648,131 @@ __global__ void __launch_bounds__(32) k_solve_srb(SolveParams P, ProblemPtrs q, 
                         zn[fc + a] = on ? fminf(fmaxf(u[fc + a] + y[fc + a], -P.hand_fmax), P.hand_fmax) : 0.0f;
                 }
             }
+            if (emit) {
+                float rp = 0.0f, rd = 0.0f, un = 0.0f, znm = 0.0f, ynm = 0.0f;
+                float *ou = o.u + ts * NU;
 #pragma unroll
-            for (int j = 0; j < NU; j++) {
-                float yn = y[j] + u[j] - zn[j];
-                rp_l = fmaxf(rp_l, fabsf(u[j] - zn[j]));
-                rd_l = fmaxf(rd_l, fabsf(zn[j] - z[j]));
-                un_l = fmaxf(un_l, fabsf(u[j])); zn_l = fmaxf(zn_l, fabsf(zn[j])); yn_l = fmaxf(yn_l, fabsf(yn));
-                V.ZZ[k * L::ZY + j] = zn[j];
-                V.YY[k * L::ZY + j] = yn;
-                if (emit) o.u[((long)b * N + k) * NU + j] = u[j];
+                for (int j = 0; j < NU; j++) {
+                    rp = fmaxf(rp, fabsf(u[j] - zn[j]));
+                    rd = fmaxf(rd, fabsf(zn[j] - z[j]));
+                    un = fmaxf(un, fabsf(u[j])); znm = fmaxf(znm, fabsf(zn[j]));
+                    ynm = fmaxf(ynm, fabsf(y[j] + u[j] - zn[j]));
+                    ou[j] = u[j];
+                }
+                // non-negative floats order like their bit patterns
+                atomicMax(&red[te * 5 + 0], __float_as_uint(rp)); atomicMax(&red[te * 5 + 1], __float_as_uint(rd));
+                atomicMax(&red[te * 5 + 2], __float_as_uint(un)); atomicMax(&red[te * 5 + 3], __float_as_uint(znm));
+                atomicMax(&red[te * 5 + 4], __float_as_uint(ynm));
             }
-            stage_sigma0(k);           // sigma0 of the next iteration from the new z, y
-        }
-        __syncwarp();
-        rp = warp_max(rp_l); rd = P.rho * warp_max(rd_l);
-        done = it + 1;
-        if (is_check) {
-            float sc = fmaxf(warp_max(un_l), warp_max(zn_l)), ys = warp_max(yn_l);
-            if (rp <= P.eps_abs + P.eps_rel * sc && rd <= P.eps_abs + P.eps_rel * P.rho * ys) break;
-        }
-    }
-    for (int k = lane; k < N; k += 32)
 #pragma unroll
-        for (int j = 0; j < NU; j++) {
-            o.z[((long)b * N + k) * NU + j] = V.ZZ[k * L::ZY + j];
-            o.y[((long)b * N + k) * NU + j] = V.YY[k * L::ZY + j];
+            for (int j = 0; j < NU; j++) { y[j] = y[j] + u[j] - zn[j]; z[j] = zn[j]; }
         }
-    if (lane == 0) { o.r_prim[b] = rp; o.r_dual[b] = rd; o.iters_done[b] = done; }
+        if (emit) {
+            __syncthreads();
+            if (tid < Gv && !done[tid]) {                  // one leader per env
+                const float rp = __uint_as_float(red[tid * 5 + 0]), rd = P.rho * __uint_as_float(red[tid * 5 + 1]);
+                o.r_prim[b0 + tid] = rp; o.r_dual[b0 + tid] = rd; o.iters_done[b0 + tid] = it + 1;
+                if (is_check) {
+                    const float sc = fmaxf(__uint_as_float(red[tid * 5 + 2]), __uint_as_float(red[tid * 5 + 3]));
+                    const float ys = __uint_as_float(red[tid * 5 + 4]);
+                    if (rp <= P.eps_abs + P.eps_rel * sc && rd <= P.eps_abs + P.eps_rel * P.rho * ys) {
+                        done[tid] = 1;
+                        atomicAdd(ndone, 1);
+                    }
+                }
+            }
+            __syncthreads();
+            if (is_check) {
+                if (*ndone == Gv) break;
+                if (tact) frozen = done[te] != 0;
+            }
+        }
+        if (tact && it + 1 < P.iters) stage_sigma0();      // frozen envs keep a well-defined (constant) sigma0
+    }
+    if (tact) {
+        float *oz = o.z + ts * NU, *oy = o.y + ts * NU;
+#pragma unroll
+        for (int j = 0; j < NU; j++) { oz[j] = z[j]; oy[j] = y[j]; }
+    }
 }
 
-template <int NU>
-size_t smem_bytes_t(int N) { return ((size_t)Lay<NU>::PER_STAGE * N + Lay<NU>::FIXED) * sizeof(float); }
+// ---------------------------------------------------------------------------------------------
+// launcher
+// ---------------------------------------------------------------------------------------------
+int fail(pinmpc_ctx *h, const char *what, cudaError_t e)
+{
+    h->sticky = e;
+    snprintf(h->err, sizeof h->err, "%s: %s", what, cudaGetErrorString(e));
+    return -1;
+}
+
+size_t iterate_smem_bytes(int N, int G, int ext)
+{
+    return ((size_t)G * arena_layout(N, ext).stride + CTL_INTS) * sizeof(float);
+}
+
+// envs per CTA: the G in 1..4 that keeps most envs resident per SM (shared memory, registers and
+// thread slots), ties to the smaller CTA (more independent CTAs overlap passes and stage phases).
+int choose_G(const pinmpc_ctx *h, int regs, int ext)
+{
+    int best = 0, best_envs = 0;
+    for (int G = 1; G <= 4; G++) {
+        int threads = (G * h->N + 31) / 32 * 32;
+        if (threads < 32) threads = 32;
+        size_t smem = iterate_smem_bytes(h->N, G, ext);
+        if (threads > 256 || smem > (size_t)h->smem_optin) continue;
+        int by_smem = (int)((size_t)(228 * 1024) / (smem + 1024));
+        int by_regs = 65536 / (threads * ((regs + 7) / 8 * 8));
+        int by_thr = 2048 / threads;
+        int ctas = by_smem < by_regs ? by_smem : by_regs;
+        if (by_thr < ctas) ctas = by_thr;
+        if (ctas > 32) ctas = 32;
+        if (ctas < 1) continue;
+        int envs = ctas * G;
+        if (envs > best_envs) { best_envs = envs; best = G; }
+    }
+    return best;
+}
 
 template <int NU>
 int launch_t(pinmpc_ctx *h, cudaStream_t st)
 {
-    size_t smem = smem_bytes_t<NU>(h->N);
-    if (smem > (size_t)h->smem_optin) {
+    SolveParams P = make_params(h);
+    ProblemPtrs q = make_problem_ptrs(h);
+    const int ext = q.ext != nullptr;
+    const long stages = (long)h->B * h->N;
+    k_assemble_srb<NU><<<(unsigned)((stages + 127) / 128), 128, 0, st>>>(P, q, h->srb);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(h, "k_assemble_srb launch", e);
+    k_factor_srb<<<(unsigned)((h->B + FAC_WARPS - 1) / FAC_WARPS), FAC_WARPS * 32, 0, st>>>(P, q.x0, h->srb, ext);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(h, "k_factor_srb launch", e);
+
+    cudaFuncAttributes fa;
+    e = cudaFuncGetAttributes(&fa, k_iterate_srb<NU>);
+    if (e != cudaSuccess) return fail(h, "k_iterate_srb attributes", e);
+    int G = h->envs_per_cta;
+    if (G > 0) {
+        int threads = (G * h->N + 31) / 32 * 32;
+        if (threads > 256 || iterate_smem_bytes(h->N, G, ext) > (size_t)h->smem_optin) G = 0;
+    }
+    if (G == 0) G = choose_G(h, fa.numRegs, ext);
+    if (G == 0) {
         snprintf(h->err, sizeof h->err, "structured solver: N=%d needs %zu B of shared memory per env (limit %d)", h->N,
-                 smem, h->smem_optin);
+                 iterate_smem_bytes(h->N, 1, ext), h->smem_optin);
         return -1;
     }
-    cudaError_t e = cudaFuncSetAttribute(k_solve_srb<NU>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e == cudaSuccess) {
-        k_solve_srb<NU><<<h->B, 32, smem, st>>>(make_params(h), make_problem_ptrs(h), h->out);
-        e = cudaGetLastError();
-    }
-    if (e != cudaSuccess) {
-        h->sticky = e;
-        snprintf(h->err, sizeof h->err, "k_solve_srb launch: %s", cudaGetErrorString(e));
-        return -1;
-    }
-    return 1;
+    int threads = (G * h->N + 31) / 32 * 32;
+    size_t smem = iterate_smem_bytes(h->N, G, ext);
+    e = cudaFuncSetAttribute(k_iterate_srb<NU>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return fail(h, "k_iterate_srb smem attribute", e);
+    k_iterate_srb<NU><<<(unsigned)((h->B + G - 1) / G), threads, smem, st>>>(P, h->srb, q.x0, q.mass, h->out, G, ext);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(h, "k_iterate_srb launch", e);
+    return 3;
 }
 
 }  // namespace
-
-size_t pinmpc_srb_smem_bytes(int nu, int N) { return nu == 12 ? smem_bytes_t<12>(N) : smem_bytes_t<18>(N); }
 
 int pinmpc_launch_solve_srb(pinmpc_ctx *h, cudaStream_t st)
 {
