@@ -101,7 +101,7 @@ pinmpc_status pinmpc_set_tolerance(pinmpc_t h, float eps_abs, float eps_rel, int
 /* Force a solver variant (default PINMPC_METHOD_AUTO). */
 pinmpc_status pinmpc_set_method(pinmpc_t h, pinmpc_method m);
 
-/* Tuning knob of the structured solver: envs solved per thread block (1..4; 0 = choose by the
+/* Tuning knob of the structured solver: envs solved per thread block (1..16; 0 = choose by the
  * occupancy heuristic of DESIGN.md "Kernels").  Results do not depend on it. */
 pinmpc_status pinmpc_set_tuning(pinmpc_t h, int envs_per_cta);
 

@@ -10,7 +10,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpinmpc.so")
 SOURCES = ["pinmpc_api.cu", "pinmpc_dense.cu", "pinmpc_srb.cu", "pinmpc_probe.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-              "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
+              "-Xcompiler", "-fPIC", "-Xptxas", "-v"] + os.environ.get("PINMPC_NVCC_EXTRA", "").split()
 
 
 def _stale() -> bool:

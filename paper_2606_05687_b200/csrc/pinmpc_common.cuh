@@ -41,13 +41,14 @@ struct DensePtrs {       // dense variant: materialised dynamics and Riccati fac
 // verbatim into shared memory; "stage" arrays are component-major [comp][st] so that threads
 // mapped lane = stage read and write them coalesced.
 struct SrbWs {
-    float *Kh;     // [st][6][12]    gain of the 6-D-input LQR, columns 0..11
+    float *Kh;     // [st][6][6][2]  gain of the 6-D-input LQR, pairs (Kh[r][j], Kh[r][6+j]), j = 0..5
     float *qv;     // [B][N+1][12]   q_k = Q xbar_k (k = 1..N), q_0 = 0
     float *c6;     // [st][6]        ch = (dt I_w^-1 tau_ext ; dt/m F_ext)   (zeros without ext_wrench)
-    float *sv;     // [st][12]       s_k = P_{k+1} E ch                      (zeros without ext_wrench)
+    float *HQ;     // [6][st]        (reserved)
     float *cs;     // [st][2]        cos, sin of the linearisation yaw
     float *MI;     // [21][st]       S_k after assembly, Mh_k^-1 after factorisation (packed symmetric)
-    float *KG;     // [6][st]        Kh[:,12] * x_12  (the constant gravity state's share of w)
+    float *KG;     // [6][st]        kg_k = Kh[:,12] x_12 - Mh^-1 hq_k: gravity state's share of w and the
+                   //                iteration-invariant part of the backward pass (response to q, s)
     float *LI;     // [21][st]       Lam_k^-1 (packed symmetric)
     float *IW;     // [6][st]        I_w (packed symmetric 3x3)
     float *RR;     // [3*nc][st]     contact offsets

@@ -304,6 +304,8 @@ __global__ void __launch_bounds__(FAC_WARPS * 32) k_factor_srb(SolveParams P, co
 
     for (int i = lane; i < 169; i += 32) sP[i] = ((i * 79) >> 10) * 14 == i ? P.Qd[(i * 79) >> 10] : 0.0f;
     __syncwarp();
+    const int jl = lane < 12 ? lane : 0;
+    float pc = W.qv[((long)b * (N + 1) + N) * 12 + jl];     // pc_N = q_N
 
     // prefetch stage N-1
     long s = (long)b * N + N - 1;
@@ -366,12 +368,33 @@ __global__ void __launch_bounds__(FAC_WARPS * 32) k_factor_srb(SolveParams P, co
 #pragma unroll
                 for (int l = 0; l < 6; l++) a = fmaf(sM[sidx(i, l)], sX[(6 + l) * NX + j], a);
                 sK[e] = a;
-                if (j < 12) W.Kh[s * 72 + i * 12 + j] = a;
-                else W.KG[(long)i * st + s] = a * x12;
+                if (j < 12) W.Kh[s * 72 + i * 12 + (j < 6 ? 2 * j : 2 * (j - 6) + 1)] = a;
             }
         }
-        if (has_ext && lane < 12) W.sv[s * 12 + lane] = sk;
         __syncwarp();
+        // iteration-invariant part of the backward vector pass (response to q and s, sigma0 = 0):
+        //   g = pc - s_k ; hq_k = E^T g ; pc <- q_k + A^T g - Kh^T hq_k        (lane j < 12 holds pc_j)
+        // The iteration kernel runs the sigma0-driven part only; hq_k enters kappa_k through kg_k.
+        {
+            const float g = pc - sk;
+            const float g_lo = __shfl_sync(FULL, g, lane >= 6 ? lane - 6 : lane);
+            const float g_nb = __shfl_sync(FULL, g, lane >= 6 ? (lane - 6) ^ 1 : lane);
+            float acc = 0.0f, mh = 0.0f;
+            const int il = lane < 6 ? lane : 0;
+#pragma unroll
+            for (int r = 0; r < 6; r++) {
+                const float hr = __shfl_sync(FULL, g, 6 + r);
+                acc = fmaf(sK[r * NX + jl], hr, acc);
+                mh = fmaf(sM[sidx(il, r)], hr, mh);
+            }
+            // constant part of kappa_k = Mh^-1 hh_k - Kh[:,12] x_12 :  kg_k = Kh[:,12] x_12 - Mh^-1 hq_k
+            if (lane < 6) W.KG[(long)lane * st + s] = fmaf(sK[lane * NX + 12], x12, -mh);
+            float atg = g;
+            if (lane == 6) atg = fmaf(dt, cs * g_lo - sn * g_nb, g);
+            else if (lane == 7) atg = fmaf(dt, cs * g_lo + sn * g_nb, g);
+            else if (lane >= 8 && lane < 12) atg = fmaf(dt, g_lo, g);
+            pc = (k >= 1 ? W.qv[((long)b * (N + 1) + k) * 12 + jl] : 0.0f) + atg - acc;
+        }
         // P <- [k>=1] Q + A^T X - G^T Kh   (upper triangle, mirrored: both terms are symmetric)
 #pragma unroll
         for (int r = 0; r < 3; r++) {
@@ -390,121 +413,220 @@ __global__ void __launch_bounds__(FAC_WARPS * 32) k_factor_srb(SolveParams P, co
 }
 
 // ---------------------------------------------------------------------------------------------
-// S3-S6  ADMM iterations: one CTA per G envs, every factor on chip
+// S3-S6  ADMM iterations: one CTA per G envs, every factor on chip (v3)
 // ---------------------------------------------------------------------------------------------
-// Shared-memory arena of one env (offsets in floats).  The arena stride is 8 mod 32 so that the
-// 8-lane groups of up to four envs in the pass warp hit disjoint banks.
-struct ArenaLay { int oQ, oX, oCS, oM, oC, oS, oF, stride; };
+// Every thread owns one (env, stage) and keeps the stage-local data (Lam^-1, I_w, r, R ubar, z, y)
+// in registers for all iterations ("stage work": u from w, projection S4, dual update S5,
+// residuals S6, sigma0 of the next iteration, kappa).  The first PW warps of the CTA also run the
+// two sequential vector recursions ("passes") of up to five envs each, six lanes per env
+// (lane = 6 e + i), exchanging the 6-D quantities with warp shuffles; the gains stream from the
+// env's shared-memory arena through explicit ld.shared with immediate offsets, one stage ahead.
+//
+// Shared-memory arena of one env (offsets in floats):
+//   Kn [N][6][6][2]  pairs -(Kh[r][j], Kh[r][6+j]): row r contiguous (forward pass, lane = row,
+//                    3 x LDS.128), pair [r][i] (backward pass, lane = column pair, 6 x LDS.64)
+//   X  [N][8]        exchange vector: sigma0 -> hh -> kappa -> w
+//   CS [N][2]        cos, sin of the linearisation yaw
+//   M  [N][28]       Mh^-1 packed symmetric (21), kg = Kh[:,12] x_12 - Mh^-1 hq (6), pad
+//   C  [N][6]        ch (ext only)
+struct ArenaLay { int oX, oCS, oM, oC, stride; };
+
+constexpr int ITER_MAX_THREADS = 512;  // 16 warps x 128 registers fill the register file of an SM
+constexpr int PASS_ENVS = 5;           // envs per pass warp (6 lanes each)
+constexpr int ARENA_PAD_MOD = 12;      // arena stride mod 32 (bank spread of the 6-lane groups)
+constexpr int G_MAX = 16;              // envs per CTA
+constexpr int CTL_INTS = 32 + 5 * G_MAX;   // done[16] | ndone | pad[15] | red[16][5]
 
 __host__ __device__ inline ArenaLay arena_layout(int N, int ext)
 {
     ArenaLay L;
-    L.oQ = 72 * N;                    // Kh [N][6][12] at 0 ; q [N+1][12]
-    L.oX = L.oQ + 12 * (N + 1);       // exchange vector [N][8]: sigma0 -> hh -> kappa -> w
-    L.oCS = L.oX + 8 * N;             // cos, sin [N][2]
-    L.oM = L.oCS + 2 * N;             // Mh^-1 (21) and kg (6) per stage, stride 27 (lane = stage)
-    L.oC = L.oM + 27 * N;             // ch [N][6]      (ext only)
-    L.oS = L.oC + (ext ? 6 * N : 0);  // s  [N][12]     (ext only)
-    L.oF = (L.oS + (ext ? 12 * N : 0) + 3) & ~3;   // forward-pass exchange scratch [2][8]
-    int size = L.oF + 16;
-    L.stride = size + ((8 - (size & 31)) & 31);
+    L.oX = 72 * N;
+    L.oCS = L.oX + 8 * N;
+    L.oM = (L.oCS + 2 * N + 3) & ~3;
+    L.oC = L.oM + 28 * N;
+    int size = (L.oC + (ext ? 6 * N : 0) + 3) & ~3;
+    L.stride = size + ((ARENA_PAD_MOD - (size & 31)) & 31);
     return L;
 }
 
-constexpr int CTL_INTS = 32;          // done[4] | ndone | pad[3] | red[4][5]
-
-// Backward vector pass of all envs of the CTA (warp 0; lane = 8 e + i, lanes i < 6 own the
-// columns i (Theta/p part) and 6 + i (omega/v part) of p).
-__device__ __forceinline__ void backward_pass(const ArenaLay &L, float *smem, int N, int Gv, float dt, int has_ext, int lane)
+// shared-memory accesses with 32-bit addresses and immediate byte offsets
+template <int OFF> __device__ __forceinline__ float lds1(unsigned a)
 {
-    const int e = lane >> 3, i0 = lane & 7, i = i0 < 6 ? i0 : 5;
-    const bool act = i0 < 6 && e < Gv;
-    float *ar = smem + (e < Gv ? e : 0) * L.stride;
-    const float *aQ = ar + L.oQ, *aCS = ar + L.oCS, *aS = ar + L.oS;
-    float *aX = ar + L.oX;
-    float pq = aQ[N * 12 + i], pv = aQ[N * 12 + 6 + i];
-    for (int k = N - 1; k >= 0; k--) {
-        const float *Kk = ar + k * 72;
-        float kq[6], kv[6];
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1+%2];" : "=f"(v) : "r"(a), "n"(OFF));
+    return v;
+}
+template <int OFF> __device__ __forceinline__ float2 lds2(unsigned a)
+{
+    float2 v;
+    asm volatile("ld.shared.v2.f32 {%0,%1}, [%2+%3];" : "=f"(v.x), "=f"(v.y) : "r"(a), "n"(OFF));
+    return v;
+}
+template <int OFF> __device__ __forceinline__ float4 lds4(unsigned a)
+{
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4+%5];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a), "n"(OFF));
+    return v;
+}
+template <int OFF> __device__ __forceinline__ void sts1(unsigned a, float v)
+{
+    asm volatile("st.shared.f32 [%0+%1], %2;" ::"r"(a), "n"(OFF), "f"(v));
+}
+
+// lane-constant description of a pass lane
+struct PassLane {
+    unsigned aK_b, aK_f, aX, aCS, aC;   // shared addresses at stage 0: Kn pair [.][i], Kn row i, X[.][i], CS, C[.][i]
+    int src[6];                         // lanes of the env's group
+    int nb;                             // lane holding the other component of the (roll, pitch) pair
+    float m, om, sg;                    // i < 2 ? 1 : 0 ;  1 - m ;  -1, +1, 0 for i = 0, 1, >= 2
+    bool act;
+};
+
+constexpr int SB_K = 72 * 4, SB_X = 8 * 4, SB_CS = 2 * 4, SB_C = 6 * 4;   // bytes per stage of the arena sections
+
+// ---- backward vector pass (the part of the costate driven by sigma0; the response to q and s is
+// iteration-invariant and folded into kg by the factorisation).  Lane (e, i) owns component i of
+// the (Theta, p) part pq and of the (omega, v) part pv.  Per stage k = N-1..0:
+//   hh = sigma0_k + pv -> X_k ;  pq <- pq - Kq^T hh ;  pv <- pv + dt rot(pq) - Kv^T hh
+struct BwdOps { float2 k[6]; float s0; float2 cs; };
+
+template <int D> __device__ __forceinline__ void bwd_load(BwdOps &o, unsigned aK, unsigned aX, unsigned aCS)
+{
+    o.k[0] = lds2<D * SB_K + 0 * 48>(aK); o.k[1] = lds2<D * SB_K + 1 * 48>(aK); o.k[2] = lds2<D * SB_K + 2 * 48>(aK);
+    o.k[3] = lds2<D * SB_K + 3 * 48>(aK); o.k[4] = lds2<D * SB_K + 4 * 48>(aK); o.k[5] = lds2<D * SB_K + 5 * 48>(aK);
+    o.s0 = lds1<D * SB_X>(aX);
+    o.cs = lds2<D * SB_CS>(aCS);
+}
+
+template <int D> __device__ __forceinline__ void bwd_step(const BwdOps &o, float &pq, float &pv, const PassLane &p, unsigned aX, float dt)
+{
+    const float hown = o.s0 + pv;
+    if (p.act) sts1<D * SB_X>(aX, hown);
+    float hh[6];
 #pragma unroll
-        for (int r = 0; r < 6; r++) { kq[r] = Kk[r * 12 + i]; kv[r] = Kk[r * 12 + 6 + i]; }
-        const float qq = aQ[k * 12 + i], qn = aQ[k * 12 + 6 + i];
-        const float s0 = aX[k * 8 + i];
-        const float csk = aCS[2 * k], snk = aCS[2 * k + 1];
-        float sq = 0.0f, sn6 = 0.0f;
-        if (has_ext) { sq = aS[k * 12 + i]; sn6 = aS[k * 12 + 6 + i]; }
-        const float gq = pq - sq, gv = pv - sn6;
-        const float hh = s0 + gv;
-        if (act) aX[k * 8 + i] = hh;
-        const float oth = __shfl_xor_sync(FULL, gq, 1);
-        __syncwarp();
-        const float4 h0 = *reinterpret_cast<const float4 *>(aX + k * 8);
-        const float2 h1 = *reinterpret_cast<const float2 *>(aX + k * 8 + 4);
-        float a0 = kq[0] * h0.x, a1 = kq[3] * h0.w, b0 = kv[0] * h0.x, b1 = kv[3] * h0.w;
-        a0 = fmaf(kq[1], h0.y, a0); a1 = fmaf(kq[4], h1.x, a1); b0 = fmaf(kv[1], h0.y, b0); b1 = fmaf(kv[4], h1.x, b1);
-        a0 = fmaf(kq[2], h0.z, a0); a1 = fmaf(kq[5], h1.y, a1); b0 = fmaf(kv[2], h0.z, b0); b1 = fmaf(kv[5], h1.y, b1);
-        // (A^T g)_nu = g_nu + dt (R_z g_Theta ; g_p)
-        const float ca = i < 2 ? csk : 1.0f, cb = i == 0 ? -snk : (i == 1 ? snk : 0.0f);
-        const float rot = fmaf(cb, oth, ca * gq);
-        pq = (qq + gq) - (a0 + a1);
-        pv = fmaf(dt, rot, qn + gv) - (b0 + b1);
+    for (int r = 0; r < 6; r++) hh[r] = __shfl_sync(FULL, hown, p.src[r]);
+    const float oth = __shfl_sync(FULL, pq, p.nb);
+    // off the chain: (A^T p)_v = pv + dt (R_z pq_Theta ; pq_p)
+    const float al = fmaf(p.m, o.cs.x, p.om), be = p.sg * o.cs.y;
+    const float basev = fmaf(dt, fmaf(be, oth, al * pq), pv);
+    float a0 = fmaf(o.k[0].x, hh[0], pq), a1 = o.k[3].x * hh[3];
+    float b0 = fmaf(o.k[0].y, hh[0], basev), b1 = o.k[3].y * hh[3];
+    a0 = fmaf(o.k[1].x, hh[1], a0); a1 = fmaf(o.k[4].x, hh[4], a1); b0 = fmaf(o.k[1].y, hh[1], b0); b1 = fmaf(o.k[4].y, hh[4], b1);
+    a0 = fmaf(o.k[2].x, hh[2], a0); a1 = fmaf(o.k[5].x, hh[5], a1); b0 = fmaf(o.k[2].y, hh[2], b0); b1 = fmaf(o.k[5].y, hh[5], b1);
+    pq = a0 + a1;
+    pv = b0 + b1;
+}
+
+__device__ __forceinline__ void backward_pass(const PassLane &p, int N, float dt)
+{
+    unsigned aK = p.aK_b + (N - 1) * SB_K, aX = p.aX + (N - 1) * SB_X, aCS = p.aCS + (N - 1) * SB_CS;
+    float pq = 0.0f, pv = 0.0f;
+    BwdOps A, B;
+    bwd_load<0>(A, aK, aX, aCS);
+    int k = N - 1;
+    for (; k >= 3; k -= 2) {
+        bwd_load<-1>(B, aK, aX, aCS);
+        bwd_step<0>(A, pq, pv, p, aX, dt);
+        bwd_load<-2>(A, aK, aX, aCS);
+        bwd_step<-1>(B, pq, pv, p, aX, dt);
+        aK -= 2 * SB_K; aX -= 2 * SB_X; aCS -= 2 * SB_CS;
+    }
+    if (k == 2) {
+        bwd_load<-1>(B, aK, aX, aCS);
+        bwd_step<0>(A, pq, pv, p, aX, dt);
+        bwd_load<-2>(A, aK, aX, aCS);
+        bwd_step<-1>(B, pq, pv, p, aX, dt);
+        bwd_step<-2>(A, pq, pv, p, aX, dt);
+    } else if (k == 1) {
+        bwd_load<-1>(B, aK, aX, aCS);
+        bwd_step<0>(A, pq, pv, p, aX, dt);
+        bwd_step<-1>(B, pq, pv, p, aX, dt);
+    } else {
+        bwd_step<0>(A, pq, pv, p, aX, dt);
     }
 }
 
-// Forward rollout of all envs of the CTA (warp 0; every active lane holds the whole state, lane i
-// owns row i of Kh and the new omega/v component i).  Writes w_k over kappa_k; optionally emits x.
-__device__ __forceinline__ void forward_pass(const ArenaLay &L, float *smem, int N, int Gv, float dt, int has_ext, int lane,
-                                             const float *__restrict__ x0g, int b0, bool emit, const int *done, float *ox)
+// ---- forward rollout.  Every lane of env e holds the whole state (the (Theta, p) part is advanced
+// redundantly, the (omega, v) part is exchanged); lane i owns row i of Kh and the new component
+// 6 + i.  Per stage k = 0..N-1:   w = kappa_k - Kh x -> X_k ;  x+ = A x + E (w + ch)
+struct FwdOps { float4 r0, r1, r2; float kap, c; float2 cs; };
+
+template <int D> __device__ __forceinline__ void fwd_load(FwdOps &o, unsigned aK, unsigned aX, unsigned aCS, unsigned aC, int has_ext, float gdt)
 {
-    const int e = lane >> 3, i0 = lane & 7, i = i0 < 6 ? i0 : 5;
-    const bool act = i0 < 6 && e < Gv;
-    const int ee = e < Gv ? e : 0;
-    float *ar = smem + ee * L.stride;
-    const float *aCS = ar + L.oCS, *aC = ar + L.oC;
-    float *aX = ar + L.oX, *aF = ar + L.oF;
-    const float *xg = x0g + (long)(b0 + ee) * NX;
-    float x0 = xg[0], x1 = xg[1], x2 = xg[2], x3 = xg[3], x4 = xg[4], x5 = xg[5];
-    float x6 = xg[6], x7 = xg[7], x8 = xg[8], x9 = xg[9], x10 = xg[10], x11 = xg[11];
-    const float x12 = xg[12];
-    float own = xg[6 + i];
-    const float gdt = i == 5 ? dt * x12 : 0.0f;
-    const bool wr = emit && act && !done[ee];
-    float *oxe = ox + (long)(b0 + ee) * N * NX;
-    int par = 0;
-    for (int k = 0; k < N; k++) {
-        const float4 *Kr = reinterpret_cast<const float4 *>(ar + k * 72 + i * 12);
-        const float4 r0 = Kr[0], r1 = Kr[1], r2 = Kr[2];
-        const float kap = aX[k * 8 + i];
-        const float csk = aCS[2 * k], snk = aCS[2 * k + 1];
-        const float c = (has_ext ? aC[k * 6 + i] : 0.0f) + gdt;
-        float a0 = r0.x * x0, a1 = r0.w * x3, a2 = r1.z * x6, a3 = r2.y * x9;
-        a0 = fmaf(r0.y, x1, a0); a1 = fmaf(r1.x, x4, a1); a2 = fmaf(r1.w, x7, a2); a3 = fmaf(r2.z, x10, a3);
-        a0 = fmaf(r0.z, x2, a0); a1 = fmaf(r1.y, x5, a1); a2 = fmaf(r2.x, x8, a2); a3 = fmaf(r2.w, x11, a3);
-        const float w = kap - ((a0 + a1) + (a2 + a3));
-        const float nun = own + (w + c);
-        if (act) { aX[k * 8 + i] = w; aF[par * 8 + i] = nun; }
-        // Theta+ = Theta + dt R_z^T omega ; p+ = p + dt v   (old omega, v)
-        x0 = fmaf(dt, fmaf(csk, x6, snk * x7), x0);
-        x1 = fmaf(dt, fmaf(csk, x7, -snk * x6), x1);
-        x2 = fmaf(dt, x8, x2); x3 = fmaf(dt, x9, x3); x4 = fmaf(dt, x10, x4); x5 = fmaf(dt, x11, x5);
-        __syncwarp();
-        const float4 n0 = *reinterpret_cast<const float4 *>(aF + par * 8);
-        const float2 n1 = *reinterpret_cast<const float2 *>(aF + par * 8 + 4);
-        x6 = n0.x; x7 = n0.y; x8 = n0.z; x9 = n0.w; x10 = n1.x; x11 = n1.y;
-        own = nun;
+    o.r0 = lds4<D * SB_K>(aK); o.r1 = lds4<D * SB_K + 16>(aK); o.r2 = lds4<D * SB_K + 32>(aK);
+    o.kap = lds1<D * SB_X>(aX);
+    o.cs = lds2<D * SB_CS>(aCS);
+    o.c = has_ext ? gdt + lds1<D * SB_C>(aC) : gdt;
+}
+
+template <int D, bool EMIT>
+__device__ __forceinline__ void fwd_step(const FwdOps &o, float *xa, float *xb, float &own, const PassLane &p, unsigned aX, float dt,
+                                         int i, bool wr, float *ox, float x12)
+{
+    const float oc = own + o.c;
+    // off the chain: the (Theta, p) columns
+    float a0 = fmaf(o.r0.x, xa[0], o.kap), a1 = o.r1.z * xa[3];
+    a0 = fmaf(o.r0.z, xa[1], a0); a1 = fmaf(o.r2.x, xa[4], a1);
+    a0 = fmaf(o.r1.x, xa[2], a0); a1 = fmaf(o.r2.z, xa[5], a1);
+    const float t = a0 + a1;
+    // on the chain: the (omega, v) columns
+    float b0 = fmaf(o.r0.y, xb[0], t), b1 = o.r1.w * xb[3];
+    b0 = fmaf(o.r0.w, xb[1], b0); b1 = fmaf(o.r2.y, xb[4], b1);
+    b0 = fmaf(o.r1.y, xb[2], b0); b1 = fmaf(o.r2.w, xb[5], b1);
+    const float w = b0 + b1;
+    const float nun = w + oc;
+    if (p.act) sts1<D * SB_X>(aX, w);
+    // Theta+ = Theta + dt R_z^T omega ; p+ = p + dt v   (old omega, v)
+    xa[0] = fmaf(dt, fmaf(o.cs.x, xb[0], o.cs.y * xb[1]), xa[0]);
+    xa[1] = fmaf(dt, fmaf(o.cs.x, xb[1], -o.cs.y * xb[0]), xa[1]);
+#pragma unroll
+    for (int j = 2; j < 6; j++) xa[j] = fmaf(dt, xb[j], xa[j]);
+#pragma unroll
+    for (int j = 0; j < 6; j++) xb[j] = __shfl_sync(FULL, nun, p.src[j]);
+    own = nun;
+    if (EMIT) {
         if (wr) {
-            const float xs = i == 0 ? x0 : i == 1 ? x1 : i == 2 ? x2 : i == 3 ? x3 : i == 4 ? x4 : x5;
-            oxe[k * NX + i] = xs;
-            oxe[k * NX + 6 + i] = nun;
-            if (i == 0) oxe[k * NX + 12] = x12;
+            const float xs = i == 0 ? xa[0] : i == 1 ? xa[1] : i == 2 ? xa[2] : i == 3 ? xa[3] : i == 4 ? xa[4] : xa[5];
+            ox[D * NX + i] = xs;
+            ox[D * NX + 6 + i] = nun;
+            if (i == 0) ox[D * NX + 12] = x12;
         }
-        par ^= 1;
+    }
+}
+
+template <bool EMIT>
+__device__ __forceinline__ void forward_pass(const PassLane &p, int N, float dt, int has_ext, int i, const float *x0s, bool wr, float *ox)
+{
+    unsigned aK = p.aK_f, aX = p.aX, aCS = p.aCS, aC = p.aC;
+    float xa[6], xb[6];
+#pragma unroll
+    for (int j = 0; j < 6; j++) { xa[j] = x0s[j]; xb[j] = x0s[6 + j]; }
+    const float x12 = x0s[12];
+    float own = x0s[6 + i];
+    const float gdt = i == 5 ? dt * x12 : 0.0f;
+    FwdOps A, B;
+    fwd_load<0>(A, aK, aX, aCS, aC, has_ext, gdt);
+    int k = 0;
+    for (; k <= N - 3; k += 2) {
+        fwd_load<1>(B, aK, aX, aCS, aC, has_ext, gdt);
+        fwd_step<0, EMIT>(A, xa, xb, own, p, aX, dt, i, wr, ox, x12);
+        fwd_load<2>(A, aK, aX, aCS, aC, has_ext, gdt);
+        fwd_step<1, EMIT>(B, xa, xb, own, p, aX, dt, i, wr, ox, x12);
+        aK += 2 * SB_K; aX += 2 * SB_X; aCS += 2 * SB_CS; aC += 2 * SB_C;
+        if (EMIT) ox += 2 * NX;
+    }
+    if (k == N - 2) {
+        fwd_load<1>(B, aK, aX, aCS, aC, has_ext, gdt);
+        fwd_step<0, EMIT>(A, xa, xb, own, p, aX, dt, i, wr, ox, x12);
+        fwd_step<1, EMIT>(B, xa, xb, own, p, aX, dt, i, wr, ox, x12);
+    } else {
+        fwd_step<0, EMIT>(A, xa, xb, own, p, aX, dt, i, wr, ox, x12);
     }
 }
 
 template <int NU>
-__global__ void __launch_bounds__(256) k_iterate_srb(SolveParams P, SrbWs W, const float *__restrict__ x0g,
-                                                     const float *__restrict__ massg, OutPtrs o, int G, int has_ext)
+__global__ void __launch_bounds__(ITER_MAX_THREADS) k_iterate_srb(SolveParams P, SrbWs W, const float *__restrict__ x0g,
+                                                                  const float *__restrict__ massg, OutPtrs o, int G, int PW, int has_ext)
 {
     constexpr int NC = NW + (NU - 12) / 3;
     extern __shared__ __align__(16) float smem[];
@@ -514,17 +636,10 @@ __global__ void __launch_bounds__(256) k_iterate_srb(SolveParams P, SrbWs W, con
     const int b0 = blockIdx.x * G;
     const int Gv = min(G, P.B - b0);
     int *ctl = reinterpret_cast<int *>(smem + G * L.stride);
-    int *done = ctl, *ndone = ctl + 4;
-    unsigned *red = reinterpret_cast<unsigned *>(ctl + 8);
+    int *done = ctl, *ndone = ctl + 16;
+    unsigned *red = reinterpret_cast<unsigned *>(ctl + 32);
+    float *x0s = smem + G * L.stride + CTL_INTS;          // [G][16] initial states
     const float dt = P.dt, idt = 1.0f / P.dt;
-
-    // this thread's stage task: env te of the CTA, stage tk
-    const int te = tid / N, tk = tid - te * N;
-    const bool tact = te < Gv;
-    const int bb = b0 + (tact ? te : 0);
-    const long ts = (long)bb * N + tk;
-    float *ar = smem + (tact ? te : 0) * L.stride;
-    float *myX = ar + L.oX + tk * 8, *myM = ar + L.oM + tk * 27;
 
     // ---- load the pass arrays of the CTA's envs into shared memory ------------------------------
     for (int e = 0; e < Gv; e++) {
@@ -532,19 +647,46 @@ __global__ void __launch_bounds__(256) k_iterate_srb(SolveParams P, SrbWs W, con
         const long s0 = (long)(b0 + e) * N;
         const float4 *src = reinterpret_cast<const float4 *>(W.Kh + s0 * 72);
         float4 *dst = reinterpret_cast<float4 *>(a);
-        for (int i = tid; i < N * 18; i += nthr) dst[i] = src[i];
-        src = reinterpret_cast<const float4 *>(W.qv + (long)(b0 + e) * (N + 1) * 12);
-        dst = reinterpret_cast<float4 *>(a + L.oQ);
-        for (int i = tid; i < (N + 1) * 3; i += nthr) dst[i] = src[i];
-        for (int i = tid; i < N * 2; i += nthr) a[L.oCS + i] = W.cs[s0 * 2 + i];
-        if (has_ext) {
-            for (int i = tid; i < N * 6; i += nthr) a[L.oC + i] = W.c6[s0 * 6 + i];
-            for (int i = tid; i < N * 12; i += nthr) a[L.oS + i] = W.sv[s0 * 12 + i];
+        for (int i = tid; i < N * 18; i += nthr) {
+            const float4 v = src[i];
+            dst[i] = make_float4(-v.x, -v.y, -v.z, -v.w);
         }
+        for (int i = tid; i < N * 2; i += nthr) a[L.oCS + i] = W.cs[s0 * 2 + i];
+        if (has_ext)
+            for (int i = tid; i < N * 6; i += nthr) a[L.oC + i] = W.c6[s0 * 6 + i];
     }
-    if (tid < CTL_INTS) ctl[tid] = 0;
+    for (int i = tid; i < CTL_INTS; i += nthr) ctl[i] = 0;
+    for (int i = tid; i < Gv * 16; i += nthr) x0s[i] = (i & 15) < NX ? x0g[(long)(b0 + (i >> 4)) * NX + (i & 15)] : 0.0f;
 
-    // ---- stage-stationary registers (lane = stage) ---------------------------------------------
+    // ---- pass role of the first PW warps -----------------------------------------------------------
+    const bool pass_warp = warp < PW && warp * PASS_ENVS < Gv;
+    PassLane pl;
+    int pi = 0, pe = 0;
+    {
+        const int eloc = lane / 6;
+        pi = lane - 6 * eloc;
+        const int e = warp * PASS_ENVS + eloc;
+        pl.act = pass_warp && eloc < PASS_ENVS && e < Gv;
+        pe = pl.act ? e : (pass_warp ? warp * PASS_ENVS : 0);      // idle lanes shadow the warp's first env
+        const int base = pl.act ? 6 * eloc : 0;
+        const unsigned ar = (unsigned)__cvta_generic_to_shared(smem + pe * L.stride);
+        pl.aK_b = ar + 8 * pi; pl.aK_f = ar + 48 * pi;
+        pl.aX = ar + 4 * (L.oX + pi); pl.aCS = ar + 4 * L.oCS; pl.aC = ar + 4 * (L.oC + pi);
+#pragma unroll
+        for (int r = 0; r < 6; r++) pl.src[r] = base + r;
+        pl.nb = lane ^ 1;
+        pl.m = pi < 2 ? 1.0f : 0.0f; pl.om = 1.0f - pl.m; pl.sg = pi == 0 ? -1.0f : (pi == 1 ? 1.0f : 0.0f);
+    }
+    float *oxe = o.x + (long)(b0 + pe) * N * NX;
+
+    // ---- stage role: this thread's (env, stage) ---------------------------------------------------
+    const int te = tid / N, tk = tid - te * N;
+    const bool tact = te < Gv;
+    const int bb = b0 + (tact ? te : 0);
+    const long ts = (long)bb * N + tk;
+    float *arena = smem + (tact ? te : 0) * L.stride;
+    float *myX = arena + L.oX + tk * 8, *myM = arena + L.oM + tk * 28;
+
     float LI[21], Iw[6], r[3 * NC], ru[NU], z[NU], y[NU];
     int bits = 0;
     float m_dt = 0.0f;
@@ -561,7 +703,7 @@ __global__ void __launch_bounds__(256) k_iterate_srb(SolveParams P, SrbWs W, con
         m_dt = massg[bb] / dt;
     }
 
-    // sigma0 = D^-1 Lam^-1 Gh u0 of the coming iteration from the current z, y  (phase P1)
+    // X_k = sigma0 = D^-1 Lam^-1 Gh u0 of the coming iteration from the current z, y
     auto stage_sigma0 = [&]() {
         float u0[NU], G0[6], l0[6], s0[6];
         stage_u0<NU>(P, ru, z, y, r, u0, G0);
@@ -578,28 +720,35 @@ __global__ void __launch_bounds__(256) k_iterate_srb(SolveParams P, SrbWs W, con
     for (int it = 0; it < P.iters; it++) {
         const bool is_check = tol_mode && ((it + 1) % P.check_every == 0);
         const bool emit = (it == P.iters - 1) || is_check;
-        __syncthreads();                                   // sigma0 of every stage is in place
-        if (warp == 0) backward_pass(L, smem, N, Gv, dt, has_ext, lane);
-        __syncthreads();
-        // ---- P2: kappa = Mh^-1 hh - Kh[:,12] x_12  (lane = stage) ----------------------------------
+        if (emit)
+            for (int i = tid; i < 5 * G_MAX; i += nthr) red[i] = 0u;
+        __syncthreads();                                   // X = sigma0 of every stage is in place
+        if (pass_warp) backward_pass(pl, N, dt);
+        __syncthreads();                                   // X = hh
+        // ---- kappa = Mh^-1 hh - kg ---------------------------------------------------------------------
         if (tact) {
+            const float4 *Mq = reinterpret_cast<const float4 *>(myM);
+            float Mi[28];
+#pragma unroll
+            for (int c = 0; c < 7; c++) {
+                const float4 v = Mq[c];
+                Mi[4 * c] = v.x; Mi[4 * c + 1] = v.y; Mi[4 * c + 2] = v.z; Mi[4 * c + 3] = v.w;
+            }
             const float4 h0 = *reinterpret_cast<const float4 *>(myX);
             const float2 h1 = *reinterpret_cast<const float2 *>(myX + 4);
             const float h[6] = { h0.x, h0.y, h0.z, h0.w, h1.x, h1.y };
-            float Mi[21], kp[6];
-#pragma unroll
-            for (int c = 0; c < 21; c++) Mi[c] = myM[c];
+            float kp[6];
             symv6(Mi, h, kp);
-#pragma unroll
-            for (int a = 0; a < 6; a++) kp[a] -= myM[21 + a];
-            *reinterpret_cast<float4 *>(myX) = make_float4(kp[0], kp[1], kp[2], kp[3]);
-            *reinterpret_cast<float2 *>(myX + 4) = make_float2(kp[4], kp[5]);
+            *reinterpret_cast<float4 *>(myX) = make_float4(kp[0] - Mi[21], kp[1] - Mi[22], kp[2] - Mi[23], kp[3] - Mi[24]);
+            *reinterpret_cast<float2 *>(myX + 4) = make_float2(kp[4] - Mi[25], kp[5] - Mi[26]);
         }
-        if (emit && tid < 20) red[tid] = 0u;
-        __syncthreads();
-        if (warp == 0) forward_pass(L, smem, N, Gv, dt, has_ext, lane, x0g, b0, emit, done, o.x);
-        __syncthreads();
-        // ---- P3: u from w, projection (S4), dual update (S5), residuals (S6)  (lane = stage) --------
+        __syncthreads();                                   // X = kappa
+        if (pass_warp) {
+            if (emit) forward_pass<true>(pl, N, dt, has_ext, pi, x0s + pe * 16, pl.act && !done[pe], oxe);
+            else forward_pass<false>(pl, N, dt, has_ext, pi, x0s + pe * 16, false, oxe);
+        }
+        __syncthreads();                                   // X = w
+        // ---- u from w, projection (S4), dual update (S5), residuals (S6) ----------------------------
         if (tact && !frozen) {
             float u0[NU], G0[6], wv[6], dl[6], lam[6];
             stage_u0<NU>(P, ru, z, y, r, u0, G0);
@@ -669,14 +818,15 @@ __global__ void __launch_bounds__(256) k_iterate_srb(SolveParams P, SrbWs W, con
         }
         if (emit) {
             __syncthreads();
-            if (tid < Gv && !done[tid]) {                  // one leader per env
-                const float rp = __uint_as_float(red[tid * 5 + 0]), rd = P.rho * __uint_as_float(red[tid * 5 + 1]);
-                o.r_prim[b0 + tid] = rp; o.r_dual[b0 + tid] = rd; o.iters_done[b0 + tid] = it + 1;
+            if (tid < Gv && !done[tid]) {        // one leader per env
+                const int e = tid;
+                const float rp = __uint_as_float(red[e * 5 + 0]), rd = P.rho * __uint_as_float(red[e * 5 + 1]);
+                o.r_prim[b0 + e] = rp; o.r_dual[b0 + e] = rd; o.iters_done[b0 + e] = it + 1;
                 if (is_check) {
-                    const float sc = fmaxf(__uint_as_float(red[tid * 5 + 2]), __uint_as_float(red[tid * 5 + 3]));
-                    const float ys = __uint_as_float(red[tid * 5 + 4]);
+                    const float sc = fmaxf(__uint_as_float(red[e * 5 + 2]), __uint_as_float(red[e * 5 + 3]));
+                    const float ys = __uint_as_float(red[e * 5 + 4]);
                     if (rp <= P.eps_abs + P.eps_rel * sc && rd <= P.eps_abs + P.eps_rel * P.rho * ys) {
-                        done[tid] = 1;
+                        done[e] = 1;
                         atomicAdd(ndone, 1);
                     }
                 }
@@ -696,6 +846,7 @@ __global__ void __launch_bounds__(256) k_iterate_srb(SolveParams P, SrbWs W, con
     }
 }
 
+
 // ---------------------------------------------------------------------------------------------
 // launcher
 // ---------------------------------------------------------------------------------------------
@@ -708,28 +859,39 @@ int fail(pinmpc_ctx *h, const char *what, cudaError_t e)
 
 size_t iterate_smem_bytes(int N, int G, int ext)
 {
-    return ((size_t)G * arena_layout(N, ext).stride + CTL_INTS) * sizeof(float);
+    return ((size_t)G * arena_layout(N, ext).stride + CTL_INTS + 16 * G) * sizeof(float);
 }
 
-// envs per CTA: the G in 1..4 that keeps most envs resident per SM (shared memory, registers and
-// thread slots), ties to the smaller CTA (more independent CTAs overlap passes and stage phases).
+int iterate_threads(int N, int G)
+{
+    const int pw = (G + PASS_ENVS - 1) / PASS_ENVS, sw = (G * N + 31) / 32;
+    return 32 * (sw > pw ? sw : pw);
+}
+
+// envs per CTA: fewest rounds of the batch over the device first (envs resident per SM, limited by
+// shared memory, registers and thread slots), then at least two CTAs per SM (their pass and stage
+// phases overlap), then full pass warps (multiples of PASS_ENVS), then the smaller CTA.
 int choose_G(const pinmpc_ctx *h, int regs, int ext)
 {
-    int best = 0, best_envs = 0;
-    for (int G = 1; G <= 4; G++) {
-        int threads = (G * h->N + 31) / 32 * 32;
-        if (threads < 32) threads = 32;
-        size_t smem = iterate_smem_bytes(h->N, G, ext);
-        if (threads > 256 || smem > (size_t)h->smem_optin) continue;
-        int by_smem = (int)((size_t)(228 * 1024) / (smem + 1024));
-        int by_regs = 65536 / (threads * ((regs + 7) / 8 * 8));
-        int by_thr = 2048 / threads;
-        int ctas = by_smem < by_regs ? by_smem : by_regs;
+    int best = 0;
+    long best_score = 0;
+    const int regs_alloc = (regs + 7) / 8 * 8;
+    for (int G = 1; G <= G_MAX; G++) {
+        const int threads = iterate_threads(h->N, G);
+        const size_t smem = iterate_smem_bytes(h->N, G, ext);
+        if (threads > ITER_MAX_THREADS || smem > (size_t)h->smem_optin) continue;
+        int ctas = (int)((size_t)(228 * 1024) / (smem + 1024));
+        const int warps_per_smsp = 16384 / (regs_alloc * 32);          // the register file is per sub-partition
+        const int by_regs = warps_per_smsp * 4 / (threads / 32), by_thr = 2048 / threads;
+        if (by_regs < ctas) ctas = by_regs;
         if (by_thr < ctas) ctas = by_thr;
         if (ctas > 32) ctas = 32;
         if (ctas < 1) continue;
-        int envs = ctas * G;
-        if (envs > best_envs) { best_envs = envs; best = G; }
+        const long per_round = (long)ctas * G * h->sm_count;
+        const long rounds = (h->B + per_round - 1) / per_round;
+        const int pw = (G + PASS_ENVS - 1) / PASS_ENVS;
+        const long score = -rounds * 1000000 + (ctas >= 2 ? 100000 : 0) + (G * 1000L) / (pw * PASS_ENVS) * 10 - G;
+        if (best == 0 || score > best_score) { best_score = score; best = G; }
     }
     return best;
 }
@@ -752,21 +914,19 @@ int launch_t(pinmpc_ctx *h, cudaStream_t st)
     e = cudaFuncGetAttributes(&fa, k_iterate_srb<NU>);
     if (e != cudaSuccess) return fail(h, "k_iterate_srb attributes", e);
     int G = h->envs_per_cta;
-    if (G > 0) {
-        int threads = (G * h->N + 31) / 32 * 32;
-        if (threads > 256 || iterate_smem_bytes(h->N, G, ext) > (size_t)h->smem_optin) G = 0;
-    }
+    if (G > 0 && (iterate_threads(h->N, G) > ITER_MAX_THREADS || iterate_smem_bytes(h->N, G, ext) > (size_t)h->smem_optin)) G = 0;
     if (G == 0) G = choose_G(h, fa.numRegs, ext);
     if (G == 0) {
         snprintf(h->err, sizeof h->err, "structured solver: N=%d needs %zu B of shared memory per env (limit %d)", h->N,
                  iterate_smem_bytes(h->N, 1, ext), h->smem_optin);
         return -1;
     }
-    int threads = (G * h->N + 31) / 32 * 32;
-    size_t smem = iterate_smem_bytes(h->N, G, ext);
+    const int threads = iterate_threads(h->N, G), PW = (G + PASS_ENVS - 1) / PASS_ENVS;
+    const size_t smem = iterate_smem_bytes(h->N, G, ext);
     e = cudaFuncSetAttribute(k_iterate_srb<NU>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_iterate_srb<NU>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
     if (e != cudaSuccess) return fail(h, "k_iterate_srb smem attribute", e);
-    k_iterate_srb<NU><<<(unsigned)((h->B + G - 1) / G), threads, smem, st>>>(P, h->srb, q.x0, q.mass, h->out, G, ext);
+    k_iterate_srb<NU><<<(unsigned)((h->B + G - 1) / G), threads, smem, st>>>(P, h->srb, q.x0, q.mass, h->out, G, PW, ext);
     e = cudaGetLastError();
     if (e != cudaSuccess) return fail(h, "k_iterate_srb launch", e);
     return 3;
