@@ -18,6 +18,11 @@ struct SolveParams {
     float mu, fz_max, cx, cy, cz, hand_fmax;
     float Qd[NX];
     float Rd[NU_MAX];
+    // host-computed reciprocals (no divisions in the iteration kernels)
+    float tR[NU_MAX];     // 1 / (R_j + rho)
+    float rtR[NU_MAX];    // rho / (R_j + rho)
+    float iw[5];          // 1 / (mu, mu, cx, cy, cz)
+    float phi_inv[3];     // 1 / sum_i tR[f_i axis]  (Lam_FF^-1, the same for every stage)
 };
 
 struct ProblemPtrs {
@@ -100,7 +105,17 @@ static inline SolveParams make_params(const pinmpc_ctx *h)
     p.mu = h->layout.mu; p.fz_max = h->layout.fz_max; p.cx = h->layout.mx_coef; p.cy = h->layout.my_coef;
     p.cz = h->layout.mz_coef; p.hand_fmax = h->layout.hand_fmax;
     for (int i = 0; i < NX; i++) p.Qd[i] = h->Qd[i];
-    for (int i = 0; i < NU_MAX; i++) p.Rd[i] = h->Rd[i];
+    for (int i = 0; i < NU_MAX; i++) {
+        p.Rd[i] = h->Rd[i];
+        p.tR[i] = 1.0f / (h->Rd[i] + h->rho);
+        p.rtR[i] = h->rho / (h->Rd[i] + h->rho);
+    }
+    p.iw[0] = p.iw[1] = 1.0f / p.mu; p.iw[2] = 1.0f / p.cx; p.iw[3] = 1.0f / p.cy; p.iw[4] = 1.0f / p.cz;
+    for (int a = 0; a < 3; a++) {
+        float sum = 0.0f;
+        for (int i = 0; i < p.nw + p.nf; i++) sum += p.tR[(i < p.nw ? 3 * i : 6 * p.nw + 3 * (i - p.nw)) + a];
+        p.phi_inv[a] = 1.0f / sum;
+    }
     return p;
 }
 
@@ -174,7 +189,7 @@ __device__ __forceinline__ void project_wrench(const SolveParams &P, float fx, f
                                                float &omz)
 {
     const float w[5] = { P.mu, P.mu, P.cx, P.cy, P.cz };
-    const float iw[5] = { 1.0f / P.mu, 1.0f / P.mu, 1.0f / P.cx, 1.0f / P.cy, 1.0f / P.cz };
+    const float iw[5] = { P.iw[0], P.iw[1], P.iw[2], P.iw[3], P.iw[4] };
     const float a[5] = { fabsf(fx), fabsf(fy), fabsf(mx), fabsf(my), fabsf(mz) };
     float t = wrench_height(fz, a, w, iw);
     t = fminf(fmaxf(t, 0.0f), P.fz_max);

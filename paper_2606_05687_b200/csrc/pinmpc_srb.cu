@@ -100,14 +100,15 @@ __device__ __forceinline__ void dinv_apply(const float *Iw, float idt, float m_d
     o[3] = v[3] * m_dt; o[4] = v[4] * m_dt; o[5] = v[5] * m_dt;
 }
 
-// u0 = Rt^-1 (R ubar + rho (z - y)) and its net wrench G0 = Gh u0 for one stage (thread-local)
+// u0 = Rt^-1 (R ubar + rho (z - y)) and its net wrench G0 = Gh u0 for one stage (thread-local);
+// ru = Rt^-1 R ubar
 template <int NU>
 __device__ __forceinline__ void stage_u0(const SolveParams &P, const float *ru, const float *z, const float *y,
                                          const float *r, float *u0, float *G0)
 {
     constexpr int NC = NW + (NU - 12) / 3;
 #pragma unroll
-    for (int j = 0; j < NU; j++) u0[j] = (ru[j] + P.rho * (z[j] - y[j])) / (P.Rd[j] + P.rho);
+    for (int j = 0; j < NU; j++) u0[j] = fmaf(P.rtR[j], z[j] - y[j], ru[j]);
 #pragma unroll
     for (int a = 0; a < 6; a++) G0[a] = 0.0f;
 #pragma unroll
@@ -123,6 +124,36 @@ __device__ __forceinline__ void stage_u0(const SolveParams &P, const float *ru, 
             G0[0] += m[0]; G0[1] += m[1]; G0[2] += m[2];
         }
     }
+}
+
+// y = Lam^-1 x through the Schur complement of the force block:
+//   y_t = T^-1 (x_t - C Phi^-1 x_F),  y_F = Phi^-1 (x_F - C^T y_t),
+//   C v = sum_i r_i x (t_fi o v),  C^T v = sum_i t_fi o (v x r_i),  Phi = diag(sum_i t_fi)
+template <int NU>
+__device__ __forceinline__ void lam_inv_apply(const SolveParams &P, const float *TI, const float *r, const float *x, float *y)
+{
+    constexpr int NC = NW + (NU - 12) / 3;
+    const float q0 = P.phi_inv[0] * x[3], q1 = P.phi_inv[1] * x[4], q2 = P.phi_inv[2] * x[5];
+    float e0 = x[0], e1 = x[1], e2 = x[2];
+#pragma unroll
+    for (int i = 0; i < NC; i++) {
+        const float rx = r[3 * i], ry = r[3 * i + 1], rz = r[3 * i + 2];
+        const float v0 = P.tR[fcol(i)] * q0, v1 = P.tR[fcol(i) + 1] * q1, v2 = P.tR[fcol(i) + 2] * q2;
+        e0 -= ry * v2 - rz * v1; e1 -= rz * v0 - rx * v2; e2 -= rx * v1 - ry * v0;
+    }
+    const float t0 = TI[0] * e0 + TI[1] * e1 + TI[2] * e2;
+    const float t1 = TI[1] * e0 + TI[3] * e1 + TI[4] * e2;
+    const float t2 = TI[2] * e0 + TI[4] * e1 + TI[5] * e2;
+    float f0 = x[3], f1 = x[4], f2 = x[5];
+#pragma unroll
+    for (int i = 0; i < NC; i++) {
+        const float rx = r[3 * i], ry = r[3 * i + 1], rz = r[3 * i + 2];
+        f0 -= P.tR[fcol(i)] * (t1 * rz - t2 * ry);
+        f1 -= P.tR[fcol(i) + 1] * (t2 * rx - t0 * rz);
+        f2 -= P.tR[fcol(i) + 2] * (t0 * ry - t1 * rx);
+    }
+    y[0] = t0; y[1] = t1; y[2] = t2;
+    y[3] = P.phi_inv[0] * f0; y[4] = P.phi_inv[1] * f1; y[5] = P.phi_inv[2] * f2;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -166,7 +197,7 @@ __global__ void __launch_bounds__(128) k_assemble_srb(SolveParams P, ProblemPtrs
     }
     W.bits[s] = bits;
 #pragma unroll
-    for (int j = 0; j < NU; j++) W.RU[j * st + s] = q.u_ref ? P.Rd[j] * q.u_ref[s * NU + j] : 0.0f;
+    for (int j = 0; j < NU; j++) W.RU[j * st + s] = q.u_ref ? P.tR[j] * P.Rd[j] * q.u_ref[s * NU + j] : 0.0f;
     // q_{k+1} = Q xbar_{k+1}  (x_ref[b,k] holds xbar_{k+1});  q_0 = 0
     {
         float *qv = W.qv + ((long)b * (N + 1) + k + 1) * 12;
@@ -197,9 +228,29 @@ __global__ void __launch_bounds__(128) k_assemble_srb(SolveParams P, ProblemPtrs
             if (i < NW) Lam[sidx(a, a)] += 1.0f / (P.Rd[mcol(i) + a] + P.rho);
         }
     }
-    spd_inv6(Lam);                                   // Lam^-1
+    // T^-1, T = Lam_tt - Lam_tF Lam_FF^-1 Lam_Ft (Schur complement; Lam_FF = diag(1 / phi_inv) for every stage):
+    // the iteration kernel applies Lam^-1 through T^-1 and r (6 + 0 words per stage instead of 21)
+    {
+        float T[6], TI[6];
 #pragma unroll
-    for (int i = 0; i < 21; i++) W.LI[i * st + s] = Lam[i];
+        for (int x = 0; x < 3; x++)
+#pragma unroll
+            for (int y = x; y < 3; y++) {
+                float a = Lam[sidx(x, y)];
+#pragma unroll
+                for (int l = 0; l < 3; l++) a = fmaf(-Lam[sidx(x, 3 + l)] * P.phi_inv[l], Lam[sidx(y, 3 + l)], a);
+                T[x * 3 - x * (x - 1) / 2 + (y - x)] = a;
+            }
+        // symmetric 3x3 inverse (xx,xy,xz,yy,yz,zz)
+        const float c00 = T[3] * T[5] - T[4] * T[4], c01 = T[2] * T[4] - T[1] * T[5], c02 = T[1] * T[4] - T[2] * T[3];
+        const float id = 1.0f / (T[0] * c00 + T[1] * c01 + T[2] * c02);
+        TI[0] = c00 * id; TI[1] = c01 * id; TI[2] = c02 * id;
+        TI[3] = (T[0] * T[5] - T[2] * T[2]) * id; TI[4] = (T[1] * T[2] - T[0] * T[4]) * id;
+        TI[5] = (T[0] * T[3] - T[1] * T[1]) * id;
+#pragma unroll
+        for (int i = 0; i < 6; i++) W.LI[i * st + s] = TI[i];
+    }
+    spd_inv6(Lam);                                   // Lam^-1 (for S below)
     // S = D^-1 Lam^-1 D^-1,  D^-1 = blkdiag(I_w / dt, m/dt I)
     {
         const float Iw3[3][3] = { { iw[0], iw[1], iw[2] }, { iw[1], iw[3], iw[4] }, { iw[2], iw[4], iw[5] } };
@@ -415,10 +466,10 @@ __global__ void __launch_bounds__(FAC_WARPS * 32) k_factor_srb(SolveParams P, co
 // ---------------------------------------------------------------------------------------------
 // S3-S6  ADMM iterations: one CTA per G envs, every factor on chip (v3)
 // ---------------------------------------------------------------------------------------------
-// Every thread owns one (env, stage) and keeps the stage-local data (Lam^-1, I_w, r, R ubar, z, y)
+// STAGE threads own one (env, stage) each and keep the stage-local data (T^-1, I_w, r, ubar, z, y)
 // in registers for all iterations ("stage work": u from w, projection S4, dual update S5,
-// residuals S6, sigma0 of the next iteration, kappa).  The first PW warps of the CTA also run the
-// two sequential vector recursions ("passes") of up to five envs each, six lanes per env
+// residuals S6, sigma0 of the next iteration, kappa).  The first PW warps of the CTA are PASS warps:
+// they run the two sequential vector recursions of up to five envs each, six lanes per env
 // (lane = 6 e + i), exchanging the 6-D quantities with warp shuffles; the gains stream from the
 // env's shared-memory arena through explicit ld.shared with immediate offsets, one stage ahead.
 //
@@ -431,7 +482,7 @@ __global__ void __launch_bounds__(FAC_WARPS * 32) k_factor_srb(SolveParams P, co
 //   C  [N][6]        ch (ext only)
 struct ArenaLay { int oX, oCS, oM, oC, stride; };
 
-constexpr int ITER_MAX_THREADS = 512;  // 16 warps x 128 registers fill the register file of an SM
+constexpr int ITER_MAX_THREADS = 512;  // 16 warps x 128 registers: four warps per SM sub-partition
 constexpr int PASS_ENVS = 5;           // envs per pass warp (6 lanes each)
 constexpr int ARENA_PAD_MOD = 12;      // arena stride mod 32 (bank spread of the 6-lane groups)
 constexpr int G_MAX = 16;              // envs per CTA
@@ -659,7 +710,7 @@ __global__ void __launch_bounds__(ITER_MAX_THREADS) k_iterate_srb(SolveParams P,
     for (int i = tid; i < Gv * 16; i += nthr) x0s[i] = (i & 15) < NX ? x0g[(long)(b0 + (i >> 4)) * NX + (i & 15)] : 0.0f;
 
     // ---- pass role of the first PW warps -----------------------------------------------------------
-    const bool pass_warp = warp < PW && warp * PASS_ENVS < Gv;
+    const bool pass_warp = warp < PW && warp * PASS_ENVS < Gv;   // dedicated: these warps hold no stage state
     PassLane pl;
     int pi = 0, pe = 0;
     {
@@ -680,21 +731,22 @@ __global__ void __launch_bounds__(ITER_MAX_THREADS) k_iterate_srb(SolveParams P,
     float *oxe = o.x + (long)(b0 + pe) * N * NX;
 
     // ---- stage role: this thread's (env, stage) ---------------------------------------------------
-    const int te = tid / N, tk = tid - te * N;
+    const int sid = tid - 32 * PW;                          // stage-thread index (negative in the pass warps)
+    const int te = sid >= 0 ? sid / N : G, tk = sid >= 0 ? sid - te * N : 0;
     const bool tact = te < Gv;
     const int bb = b0 + (tact ? te : 0);
     const long ts = (long)bb * N + tk;
     float *arena = smem + (tact ? te : 0) * L.stride;
     float *myX = arena + L.oX + tk * 8, *myM = arena + L.oM + tk * 28;
 
-    float LI[21], Iw[6], r[3 * NC], ru[NU], z[NU], y[NU];
+    float TI[6], Iw[6], r[3 * NC], ru[NU], z[NU], y[NU];
     int bits = 0;
     float m_dt = 0.0f;
     if (tact) {
 #pragma unroll
-        for (int c = 0; c < 21; c++) { LI[c] = W.LI[c * st + ts]; myM[c] = W.MI[c * st + ts]; }
+        for (int c = 0; c < 21; c++) myM[c] = W.MI[c * st + ts];
 #pragma unroll
-        for (int c = 0; c < 6; c++) { Iw[c] = W.IW[c * st + ts]; myM[21 + c] = W.KG[c * st + ts]; }
+        for (int c = 0; c < 6; c++) { TI[c] = W.LI[c * st + ts]; Iw[c] = W.IW[c * st + ts]; myM[21 + c] = W.KG[c * st + ts]; }
 #pragma unroll
         for (int c = 0; c < 3 * NC; c++) r[c] = W.RR[c * st + ts];
 #pragma unroll
@@ -707,7 +759,7 @@ __global__ void __launch_bounds__(ITER_MAX_THREADS) k_iterate_srb(SolveParams P,
     auto stage_sigma0 = [&]() {
         float u0[NU], G0[6], l0[6], s0[6];
         stage_u0<NU>(P, ru, z, y, r, u0, G0);
-        symv6(LI, G0, l0);
+        lam_inv_apply<NU>(P, TI, r, G0, l0);
         dinv_apply(Iw, idt, m_dt, l0, s0);
         *reinterpret_cast<float4 *>(myX) = make_float4(s0[0], s0[1], s0[2], s0[3]);
         *reinterpret_cast<float2 *>(myX + 4) = make_float2(s0[4], s0[5]);
@@ -760,7 +812,7 @@ __global__ void __launch_bounds__(ITER_MAX_THREADS) k_iterate_srb(SolveParams P,
             dinv_apply(Iw, idt, m_dt, wv, dl);
 #pragma unroll
             for (int a = 0; a < 6; a++) dl[a] -= G0[a];
-            symv6(LI, dl, lam);
+            lam_inv_apply<NU>(P, TI, r, dl, lam);
             // u = u0 + Rt^-1 Gh^T lam :  f_i += lam_tau x r_i + lam_F ;  m_i += lam_tau
             float u[NU];
 #pragma unroll
@@ -770,13 +822,13 @@ __global__ void __launch_bounds__(ITER_MAX_THREADS) k_iterate_srb(SolveParams P,
                 float c1 = lam[2] * rx - lam[0] * rz + lam[4];
                 float c2 = lam[0] * ry - lam[1] * rx + lam[5];
                 const int fc = fcol(i);
-                u[fc] = u0[fc] + c0 / (P.Rd[fc] + P.rho);
-                u[fc + 1] = u0[fc + 1] + c1 / (P.Rd[fc + 1] + P.rho);
-                u[fc + 2] = u0[fc + 2] + c2 / (P.Rd[fc + 2] + P.rho);
+                u[fc] = fmaf(P.tR[fc], c0, u0[fc]);
+                u[fc + 1] = fmaf(P.tR[fc + 1], c1, u0[fc + 1]);
+                u[fc + 2] = fmaf(P.tR[fc + 2], c2, u0[fc + 2]);
                 if (i < NW) {
                     const int mc = mcol(i);
 #pragma unroll
-                    for (int a = 0; a < 3; a++) u[mc + a] = u0[mc + a] + lam[a] / (P.Rd[mc + a] + P.rho);
+                    for (int a = 0; a < 3; a++) u[mc + a] = fmaf(P.tR[mc + a], lam[a], u0[mc + a]);
                 }
             }
             float zn[NU];
@@ -818,8 +870,8 @@ __global__ void __launch_bounds__(ITER_MAX_THREADS) k_iterate_srb(SolveParams P,
         }
         if (emit) {
             __syncthreads();
-            if (tid < Gv && !done[tid]) {        // one leader per env
-                const int e = tid;
+            if (sid >= 0 && sid < Gv && !done[sid]) {        // one leader per env
+                const int e = sid;
                 const float rp = __uint_as_float(red[e * 5 + 0]), rd = P.rho * __uint_as_float(red[e * 5 + 1]);
                 o.r_prim[b0 + e] = rp; o.r_dual[b0 + e] = rd; o.iters_done[b0 + e] = it + 1;
                 if (is_check) {
@@ -865,7 +917,7 @@ size_t iterate_smem_bytes(int N, int G, int ext)
 int iterate_threads(int N, int G)
 {
     const int pw = (G + PASS_ENVS - 1) / PASS_ENVS, sw = (G * N + 31) / 32;
-    return 32 * (sw > pw ? sw : pw);
+    return 32 * (pw + sw);
 }
 
 // envs per CTA: fewest rounds of the batch over the device first (envs resident per SM, limited by
