@@ -476,11 +476,12 @@ __global__ void __launch_bounds__(FAC_WARPS * 32) k_factor_srb(SolveParams P, co
 // Shared-memory arena of one env (offsets in floats):
 //   Kn [N][6][6][2]  pairs -(Kh[r][j], Kh[r][6+j]): row r contiguous (forward pass, lane = row,
 //                    3 x LDS.128), pair [r][i] (backward pass, lane = column pair, 6 x LDS.64)
-//   X  [N][8]        exchange vector: sigma0 -> hh -> kappa -> w
-//   CS [N][2]        cos, sin of the linearisation yaw
+//   X  [N][8]        exchange record [v0 v1 cos sin v2 v3 v4 v5], v: sigma0 -> hh -> kappa -> w;
+//                    cos, sin of the linearisation yaw ride along (one LDS.128 serves lanes 0, 1)
 //   M  [N][28]       Mh^-1 packed symmetric (21), kg = Kh[:,12] x_12 - Mh^-1 hq (6), pad
 //   C  [N][6]        ch (ext only)
-struct ArenaLay { int oX, oCS, oM, oC, stride; };
+//   F  [2][8]        forward-pass exchange scratch (new omega, v), two slots
+struct ArenaLay { int oX, oM, oC, oF, stride; };
 
 constexpr int ITER_MAX_THREADS = 512;  // 16 warps x 128 registers: four warps per SM sub-partition
 constexpr int PASS_ENVS = 5;           // envs per pass warp (6 lanes each)
@@ -492,10 +493,10 @@ __host__ __device__ inline ArenaLay arena_layout(int N, int ext)
 {
     ArenaLay L;
     L.oX = 72 * N;
-    L.oCS = L.oX + 8 * N;
-    L.oM = (L.oCS + 2 * N + 3) & ~3;
+    L.oM = L.oX + 8 * N;
     L.oC = L.oM + 28 * N;
-    int size = (L.oC + (ext ? 6 * N : 0) + 3) & ~3;
+    L.oF = (L.oC + (ext ? 6 * N : 0) + 3) & ~3;
+    int size = L.oF + 16;
     L.stride = size + ((ARENA_PAD_MOD - (size & 31)) & 31);
     return L;
 }
@@ -504,61 +505,72 @@ __host__ __device__ inline ArenaLay arena_layout(int N, int ext)
 template <int OFF> __device__ __forceinline__ float lds1(unsigned a)
 {
     float v;
-    asm volatile("ld.shared.f32 %0, [%1+%2];" : "=f"(v) : "r"(a), "n"(OFF));
+    asm volatile("ld.shared.f32 %0, [%1+%2];" : "=f"(v) : "r"(a), "n"(OFF) : "memory");
     return v;
 }
 template <int OFF> __device__ __forceinline__ float2 lds2(unsigned a)
 {
     float2 v;
-    asm volatile("ld.shared.v2.f32 {%0,%1}, [%2+%3];" : "=f"(v.x), "=f"(v.y) : "r"(a), "n"(OFF));
+    asm volatile("ld.shared.v2.f32 {%0,%1}, [%2+%3];" : "=f"(v.x), "=f"(v.y) : "r"(a), "n"(OFF) : "memory");
     return v;
 }
 template <int OFF> __device__ __forceinline__ float4 lds4(unsigned a)
 {
     float4 v;
-    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4+%5];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a), "n"(OFF));
+    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4+%5];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a), "n"(OFF) : "memory");
     return v;
 }
 template <int OFF> __device__ __forceinline__ void sts1(unsigned a, float v)
 {
-    asm volatile("st.shared.f32 [%0+%1], %2;" ::"r"(a), "n"(OFF), "f"(v));
+    asm volatile("st.shared.f32 [%0+%1], %2;" ::"r"(a), "n"(OFF), "f"(v) : "memory");
 }
 
-// lane-constant description of a pass lane
+// word of component i inside the 8-word exchange record  [v0 v1 cos sin v2 v3 v4 v5]
+__host__ __device__ constexpr int xslot(int i) { return i < 2 ? i : i + 2; }
+
+// lane-constant description of a pass lane (lane = 6 e + i)
 struct PassLane {
-    unsigned aK_b, aK_f, aX, aCS, aC;   // shared addresses at stage 0: Kn pair [.][i], Kn row i, X[.][i], CS, C[.][i]
-    int src[6];                         // lanes of the env's group
-    int nb;                             // lane holding the other component of the (roll, pitch) pair
-    float m, om, sg;                    // i < 2 ? 1 : 0 ;  1 - m ;  -1, +1, 0 for i = 0, 1, >= 2
+    unsigned aK_b, aK_f;     // Kn pair [.][i] (backward), Kn row i (forward), stage 0
+    unsigned aXr, aXo, aXq;  // X record of stage 0: base, own slot, the quad holding the own slot
+    unsigned aC;             // ch[.][i] (ext)
+    int src[6];              // lanes of the env's group
+    int nb;                  // lane holding the other component of the (roll, pitch) pair
+    int q;                   // own component inside the quad
+    float m, om, sg;         // i < 2 ? 1 : 0 ;  1 - m ;  -1, +1, 0 for i = 0, 1, >= 2
     bool act;
 };
 
-constexpr int SB_K = 72 * 4, SB_X = 8 * 4, SB_CS = 2 * 4, SB_C = 6 * 4;   // bytes per stage of the arena sections
+constexpr int SB_K = 72 * 4, SB_X = 8 * 4, SB_C = 6 * 4;   // bytes per stage of the arena sections
 
 // ---- backward vector pass (the part of the costate driven by sigma0; the response to q and s is
 // iteration-invariant and folded into kg by the factorisation).  Lane (e, i) owns component i of
 // the (Theta, p) part pq and of the (omega, v) part pv.  Per stage k = N-1..0:
 //   hh = sigma0_k + pv -> X_k ;  pq <- pq - Kq^T hh ;  pv <- pv + dt rot(pq) - Kv^T hh
-struct BwdOps { float2 k[6]; float s0; float2 cs; };
+// Instruction order inside a step: the exchange shuffles of the dependent chain go first, the
+// operand loads of the next stage are issued in their shadow.
+struct BwdOps { float2 k[6]; float4 xq; };
 
-template <int D> __device__ __forceinline__ void bwd_load(BwdOps &o, unsigned aK, unsigned aX, unsigned aCS)
+template <int D> __device__ __forceinline__ void bwd_load(BwdOps &o, unsigned aK, unsigned aXq)
 {
     o.k[0] = lds2<D * SB_K + 0 * 48>(aK); o.k[1] = lds2<D * SB_K + 1 * 48>(aK); o.k[2] = lds2<D * SB_K + 2 * 48>(aK);
     o.k[3] = lds2<D * SB_K + 3 * 48>(aK); o.k[4] = lds2<D * SB_K + 4 * 48>(aK); o.k[5] = lds2<D * SB_K + 5 * 48>(aK);
-    o.s0 = lds1<D * SB_X>(aX);
-    o.cs = lds2<D * SB_CS>(aCS);
+    o.xq = lds4<D * SB_X>(aXq);
 }
 
-template <int D> __device__ __forceinline__ void bwd_step(const BwdOps &o, float &pq, float &pv, const PassLane &p, unsigned aX, float dt)
+template <int D, bool NEXT>
+__device__ __forceinline__ void bwd_step(const BwdOps &o, BwdOps &nxt, float &pq, float &pv, const PassLane &p, unsigned aK, unsigned aXq,
+                                         unsigned aXo, float dt)
 {
-    const float hown = o.s0 + pv;
-    if (p.act) sts1<D * SB_X>(aX, hown);
+    const float s0 = p.q == 0 ? o.xq.x : p.q == 1 ? o.xq.y : p.q == 2 ? o.xq.z : o.xq.w;
+    const float hown = s0 + pv;
     float hh[6];
 #pragma unroll
     for (int r = 0; r < 6; r++) hh[r] = __shfl_sync(FULL, hown, p.src[r]);
     const float oth = __shfl_sync(FULL, pq, p.nb);
-    // off the chain: (A^T p)_v = pv + dt (R_z pq_Theta ; pq_p)
-    const float al = fmaf(p.m, o.cs.x, p.om), be = p.sg * o.cs.y;
+    if (p.act) sts1<D * SB_X>(aXo, hown);
+    if (NEXT) bwd_load<D - 1>(nxt, aK, aXq);
+    // off the chain: (A^T p)_v = pv + dt (R_z pq_Theta ; pq_p)   (cos, sin ride in the quad of lanes 0, 1)
+    const float al = fmaf(p.m, o.xq.z, p.om), be = p.sg * o.xq.w;
     const float basev = fmaf(dt, fmaf(be, oth, al * pq), pv);
     float a0 = fmaf(o.k[0].x, hh[0], pq), a1 = o.k[3].x * hh[3];
     float b0 = fmaf(o.k[0].y, hh[0], basev), b1 = o.k[3].y * hh[3];
@@ -570,71 +582,74 @@ template <int D> __device__ __forceinline__ void bwd_step(const BwdOps &o, float
 
 __device__ __forceinline__ void backward_pass(const PassLane &p, int N, float dt)
 {
-    unsigned aK = p.aK_b + (N - 1) * SB_K, aX = p.aX + (N - 1) * SB_X, aCS = p.aCS + (N - 1) * SB_CS;
+    unsigned aK = p.aK_b + (N - 1) * SB_K, aXq = p.aXq + (N - 1) * SB_X, aXo = p.aXo + (N - 1) * SB_X;
     float pq = 0.0f, pv = 0.0f;
     BwdOps A, B;
-    bwd_load<0>(A, aK, aX, aCS);
+    bwd_load<0>(A, aK, aXq);
     int k = N - 1;
-    for (; k >= 3; k -= 2) {
-        bwd_load<-1>(B, aK, aX, aCS);
-        bwd_step<0>(A, pq, pv, p, aX, dt);
-        bwd_load<-2>(A, aK, aX, aCS);
-        bwd_step<-1>(B, pq, pv, p, aX, dt);
-        aK -= 2 * SB_K; aX -= 2 * SB_X; aCS -= 2 * SB_CS;
+    for (; k >= 2; k -= 2) {
+        bwd_step<0, true>(A, B, pq, pv, p, aK, aXq, aXo, dt);
+        bwd_step<-1, true>(B, A, pq, pv, p, aK, aXq, aXo, dt);
+        aK -= 2 * SB_K; aXq -= 2 * SB_X; aXo -= 2 * SB_X;
     }
-    if (k == 2) {
-        bwd_load<-1>(B, aK, aX, aCS);
-        bwd_step<0>(A, pq, pv, p, aX, dt);
-        bwd_load<-2>(A, aK, aX, aCS);
-        bwd_step<-1>(B, pq, pv, p, aX, dt);
-        bwd_step<-2>(A, pq, pv, p, aX, dt);
-    } else if (k == 1) {
-        bwd_load<-1>(B, aK, aX, aCS);
-        bwd_step<0>(A, pq, pv, p, aX, dt);
-        bwd_step<-1>(B, pq, pv, p, aX, dt);
+    if (k == 1) {
+        bwd_step<0, true>(A, B, pq, pv, p, aK, aXq, aXo, dt);
+        bwd_step<-1, false>(B, A, pq, pv, p, aK, aXq, aXo, dt);
     } else {
-        bwd_step<0>(A, pq, pv, p, aX, dt);
+        bwd_step<0, false>(A, B, pq, pv, p, aK, aXq, aXo, dt);
     }
 }
 
 // ---- forward rollout.  Every lane of env e holds the whole state (the (Theta, p) part is advanced
-// redundantly, the (omega, v) part is exchanged); lane i owns row i of Kh and the new component
-// 6 + i.  Per stage k = 0..N-1:   w = kappa_k - Kh x -> X_k ;  x+ = A x + E (w + ch)
+// redundantly, the (omega, v) part is exchanged with shuffles); lane i owns row i of Kh and the new
+// component 6 + i.  Per stage k = 0..N-1:   w = kappa_k - Kh x -> X_k ;  x+ = A x + E (w + ch)
+// Software pipeline: the part of w_{k+1} that does not depend on the new (omega, v) is computed in
+// the shadow of the exchange of stage k; operands are loaded two stages ahead (reads may run up
+// to two stages past the horizon: still inside the arena, never used).
 struct FwdOps { float4 r0, r1, r2; float kap, c; float2 cs; };
 
-template <int D> __device__ __forceinline__ void fwd_load(FwdOps &o, unsigned aK, unsigned aX, unsigned aCS, unsigned aC, int has_ext, float gdt)
+template <int D> __device__ __forceinline__ void fwd_load(FwdOps &o, unsigned aK, unsigned aXo, unsigned aXr, unsigned aC, int has_ext, float gdt)
 {
     o.r0 = lds4<D * SB_K>(aK); o.r1 = lds4<D * SB_K + 16>(aK); o.r2 = lds4<D * SB_K + 32>(aK);
-    o.kap = lds1<D * SB_X>(aX);
-    o.cs = lds2<D * SB_CS>(aCS);
+    o.kap = lds1<D * SB_X>(aXo);
+    o.cs = lds2<D * SB_X + 8>(aXr);
     o.c = has_ext ? gdt + lds1<D * SB_C>(aC) : gdt;
 }
 
-template <int D, bool EMIT>
-__device__ __forceinline__ void fwd_step(const FwdOps &o, float *xa, float *xb, float &own, const PassLane &p, unsigned aX, float dt,
-                                         int i, bool wr, float *ox, float x12)
+// t = kappa + (Theta, p) columns of -Kh x
+__device__ __forceinline__ float fwd_pre(const FwdOps &o, const float *xa)
 {
-    const float oc = own + o.c;
-    // off the chain: the (Theta, p) columns
     float a0 = fmaf(o.r0.x, xa[0], o.kap), a1 = o.r1.z * xa[3];
     a0 = fmaf(o.r0.z, xa[1], a0); a1 = fmaf(o.r2.x, xa[4], a1);
     a0 = fmaf(o.r1.x, xa[2], a0); a1 = fmaf(o.r2.z, xa[5], a1);
-    const float t = a0 + a1;
+    return a0 + a1;
+}
+
+template <int D, bool EMIT>
+__device__ __forceinline__ void fwd_step(FwdOps &cur, const FwdOps &nxt, float *xa, float *xb, float &own, float &t, const PassLane &p,
+                                         unsigned aK, unsigned aXo, unsigned aXr, unsigned aC, int has_ext, float gdt, float dt, int i,
+                                         bool wr, float *ox, float x12)
+{
     // on the chain: the (omega, v) columns
-    float b0 = fmaf(o.r0.y, xb[0], t), b1 = o.r1.w * xb[3];
-    b0 = fmaf(o.r0.w, xb[1], b0); b1 = fmaf(o.r2.y, xb[4], b1);
-    b0 = fmaf(o.r1.y, xb[2], b0); b1 = fmaf(o.r2.w, xb[5], b1);
+    float b0 = fmaf(cur.r0.y, xb[0], t), b1 = cur.r1.w * xb[3];
+    b0 = fmaf(cur.r0.w, xb[1], b0); b1 = fmaf(cur.r2.y, xb[4], b1);
+    b0 = fmaf(cur.r1.y, xb[2], b0); b1 = fmaf(cur.r2.w, xb[5], b1);
     const float w = b0 + b1;
-    const float nun = w + oc;
-    if (p.act) sts1<D * SB_X>(aX, w);
+    const float nun = w + (own + cur.c);
+    float nb[6];
+#pragma unroll
+    for (int j = 0; j < 6; j++) nb[j] = __shfl_sync(FULL, nun, p.src[j]);
+    if (p.act) sts1<D * SB_X>(aXo, w);
     // Theta+ = Theta + dt R_z^T omega ; p+ = p + dt v   (old omega, v)
-    xa[0] = fmaf(dt, fmaf(o.cs.x, xb[0], o.cs.y * xb[1]), xa[0]);
-    xa[1] = fmaf(dt, fmaf(o.cs.x, xb[1], -o.cs.y * xb[0]), xa[1]);
+    xa[0] = fmaf(dt, fmaf(cur.cs.x, xb[0], cur.cs.y * xb[1]), xa[0]);
+    xa[1] = fmaf(dt, fmaf(cur.cs.x, xb[1], -cur.cs.y * xb[0]), xa[1]);
 #pragma unroll
     for (int j = 2; j < 6; j++) xa[j] = fmaf(dt, xb[j], xa[j]);
-#pragma unroll
-    for (int j = 0; j < 6; j++) xb[j] = __shfl_sync(FULL, nun, p.src[j]);
+    fwd_load<D + 2>(cur, aK, aXo, aXr, aC, has_ext, gdt);
+    t = fwd_pre(nxt, xa);
     own = nun;
+#pragma unroll
+    for (int j = 0; j < 6; j++) xb[j] = nb[j];
     if (EMIT) {
         if (wr) {
             const float xs = i == 0 ? xa[0] : i == 1 ? xa[1] : i == 2 ? xa[2] : i == 3 ? xa[3] : i == 4 ? xa[4] : xa[5];
@@ -648,7 +663,7 @@ __device__ __forceinline__ void fwd_step(const FwdOps &o, float *xa, float *xb, 
 template <bool EMIT>
 __device__ __forceinline__ void forward_pass(const PassLane &p, int N, float dt, int has_ext, int i, const float *x0s, bool wr, float *ox)
 {
-    unsigned aK = p.aK_f, aX = p.aX, aCS = p.aCS, aC = p.aC;
+    unsigned aK = p.aK_f, aXo = p.aXo, aXr = p.aXr, aC = p.aC;
     float xa[6], xb[6];
 #pragma unroll
     for (int j = 0; j < 6; j++) { xa[j] = x0s[j]; xb[j] = x0s[6 + j]; }
@@ -656,23 +671,17 @@ __device__ __forceinline__ void forward_pass(const PassLane &p, int N, float dt,
     float own = x0s[6 + i];
     const float gdt = i == 5 ? dt * x12 : 0.0f;
     FwdOps A, B;
-    fwd_load<0>(A, aK, aX, aCS, aC, has_ext, gdt);
+    fwd_load<0>(A, aK, aXo, aXr, aC, has_ext, gdt);
+    fwd_load<1>(B, aK, aXo, aXr, aC, has_ext, gdt);
+    float t = fwd_pre(A, xa);
     int k = 0;
-    for (; k <= N - 3; k += 2) {
-        fwd_load<1>(B, aK, aX, aCS, aC, has_ext, gdt);
-        fwd_step<0, EMIT>(A, xa, xb, own, p, aX, dt, i, wr, ox, x12);
-        fwd_load<2>(A, aK, aX, aCS, aC, has_ext, gdt);
-        fwd_step<1, EMIT>(B, xa, xb, own, p, aX, dt, i, wr, ox, x12);
-        aK += 2 * SB_K; aX += 2 * SB_X; aCS += 2 * SB_CS; aC += 2 * SB_C;
+    for (; k + 1 < N; k += 2) {
+        fwd_step<0, EMIT>(A, B, xa, xb, own, t, p, aK, aXo, aXr, aC, has_ext, gdt, dt, i, wr, ox, x12);
+        fwd_step<1, EMIT>(B, A, xa, xb, own, t, p, aK, aXo, aXr, aC, has_ext, gdt, dt, i, wr, ox, x12);
+        aK += 2 * SB_K; aXo += 2 * SB_X; aXr += 2 * SB_X; aC += 2 * SB_C;
         if (EMIT) ox += 2 * NX;
     }
-    if (k == N - 2) {
-        fwd_load<1>(B, aK, aX, aCS, aC, has_ext, gdt);
-        fwd_step<0, EMIT>(A, xa, xb, own, p, aX, dt, i, wr, ox, x12);
-        fwd_step<1, EMIT>(B, xa, xb, own, p, aX, dt, i, wr, ox, x12);
-    } else {
-        fwd_step<0, EMIT>(A, xa, xb, own, p, aX, dt, i, wr, ox, x12);
-    }
+    if (k < N) fwd_step<0, EMIT>(A, B, xa, xb, own, t, p, aK, aXo, aXr, aC, has_ext, gdt, dt, i, wr, ox, x12);
 }
 
 template <int NU>
@@ -702,7 +711,7 @@ __global__ void __launch_bounds__(ITER_MAX_THREADS) k_iterate_srb(SolveParams P,
             const float4 v = src[i];
             dst[i] = make_float4(-v.x, -v.y, -v.z, -v.w);
         }
-        for (int i = tid; i < N * 2; i += nthr) a[L.oCS + i] = W.cs[s0 * 2 + i];
+        for (int i = tid; i < N * 2; i += nthr) a[L.oX + (i >> 1) * 8 + 2 + (i & 1)] = W.cs[s0 * 2 + i];
         if (has_ext)
             for (int i = tid; i < N * 6; i += nthr) a[L.oC + i] = W.c6[s0 * 6 + i];
     }
@@ -719,12 +728,16 @@ __global__ void __launch_bounds__(ITER_MAX_THREADS) k_iterate_srb(SolveParams P,
         const int e = warp * PASS_ENVS + eloc;
         pl.act = pass_warp && eloc < PASS_ENVS && e < Gv;
         pe = pl.act ? e : (pass_warp ? warp * PASS_ENVS : 0);      // idle lanes shadow the warp's first env
-        const int base = pl.act ? 6 * eloc : 0;
         const unsigned ar = (unsigned)__cvta_generic_to_shared(smem + pe * L.stride);
         pl.aK_b = ar + 8 * pi; pl.aK_f = ar + 48 * pi;
-        pl.aX = ar + 4 * (L.oX + pi); pl.aCS = ar + 4 * L.oCS; pl.aC = ar + 4 * (L.oC + pi);
+        pl.aXr = ar + 4 * L.oX; pl.aXo = pl.aXr + 4 * xslot(pi); pl.aXq = pl.aXr + (pi < 2 ? 0 : 16);
+        pl.q = pi < 2 ? pi : pi - 2;
+        pl.aC = ar + 4 * (L.oC + pi);
+        {
+            const int base = pl.act ? 6 * eloc : 0;
 #pragma unroll
-        for (int r = 0; r < 6; r++) pl.src[r] = base + r;
+            for (int r = 0; r < 6; r++) pl.src[r] = base + r;
+        }
         pl.nb = lane ^ 1;
         pl.m = pi < 2 ? 1.0f : 0.0f; pl.om = 1.0f - pl.m; pl.sg = pi == 0 ? -1.0f : (pi == 1 ? 1.0f : 0.0f);
     }
@@ -761,8 +774,8 @@ __global__ void __launch_bounds__(ITER_MAX_THREADS) k_iterate_srb(SolveParams P,
         stage_u0<NU>(P, ru, z, y, r, u0, G0);
         lam_inv_apply<NU>(P, TI, r, G0, l0);
         dinv_apply(Iw, idt, m_dt, l0, s0);
-        *reinterpret_cast<float4 *>(myX) = make_float4(s0[0], s0[1], s0[2], s0[3]);
-        *reinterpret_cast<float2 *>(myX + 4) = make_float2(s0[4], s0[5]);
+        *reinterpret_cast<float2 *>(myX) = make_float2(s0[0], s0[1]);
+        *reinterpret_cast<float4 *>(myX + 4) = make_float4(s0[2], s0[3], s0[4], s0[5]);
     };
     if (tact) stage_sigma0();
 
@@ -786,13 +799,13 @@ __global__ void __launch_bounds__(ITER_MAX_THREADS) k_iterate_srb(SolveParams P,
                 const float4 v = Mq[c];
                 Mi[4 * c] = v.x; Mi[4 * c + 1] = v.y; Mi[4 * c + 2] = v.z; Mi[4 * c + 3] = v.w;
             }
-            const float4 h0 = *reinterpret_cast<const float4 *>(myX);
-            const float2 h1 = *reinterpret_cast<const float2 *>(myX + 4);
-            const float h[6] = { h0.x, h0.y, h0.z, h0.w, h1.x, h1.y };
+            const float2 h0 = *reinterpret_cast<const float2 *>(myX);
+            const float4 h1 = *reinterpret_cast<const float4 *>(myX + 4);
+            const float h[6] = { h0.x, h0.y, h1.x, h1.y, h1.z, h1.w };
             float kp[6];
             symv6(Mi, h, kp);
-            *reinterpret_cast<float4 *>(myX) = make_float4(kp[0] - Mi[21], kp[1] - Mi[22], kp[2] - Mi[23], kp[3] - Mi[24]);
-            *reinterpret_cast<float2 *>(myX + 4) = make_float2(kp[4] - Mi[25], kp[5] - Mi[26]);
+            *reinterpret_cast<float2 *>(myX) = make_float2(kp[0] - Mi[21], kp[1] - Mi[22]);
+            *reinterpret_cast<float4 *>(myX + 4) = make_float4(kp[2] - Mi[23], kp[3] - Mi[24], kp[4] - Mi[25], kp[5] - Mi[26]);
         }
         __syncthreads();                                   // X = kappa
         if (pass_warp) {
@@ -805,9 +818,9 @@ __global__ void __launch_bounds__(ITER_MAX_THREADS) k_iterate_srb(SolveParams P,
             float u0[NU], G0[6], wv[6], dl[6], lam[6];
             stage_u0<NU>(P, ru, z, y, r, u0, G0);
             {
-                const float4 w0 = *reinterpret_cast<const float4 *>(myX);
-                const float2 w1 = *reinterpret_cast<const float2 *>(myX + 4);
-                wv[0] = w0.x; wv[1] = w0.y; wv[2] = w0.z; wv[3] = w0.w; wv[4] = w1.x; wv[5] = w1.y;
+                const float2 w0 = *reinterpret_cast<const float2 *>(myX);
+                const float4 w1 = *reinterpret_cast<const float4 *>(myX + 4);
+                wv[0] = w0.x; wv[1] = w0.y; wv[2] = w1.x; wv[3] = w1.y; wv[4] = w1.z; wv[5] = w1.w;
             }
             dinv_apply(Iw, idt, m_dt, wv, dl);
 #pragma unroll
