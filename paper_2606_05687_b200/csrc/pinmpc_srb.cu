@@ -478,25 +478,26 @@ __global__ void __launch_bounds__(FAC_WARPS * 32) k_factor_srb(SolveParams P, co
 //                    3 x LDS.128), pair [r][i] (backward pass, lane = column pair, 6 x LDS.64)
 //   X  [N][8]        exchange record [v0 v1 cos sin v2 v3 v4 v5], v: sigma0 -> hh -> kappa -> w;
 //                    cos, sin of the linearisation yaw ride along (one LDS.128 serves lanes 0, 1)
-//   M  [N][28]       Mh^-1 packed symmetric (21), kg = Kh[:,12] x_12 - Mh^-1 hq (6), pad
+//   ZY [2 nu][N]     z and y of every stage, component-major (read and written once per iteration by the
+//                    stage threads: they hold them in registers only while they work on the stage)
 //   C  [N][6]        ch (ext only)
-//   F  [2][8]        forward-pass exchange scratch (new omega, v), two slots
-struct ArenaLay { int oX, oM, oC, oF, stride; };
+// Mh^-1 and kg (27 words per stage) stay in global memory (L2-resident): the stage threads fetch them
+// while the backward pass runs.
+struct ArenaLay { int oX, oZ, oC, stride; };
 
-constexpr int ITER_MAX_THREADS = 512;  // 16 warps x 128 registers: four warps per SM sub-partition
+constexpr int ITER_MAX_THREADS = 640;  // 20 warps x 96 registers: five warps per SM sub-partition
 constexpr int PASS_ENVS = 5;           // envs per pass warp (6 lanes each)
 constexpr int ARENA_PAD_MOD = 12;      // arena stride mod 32 (bank spread of the 6-lane groups)
 constexpr int G_MAX = 16;              // envs per CTA
 constexpr int CTL_INTS = 32 + 5 * G_MAX;   // done[16] | ndone | pad[15] | red[16][5]
 
-__host__ __device__ inline ArenaLay arena_layout(int N, int ext)
+__host__ __device__ inline ArenaLay arena_layout(int N, int ext, int nu)
 {
     ArenaLay L;
     L.oX = 72 * N;
-    L.oM = L.oX + 8 * N;
-    L.oC = L.oM + 28 * N;
-    L.oF = (L.oC + (ext ? 6 * N : 0) + 3) & ~3;
-    int size = L.oF + 16;
+    L.oZ = L.oX + 8 * N;
+    L.oC = L.oZ + 2 * nu * N;
+    int size = (L.oC + (ext ? 6 * N : 0) + 8 + 3) & ~3;    // + 8: the forward pass reads up to two stages past the horizon
     L.stride = size + ((ARENA_PAD_MOD - (size & 31)) & 31);
     return L;
 }
@@ -692,7 +693,7 @@ __global__ void __launch_bounds__(ITER_MAX_THREADS) k_iterate_srb(SolveParams P,
     extern __shared__ __align__(16) float smem[];
     const int N = P.N, tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, warp = tid >> 5;
     const long st = (long)P.B * N;
-    const ArenaLay L = arena_layout(N, has_ext);
+    const ArenaLay L = arena_layout(N, has_ext, NU);
     const int b0 = blockIdx.x * G;
     const int Gv = min(G, P.B - b0);
     int *ctl = reinterpret_cast<int *>(smem + G * L.stride);
@@ -743,35 +744,64 @@ __global__ void __launch_bounds__(ITER_MAX_THREADS) k_iterate_srb(SolveParams P,
     }
     float *oxe = o.x + (long)(b0 + pe) * N * NX;
 
-    // ---- stage role: this thread's (env, stage) ---------------------------------------------------
-    const int sid = tid - 32 * PW;                          // stage-thread index (negative in the pass warps)
-    const int te = sid >= 0 ? sid / N : G, tk = sid >= 0 ? sid - te * N : 0;
+    const bool tol_mode = (P.eps_abs > 0.0f || P.eps_rel > 0.0f) && P.check_every > 0;
+    if (warp < PW) {
+        // =========================== PASS WARP: the sequential recursions, nothing else =============
+        for (int it = 0; it < P.iters; it++) {
+            const bool is_check = tol_mode && ((it + 1) % P.check_every == 0);
+            const bool emit = (it == P.iters - 1) || is_check;
+            __syncthreads();                               // X = sigma0 of every stage is in place
+            if (pass_warp) backward_pass(pl, N, dt);
+            __syncthreads();                               // X = hh
+            __syncthreads();                               // X = kappa
+            if (pass_warp) {
+                if (emit) forward_pass<true>(pl, N, dt, has_ext, pi, x0s + pe * 16, pl.act && !done[pe], oxe);
+                else forward_pass<false>(pl, N, dt, has_ext, pi, x0s + pe * 16, false, oxe);
+            }
+            __syncthreads();                               // X = w
+            if (emit) {
+                __syncthreads();                           // residuals reduced
+                __syncthreads();                           // done flags updated
+                if (is_check && *ndone == Gv) break;
+            }
+        }
+        return;
+    }
+
+    // ---- STAGE THREADS: this thread's (env, stage) ---------------------------------------------------
+    const int sid = tid - 32 * PW, nstage = nthr - 32 * PW;  // stage-thread index
+    const int te = sid / N, tk = sid - te * N;
     const bool tact = te < Gv;
     const int bb = b0 + (tact ? te : 0);
     const long ts = (long)bb * N + tk;
     float *arena = smem + (tact ? te : 0) * L.stride;
-    float *myX = arena + L.oX + tk * 8, *myM = arena + L.oM + tk * 28;
+    float *myX = arena + L.oX + tk * 8, *myZ = arena + L.oZ + tk;   // z_j at myZ[j N], y_j at myZ[(NU + j) N]
 
-    float TI[6], Iw[6], r[3 * NC], ru[NU], z[NU], y[NU];
+    float TI[6], Iw[6], r[3 * NC], ru[NU];
     int bits = 0;
     float m_dt = 0.0f;
     if (tact) {
 #pragma unroll
-        for (int c = 0; c < 21; c++) myM[c] = W.MI[c * st + ts];
-#pragma unroll
-        for (int c = 0; c < 6; c++) { TI[c] = W.LI[c * st + ts]; Iw[c] = W.IW[c * st + ts]; myM[21 + c] = W.KG[c * st + ts]; }
+        for (int c = 0; c < 6; c++) { TI[c] = W.LI[c * st + ts]; Iw[c] = W.IW[c * st + ts]; }
 #pragma unroll
         for (int c = 0; c < 3 * NC; c++) r[c] = W.RR[c * st + ts];
 #pragma unroll
-        for (int c = 0; c < NU; c++) { ru[c] = W.RU[c * st + ts]; z[c] = 0.0f; y[c] = 0.0f; }
+        for (int c = 0; c < NU; c++) { ru[c] = W.RU[c * st + ts]; myZ[c * N] = 0.0f; myZ[(NU + c) * N] = 0.0f; }
         bits = W.bits[ts];
         m_dt = massg[bb] / dt;
     }
 
-    // X_k = sigma0 = D^-1 Lam^-1 Gh u0 of the coming iteration from the current z, y
+    // G0 = Gh u0 of the coming iteration (u0 = Rt^-1 (R ubar + rho (z - y)); z = y = 0 at the start)
+    float G0[6] = { 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f };
+    if (tact) {
+        float zz[NU], u0[NU];
+#pragma unroll
+        for (int j = 0; j < NU; j++) zz[j] = 0.0f;
+        stage_u0<NU>(P, ru, zz, zz, r, u0, G0);
+    }
+    // X_k = sigma0 = D^-1 Lam^-1 G0
     auto stage_sigma0 = [&]() {
-        float u0[NU], G0[6], l0[6], s0[6];
-        stage_u0<NU>(P, ru, z, y, r, u0, G0);
+        float l0[6], s0[6];
         lam_inv_apply<NU>(P, TI, r, G0, l0);
         dinv_apply(Iw, idt, m_dt, l0, s0);
         *reinterpret_cast<float2 *>(myX) = make_float2(s0[0], s0[1]);
@@ -779,26 +809,25 @@ __global__ void __launch_bounds__(ITER_MAX_THREADS) k_iterate_srb(SolveParams P,
     };
     if (tact) stage_sigma0();
 
-    const bool tol_mode = (P.eps_abs > 0.0f || P.eps_rel > 0.0f) && P.check_every > 0;
     bool frozen = false;          // this thread's env has met the tolerances (tolerance mode only)
 
     for (int it = 0; it < P.iters; it++) {
         const bool is_check = tol_mode && ((it + 1) % P.check_every == 0);
         const bool emit = (it == P.iters - 1) || is_check;
         if (emit)
-            for (int i = tid; i < 5 * G_MAX; i += nthr) red[i] = 0u;
-        __syncthreads();                                   // X = sigma0 of every stage is in place
-        if (pass_warp) backward_pass(pl, N, dt);
+            for (int i = sid; i < 5 * G_MAX; i += nstage) red[i] = 0u;
+        // Mh^-1 and kg of this stage: in flight while the backward pass runs
+        float Mi[27];
+        if (tact) {
+#pragma unroll
+            for (int c = 0; c < 21; c++) Mi[c] = __ldg(W.MI + c * st + ts);
+#pragma unroll
+            for (int c = 0; c < 6; c++) Mi[21 + c] = __ldg(W.KG + c * st + ts);
+        }
+        __syncthreads();                                   // X = sigma0 of every stage is in place: backward pass
         __syncthreads();                                   // X = hh
         // ---- kappa = Mh^-1 hh - kg ---------------------------------------------------------------------
         if (tact) {
-            const float4 *Mq = reinterpret_cast<const float4 *>(myM);
-            float Mi[28];
-#pragma unroll
-            for (int c = 0; c < 7; c++) {
-                const float4 v = Mq[c];
-                Mi[4 * c] = v.x; Mi[4 * c + 1] = v.y; Mi[4 * c + 2] = v.z; Mi[4 * c + 3] = v.w;
-            }
             const float2 h0 = *reinterpret_cast<const float2 *>(myX);
             const float4 h1 = *reinterpret_cast<const float4 *>(myX + 4);
             const float h[6] = { h0.x, h0.y, h1.x, h1.y, h1.z, h1.w };
@@ -807,16 +836,12 @@ __global__ void __launch_bounds__(ITER_MAX_THREADS) k_iterate_srb(SolveParams P,
             *reinterpret_cast<float2 *>(myX) = make_float2(kp[0] - Mi[21], kp[1] - Mi[22]);
             *reinterpret_cast<float4 *>(myX + 4) = make_float4(kp[2] - Mi[23], kp[3] - Mi[24], kp[4] - Mi[25], kp[5] - Mi[26]);
         }
-        __syncthreads();                                   // X = kappa
-        if (pass_warp) {
-            if (emit) forward_pass<true>(pl, N, dt, has_ext, pi, x0s + pe * 16, pl.act && !done[pe], oxe);
-            else forward_pass<false>(pl, N, dt, has_ext, pi, x0s + pe * 16, false, oxe);
-        }
+        __syncthreads();                                   // X = kappa: forward pass
         __syncthreads();                                   // X = w
         // ---- u from w, projection (S4), dual update (S5), residuals (S6) ----------------------------
+        // ---- u from w, projection (S4), dual update (S5), residuals (S6), contact by contact -------------
         if (tact && !frozen) {
-            float u0[NU], G0[6], wv[6], dl[6], lam[6];
-            stage_u0<NU>(P, ru, z, y, r, u0, G0);
+            float wv[6], dl[6], lam[6];
             {
                 const float2 w0 = *reinterpret_cast<const float2 *>(myX);
                 const float4 w1 = *reinterpret_cast<const float4 *>(myX + 4);
@@ -826,64 +851,71 @@ __global__ void __launch_bounds__(ITER_MAX_THREADS) k_iterate_srb(SolveParams P,
 #pragma unroll
             for (int a = 0; a < 6; a++) dl[a] -= G0[a];
             lam_inv_apply<NU>(P, TI, r, dl, lam);
-            // u = u0 + Rt^-1 Gh^T lam :  f_i += lam_tau x r_i + lam_F ;  m_i += lam_tau
-            float u[NU];
-#pragma unroll
-            for (int i = 0; i < NC; i++) {
-                float rx = r[3 * i], ry = r[3 * i + 1], rz = r[3 * i + 2];
-                float c0 = lam[1] * rz - lam[2] * ry + lam[3];
-                float c1 = lam[2] * rx - lam[0] * rz + lam[4];
-                float c2 = lam[0] * ry - lam[1] * rx + lam[5];
-                const int fc = fcol(i);
-                u[fc] = fmaf(P.tR[fc], c0, u0[fc]);
-                u[fc + 1] = fmaf(P.tR[fc + 1], c1, u0[fc + 1]);
-                u[fc + 2] = fmaf(P.tR[fc + 2], c2, u0[fc + 2]);
-                if (i < NW) {
-                    const int mc = mcol(i);
-#pragma unroll
-                    for (int a = 0; a < 3; a++) u[mc + a] = fmaf(P.tR[mc + a], lam[a], u0[mc + a]);
-                }
-            }
-            float zn[NU];
+            float Gn[6] = { 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f };
+            float rp = 0.0f, rd = 0.0f, un = 0.0f, znm = 0.0f, ynm = 0.0f;
+            float *ou = o.u + ts * NU;
 #pragma unroll
             for (int i = 0; i < NC; i++) {
                 const bool on = (bits >> i) & 1;
-                const int fc = fcol(i);
+                const int fc = fcol(i), mc = mcol(i);
+                const float rx = r[3 * i], ry = r[3 * i + 1], rz = r[3 * i + 2];
+                constexpr int NV = 6;                       // f (3) and, for a foot, m (3)
+                const int nv = i < NW ? 6 : 3;
+                int col[NV];
+                float zo[NV], yo[NV], uu[NV], zn[NV];
+#pragma unroll
+                for (int a = 0; a < 3; a++) { col[a] = fc + a; col[3 + a] = mc + a; }
+                // u = u0 + Rt^-1 Gh^T lam :  f_i += lam_tau x r_i + lam_F ;  m_i += lam_tau
+                const float g[NV] = { lam[1] * rz - lam[2] * ry + lam[3], lam[2] * rx - lam[0] * rz + lam[4],
+                                      lam[0] * ry - lam[1] * rx + lam[5], lam[0], lam[1], lam[2] };
+#pragma unroll
+                for (int a = 0; a < NV; a++)
+                    if (a < nv) {
+                        zo[a] = myZ[col[a] * N]; yo[a] = myZ[(NU + col[a]) * N];
+                        const float u0 = fmaf(P.rtR[col[a]], zo[a] - yo[a], ru[col[a]]);
+                        uu[a] = fmaf(P.tR[col[a]], g[a], u0);
+                    }
                 if (i < NW) {
-                    const int mc = mcol(i);
                     float a0, a1, a2, a3, a4, a5;
-                    project_wrench(P, u[fc] + y[fc], u[fc + 1] + y[fc + 1], u[fc + 2] + y[fc + 2], u[mc] + y[mc],
-                                   u[mc + 1] + y[mc + 1], u[mc + 2] + y[mc + 2], a0, a1, a2, a3, a4, a5);
-                    zn[fc] = on ? a0 : 0.0f; zn[fc + 1] = on ? a1 : 0.0f; zn[fc + 2] = on ? a2 : 0.0f;
-                    zn[mc] = on ? a3 : 0.0f; zn[mc + 1] = on ? a4 : 0.0f; zn[mc + 2] = on ? a5 : 0.0f;
+                    project_wrench(P, uu[0] + yo[0], uu[1] + yo[1], uu[2] + yo[2], uu[3] + yo[3], uu[4] + yo[4], uu[5] + yo[5],
+                                   a0, a1, a2, a3, a4, a5);
+                    zn[0] = on ? a0 : 0.0f; zn[1] = on ? a1 : 0.0f; zn[2] = on ? a2 : 0.0f;
+                    zn[3] = on ? a3 : 0.0f; zn[4] = on ? a4 : 0.0f; zn[5] = on ? a5 : 0.0f;
                 } else {
 #pragma unroll
-                    for (int a = 0; a < 3; a++)
-                        zn[fc + a] = on ? fminf(fmaxf(u[fc + a] + y[fc + a], -P.hand_fmax), P.hand_fmax) : 0.0f;
+                    for (int a = 0; a < 3; a++) zn[a] = on ? fminf(fmaxf(uu[a] + yo[a], -P.hand_fmax), P.hand_fmax) : 0.0f;
                 }
-            }
-            if (emit) {
-                float rp = 0.0f, rd = 0.0f, un = 0.0f, znm = 0.0f, ynm = 0.0f;
-                float *ou = o.u + ts * NU;
+                float u0n[NV];
 #pragma unroll
-                for (int j = 0; j < NU; j++) {
-                    rp = fmaxf(rp, fabsf(u[j] - zn[j]));
-                    rd = fmaxf(rd, fabsf(zn[j] - z[j]));
-                    un = fmaxf(un, fabsf(u[j])); znm = fmaxf(znm, fabsf(zn[j]));
-                    ynm = fmaxf(ynm, fabsf(y[j] + u[j] - zn[j]));
-                    ou[j] = u[j];
-                }
+                for (int a = 0; a < NV; a++)
+                    if (a < nv) {
+                        const float yn = yo[a] + uu[a] - zn[a];
+                        myZ[col[a] * N] = zn[a]; myZ[(NU + col[a]) * N] = yn;
+                        if (emit) {
+                            rp = fmaxf(rp, fabsf(uu[a] - zn[a]));
+                            rd = fmaxf(rd, fabsf(zn[a] - zo[a]));
+                            un = fmaxf(un, fabsf(uu[a])); znm = fmaxf(znm, fabsf(zn[a]));
+                            ynm = fmaxf(ynm, fabsf(yn));
+                            ou[col[a]] = uu[a];
+                        }
+                        u0n[a] = fmaf(P.rtR[col[a]], zn[a] - yn, ru[col[a]]);       // u0 of the next iteration
+                    }
+                Gn[0] += ry * u0n[2] - rz * u0n[1]; Gn[1] += rz * u0n[0] - rx * u0n[2]; Gn[2] += rx * u0n[1] - ry * u0n[0];
+                Gn[3] += u0n[0]; Gn[4] += u0n[1]; Gn[5] += u0n[2];
+                if (i < NW) { Gn[0] += u0n[3]; Gn[1] += u0n[4]; Gn[2] += u0n[5]; }
+            }
+#pragma unroll
+            for (int a = 0; a < 6; a++) G0[a] = Gn[a];
+            if (emit) {
                 // non-negative floats order like their bit patterns
                 atomicMax(&red[te * 5 + 0], __float_as_uint(rp)); atomicMax(&red[te * 5 + 1], __float_as_uint(rd));
                 atomicMax(&red[te * 5 + 2], __float_as_uint(un)); atomicMax(&red[te * 5 + 3], __float_as_uint(znm));
                 atomicMax(&red[te * 5 + 4], __float_as_uint(ynm));
             }
-#pragma unroll
-            for (int j = 0; j < NU; j++) { y[j] = y[j] + u[j] - zn[j]; z[j] = zn[j]; }
         }
         if (emit) {
             __syncthreads();
-            if (sid >= 0 && sid < Gv && !done[sid]) {        // one leader per env
+            if (sid < Gv && !done[sid]) {                  // one leader per env
                 const int e = sid;
                 const float rp = __uint_as_float(red[e * 5 + 0]), rd = P.rho * __uint_as_float(red[e * 5 + 1]);
                 o.r_prim[b0 + e] = rp; o.r_dual[b0 + e] = rd; o.iters_done[b0 + e] = it + 1;
@@ -907,7 +939,7 @@ __global__ void __launch_bounds__(ITER_MAX_THREADS) k_iterate_srb(SolveParams P,
     if (tact) {
         float *oz = o.z + ts * NU, *oy = o.y + ts * NU;
 #pragma unroll
-        for (int j = 0; j < NU; j++) { oz[j] = z[j]; oy[j] = y[j]; }
+        for (int j = 0; j < NU; j++) { oz[j] = myZ[j * N]; oy[j] = myZ[(NU + j) * N]; }
     }
 }
 
@@ -922,9 +954,9 @@ int fail(pinmpc_ctx *h, const char *what, cudaError_t e)
     return -1;
 }
 
-size_t iterate_smem_bytes(int N, int G, int ext)
+size_t iterate_smem_bytes(int N, int G, int ext, int nu)
 {
-    return ((size_t)G * arena_layout(N, ext).stride + CTL_INTS + 16 * G) * sizeof(float);
+    return ((size_t)G * arena_layout(N, ext, nu).stride + CTL_INTS + 16 * G) * sizeof(float);
 }
 
 int iterate_threads(int N, int G)
@@ -943,7 +975,7 @@ int choose_G(const pinmpc_ctx *h, int regs, int ext)
     const int regs_alloc = (regs + 7) / 8 * 8;
     for (int G = 1; G <= G_MAX; G++) {
         const int threads = iterate_threads(h->N, G);
-        const size_t smem = iterate_smem_bytes(h->N, G, ext);
+        const size_t smem = iterate_smem_bytes(h->N, G, ext, h->nu);
         if (threads > ITER_MAX_THREADS || smem > (size_t)h->smem_optin) continue;
         int ctas = (int)((size_t)(228 * 1024) / (smem + 1024));
         const int warps_per_smsp = 16384 / (regs_alloc * 32);          // the register file is per sub-partition
@@ -979,15 +1011,15 @@ int launch_t(pinmpc_ctx *h, cudaStream_t st)
     e = cudaFuncGetAttributes(&fa, k_iterate_srb<NU>);
     if (e != cudaSuccess) return fail(h, "k_iterate_srb attributes", e);
     int G = h->envs_per_cta;
-    if (G > 0 && (iterate_threads(h->N, G) > ITER_MAX_THREADS || iterate_smem_bytes(h->N, G, ext) > (size_t)h->smem_optin)) G = 0;
+    if (G > 0 && (iterate_threads(h->N, G) > ITER_MAX_THREADS || iterate_smem_bytes(h->N, G, ext, h->nu) > (size_t)h->smem_optin)) G = 0;
     if (G == 0) G = choose_G(h, fa.numRegs, ext);
     if (G == 0) {
         snprintf(h->err, sizeof h->err, "structured solver: N=%d needs %zu B of shared memory per env (limit %d)", h->N,
-                 iterate_smem_bytes(h->N, 1, ext), h->smem_optin);
+                 iterate_smem_bytes(h->N, 1, ext, h->nu), h->smem_optin);
         return -1;
     }
     const int threads = iterate_threads(h->N, G), PW = (G + PASS_ENVS - 1) / PASS_ENVS;
-    const size_t smem = iterate_smem_bytes(h->N, G, ext);
+    const size_t smem = iterate_smem_bytes(h->N, G, ext, h->nu);
     e = cudaFuncSetAttribute(k_iterate_srb<NU>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_iterate_srb<NU>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
     if (e != cudaSuccess) return fail(h, "k_iterate_srb smem attribute", e);
