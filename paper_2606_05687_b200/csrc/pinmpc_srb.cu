@@ -478,14 +478,12 @@ __global__ void __launch_bounds__(FAC_WARPS * 32) k_factor_srb(SolveParams P, co
 //                    3 x LDS.128), pair [r][i] (backward pass, lane = column pair, 6 x LDS.64)
 //   X  [N][8]        exchange record [v0 v1 cos sin v2 v3 v4 v5], v: sigma0 -> hh -> kappa -> w;
 //                    cos, sin of the linearisation yaw ride along (one LDS.128 serves lanes 0, 1)
-//   ZY [2 nu][N]     z and y of every stage, component-major (read and written once per iteration by the
-//                    stage threads: they hold them in registers only while they work on the stage)
 //   C  [N][6]        ch (ext only)
-// Mh^-1 and kg (27 words per stage) stay in global memory (L2-resident): the stage threads fetch them
-// while the backward pass runs.
-struct ArenaLay { int oX, oZ, oC, stride; };
+// Everything else a stage needs (58 words: Mh^-1, kg, T^-1, I_w, r, ubar', contact bits) stays in the
+// workspace in global memory (L2-resident) and is streamed by the stage threads every iteration.
+struct ArenaLay { int oX, oC, stride; };
 
-constexpr int ITER_MAX_THREADS = 640;  // 20 warps x 96 registers: five warps per SM sub-partition
+constexpr int ITER_MAX_THREADS = 512;  // 16 warps x 128 registers: four warps per SM sub-partition
 constexpr int PASS_ENVS = 5;           // envs per pass warp (6 lanes each)
 constexpr int ARENA_PAD_MOD = 12;      // arena stride mod 32 (bank spread of the 6-lane groups)
 constexpr int G_MAX = 16;              // envs per CTA
@@ -495,8 +493,7 @@ __host__ __device__ inline ArenaLay arena_layout(int N, int ext, int nu)
 {
     ArenaLay L;
     L.oX = 72 * N;
-    L.oZ = L.oX + 8 * N;
-    L.oC = L.oZ + 2 * nu * N;
+    L.oC = L.oX + 8 * N;
     int size = (L.oC + (ext ? 6 * N : 0) + 8 + 3) & ~3;    // + 8: the forward pass reads up to two stages past the horizon
     L.stride = size + ((ARENA_PAD_MOD - (size & 31)) & 31);
     return L;
@@ -685,6 +682,162 @@ __device__ __forceinline__ void forward_pass(const PassLane &p, int N, float dt,
     if (k < N) fwd_step<0, EMIT>(A, B, xa, xb, own, t, p, aK, aXo, aXr, aC, has_ext, gdt, dt, i, wr, ox, x12);
 }
 
+// ---- stage work (one thread, one stage): everything that is local to a stage ------------------------
+// Each stage thread owns STAGES_PER_THREAD stages of one env and keeps only z, y and G0 = Gh u0 of
+// every owned stage in registers; the stage constants (T^-1, I_w, r, ubar', contact bits, Mh^-1, kg:
+// 58 words per stage) are streamed from the L2-resident workspace whenever a phase needs them.
+constexpr int STAGES_PER_THREAD = 2;
+
+template <int NU> struct StageState { float z[NU], y[NU], G0[6]; };
+
+template <int NU> struct StageGeom {
+    float TI[6], Iw[6], r[3 * (NW + (NU - 12) / 3)];
+};
+
+template <int NU> __device__ __forceinline__ void load_geom(const SrbWs &W, long st, long ts, StageGeom<NU> &g)
+{
+    constexpr int NC = NW + (NU - 12) / 3;
+#pragma unroll
+    for (int c = 0; c < 6; c++) { g.TI[c] = __ldg(W.LI + c * st + ts); g.Iw[c] = __ldg(W.IW + c * st + ts); }
+#pragma unroll
+    for (int c = 0; c < 3 * NC; c++) g.r[c] = __ldg(W.RR + c * st + ts);
+}
+
+// X_k = sigma0 = D^-1 Lam^-1 G0
+template <int NU>
+__device__ __forceinline__ void write_sigma0(const SolveParams &P, const StageGeom<NU> &g, const float *G0, float idt, float m_dt, float *myX)
+{
+    float l0[6], s0[6];
+    lam_inv_apply<NU>(P, g.TI, g.r, G0, l0);
+    dinv_apply(g.Iw, idt, m_dt, l0, s0);
+    *reinterpret_cast<float2 *>(myX) = make_float2(s0[0], s0[1]);
+    *reinterpret_cast<float4 *>(myX + 4) = make_float4(s0[2], s0[3], s0[4], s0[5]);
+}
+
+// start of a solve: z = y = 0, u0 = ubar', G0 = Gh u0, sigma0 -> X
+template <int NU>
+__device__ __forceinline__ void stage_init(const SolveParams &P, const SrbWs &W, long st, long ts, StageState<NU> &S, float idt, float m_dt,
+                                           float *myX)
+{
+    constexpr int NC = NW + (NU - 12) / 3;
+    StageGeom<NU> g;
+    load_geom<NU>(W, st, ts, g);
+#pragma unroll
+    for (int j = 0; j < NU; j++) { S.z[j] = 0.0f; S.y[j] = 0.0f; }
+#pragma unroll
+    for (int a = 0; a < 6; a++) S.G0[a] = 0.0f;
+#pragma unroll
+    for (int i = 0; i < NC; i++) {
+        const float rx = g.r[3 * i], ry = g.r[3 * i + 1], rz = g.r[3 * i + 2];
+        const int fc = fcol(i);
+        const float f0 = __ldg(W.RU + (long)fc * st + ts), f1 = __ldg(W.RU + (long)(fc + 1) * st + ts), f2 = __ldg(W.RU + (long)(fc + 2) * st + ts);
+        S.G0[0] += ry * f2 - rz * f1; S.G0[1] += rz * f0 - rx * f2; S.G0[2] += rx * f1 - ry * f0;
+        S.G0[3] += f0; S.G0[4] += f1; S.G0[5] += f2;
+        if (i < NW) {
+            const int mc = mcol(i);
+            S.G0[0] += __ldg(W.RU + (long)mc * st + ts); S.G0[1] += __ldg(W.RU + (long)(mc + 1) * st + ts);
+            S.G0[2] += __ldg(W.RU + (long)(mc + 2) * st + ts);
+        }
+    }
+    write_sigma0<NU>(P, g, S.G0, idt, m_dt, myX);
+}
+
+// kappa = Mh^-1 hh - kg  (X: hh -> kappa)
+__device__ __forceinline__ void stage_kappa(const SrbWs &W, long st, long ts, float *myX)
+{
+    float Mi[27];
+#pragma unroll
+    for (int c = 0; c < 21; c++) Mi[c] = __ldg(W.MI + c * st + ts);
+#pragma unroll
+    for (int c = 0; c < 6; c++) Mi[21 + c] = __ldg(W.KG + c * st + ts);
+    const float2 h0 = *reinterpret_cast<const float2 *>(myX);
+    const float4 h1 = *reinterpret_cast<const float4 *>(myX + 4);
+    const float h[6] = { h0.x, h0.y, h1.x, h1.y, h1.z, h1.w };
+    float kp[6];
+    symv6(Mi, h, kp);
+    *reinterpret_cast<float2 *>(myX) = make_float2(kp[0] - Mi[21], kp[1] - Mi[22]);
+    *reinterpret_cast<float4 *>(myX + 4) = make_float4(kp[2] - Mi[23], kp[3] - Mi[24], kp[4] - Mi[25], kp[5] - Mi[26]);
+}
+
+// u from w, projection (S4), dual update (S5), residuals (S6), contact by contact; then G0 and sigma0 of
+// the next iteration.  res = running maxima (r_prim, |dz|, |u|, |z|, |y|) of this thread's env.
+template <int NU>
+__device__ __forceinline__ void stage_update(const SolveParams &P, const SrbWs &W, long st, long ts, StageState<NU> &S, float idt, float m_dt,
+                                             float *myX, bool update, bool emit, bool next, float *ou, float *res)
+{
+    constexpr int NC = NW + (NU - 12) / 3;
+    StageGeom<NU> g;
+    load_geom<NU>(W, st, ts, g);
+    if (update) {
+        const int bits = __ldg(W.bits + ts);
+        float wv[6], dl[6], lam[6];
+        {
+            const float2 w0 = *reinterpret_cast<const float2 *>(myX);
+            const float4 w1 = *reinterpret_cast<const float4 *>(myX + 4);
+            wv[0] = w0.x; wv[1] = w0.y; wv[2] = w1.x; wv[3] = w1.y; wv[4] = w1.z; wv[5] = w1.w;
+        }
+        dinv_apply(g.Iw, idt, m_dt, wv, dl);
+#pragma unroll
+        for (int a = 0; a < 6; a++) dl[a] -= S.G0[a];
+        lam_inv_apply<NU>(P, g.TI, g.r, dl, lam);
+        float Gn[6] = { 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f };
+#pragma unroll
+        for (int i = 0; i < NC; i++) {
+            const bool on = (bits >> i) & 1;
+            const int fc = fcol(i), mc = mcol(i);
+            const float rx = g.r[3 * i], ry = g.r[3 * i + 1], rz = g.r[3 * i + 2];
+            constexpr int NV = 6;                           // f (3) and, for a foot, m (3)
+            const int nv = i < NW ? 6 : 3;
+            int col[NV];
+            float ru[NV], uu[NV], zn[NV], u0n[NV];
+#pragma unroll
+            for (int a = 0; a < 3; a++) { col[a] = fc + a; col[3 + a] = mc + a; }
+#pragma unroll
+            for (int a = 0; a < NV; a++)
+                if (a < nv) ru[a] = __ldg(W.RU + (long)col[a] * st + ts);
+            // u = u0 + Rt^-1 Gh^T lam :  f_i += lam_tau x r_i + lam_F ;  m_i += lam_tau
+            const float gl[NV] = { lam[1] * rz - lam[2] * ry + lam[3], lam[2] * rx - lam[0] * rz + lam[4],
+                                   lam[0] * ry - lam[1] * rx + lam[5], lam[0], lam[1], lam[2] };
+#pragma unroll
+            for (int a = 0; a < NV; a++)
+                if (a < nv) {
+                    const float u0 = fmaf(P.rtR[col[a]], S.z[col[a]] - S.y[col[a]], ru[a]);
+                    uu[a] = fmaf(P.tR[col[a]], gl[a], u0);
+                }
+            if (i < NW) {
+                float a0, a1, a2, a3, a4, a5;
+                project_wrench(P, uu[0] + S.y[col[0]], uu[1] + S.y[col[1]], uu[2] + S.y[col[2]], uu[3] + S.y[col[3]],
+                               uu[4] + S.y[col[4]], uu[5] + S.y[col[5]], a0, a1, a2, a3, a4, a5);
+                zn[0] = on ? a0 : 0.0f; zn[1] = on ? a1 : 0.0f; zn[2] = on ? a2 : 0.0f;
+                zn[3] = on ? a3 : 0.0f; zn[4] = on ? a4 : 0.0f; zn[5] = on ? a5 : 0.0f;
+            } else {
+#pragma unroll
+                for (int a = 0; a < 3; a++) zn[a] = on ? fminf(fmaxf(uu[a] + S.y[col[a]], -P.hand_fmax), P.hand_fmax) : 0.0f;
+            }
+#pragma unroll
+            for (int a = 0; a < NV; a++)
+                if (a < nv) {
+                    const float yn = S.y[col[a]] + uu[a] - zn[a];
+                    if (emit) {
+                        res[0] = fmaxf(res[0], fabsf(uu[a] - zn[a]));
+                        res[1] = fmaxf(res[1], fabsf(zn[a] - S.z[col[a]]));
+                        res[2] = fmaxf(res[2], fabsf(uu[a])); res[3] = fmaxf(res[3], fabsf(zn[a]));
+                        res[4] = fmaxf(res[4], fabsf(yn));
+                        ou[col[a]] = uu[a];
+                    }
+                    S.z[col[a]] = zn[a]; S.y[col[a]] = yn;
+                    u0n[a] = fmaf(P.rtR[col[a]], zn[a] - yn, ru[a]);               // u0 of the next iteration
+                }
+            Gn[0] += ry * u0n[2] - rz * u0n[1]; Gn[1] += rz * u0n[0] - rx * u0n[2]; Gn[2] += rx * u0n[1] - ry * u0n[0];
+            Gn[3] += u0n[0]; Gn[4] += u0n[1]; Gn[5] += u0n[2];
+            if (i < NW) { Gn[0] += u0n[3]; Gn[1] += u0n[4]; Gn[2] += u0n[5]; }
+        }
+#pragma unroll
+        for (int a = 0; a < 6; a++) S.G0[a] = Gn[a];
+    }
+    if (next) write_sigma0<NU>(P, g, S.G0, idt, m_dt, myX);   // frozen envs keep a well-defined (constant) sigma0
+}
+
 template <int NU>
 __global__ void __launch_bounds__(ITER_MAX_THREADS) k_iterate_srb(SolveParams P, SrbWs W, const float *__restrict__ x0g,
                                                                   const float *__restrict__ massg, OutPtrs o, int G, int PW, int has_ext)
@@ -768,149 +921,44 @@ __global__ void __launch_bounds__(ITER_MAX_THREADS) k_iterate_srb(SolveParams P,
         return;
     }
 
-    // ---- STAGE THREADS: this thread's (env, stage) ---------------------------------------------------
-    const int sid = tid - 32 * PW, nstage = nthr - 32 * PW;  // stage-thread index
-    const int te = sid / N, tk = sid - te * N;
+    // ---- STAGE THREADS: thread (env te, slot tj) owns stages tj and tj + H, H = ceil(N / 2) --------------
+    const int H = (N + STAGES_PER_THREAD - 1) / STAGES_PER_THREAD;
+    const int sid = tid - 32 * PW, nstage = nthr - 32 * PW;
+    const int te = sid / H, tj = sid - te * H;
     const bool tact = te < Gv;
+    const bool act1 = tact && tj + H < N;                     // the second stage exists
     const int bb = b0 + (tact ? te : 0);
-    const long ts = (long)bb * N + tk;
+    const long ts0 = (long)bb * N + tj, ts1 = ts0 + (act1 ? H : 0);
     float *arena = smem + (tact ? te : 0) * L.stride;
-    float *myX = arena + L.oX + tk * 8, *myZ = arena + L.oZ + tk;   // z_j at myZ[j N], y_j at myZ[(NU + j) N]
+    float *myX0 = arena + L.oX + tj * 8, *myX1 = myX0 + (act1 ? H * 8 : 0);
+    const float m_dt = massg[bb] / dt;
 
-    float TI[6], Iw[6], r[3 * NC], ru[NU];
-    int bits = 0;
-    float m_dt = 0.0f;
-    if (tact) {
-#pragma unroll
-        for (int c = 0; c < 6; c++) { TI[c] = W.LI[c * st + ts]; Iw[c] = W.IW[c * st + ts]; }
-#pragma unroll
-        for (int c = 0; c < 3 * NC; c++) r[c] = W.RR[c * st + ts];
-#pragma unroll
-        for (int c = 0; c < NU; c++) { ru[c] = W.RU[c * st + ts]; myZ[c * N] = 0.0f; myZ[(NU + c) * N] = 0.0f; }
-        bits = W.bits[ts];
-        m_dt = massg[bb] / dt;
-    }
-
-    // G0 = Gh u0 of the coming iteration (u0 = Rt^-1 (R ubar + rho (z - y)); z = y = 0 at the start)
-    float G0[6] = { 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f };
-    if (tact) {
-        float zz[NU], u0[NU];
-#pragma unroll
-        for (int j = 0; j < NU; j++) zz[j] = 0.0f;
-        stage_u0<NU>(P, ru, zz, zz, r, u0, G0);
-    }
-    // X_k = sigma0 = D^-1 Lam^-1 G0
-    auto stage_sigma0 = [&]() {
-        float l0[6], s0[6];
-        lam_inv_apply<NU>(P, TI, r, G0, l0);
-        dinv_apply(Iw, idt, m_dt, l0, s0);
-        *reinterpret_cast<float2 *>(myX) = make_float2(s0[0], s0[1]);
-        *reinterpret_cast<float4 *>(myX + 4) = make_float4(s0[2], s0[3], s0[4], s0[5]);
-    };
-    if (tact) stage_sigma0();
-
+    StageState<NU> S0, S1;
+    if (tact) stage_init<NU>(P, W, st, ts0, S0, idt, m_dt, myX0);
+    if (act1) stage_init<NU>(P, W, st, ts1, S1, idt, m_dt, myX1);
     bool frozen = false;          // this thread's env has met the tolerances (tolerance mode only)
 
     for (int it = 0; it < P.iters; it++) {
         const bool is_check = tol_mode && ((it + 1) % P.check_every == 0);
         const bool emit = (it == P.iters - 1) || is_check;
+        const bool next = it + 1 < P.iters;
         if (emit)
             for (int i = sid; i < 5 * G_MAX; i += nstage) red[i] = 0u;
-        // Mh^-1 and kg of this stage: in flight while the backward pass runs
-        float Mi[27];
-        if (tact) {
-#pragma unroll
-            for (int c = 0; c < 21; c++) Mi[c] = __ldg(W.MI + c * st + ts);
-#pragma unroll
-            for (int c = 0; c < 6; c++) Mi[21 + c] = __ldg(W.KG + c * st + ts);
-        }
         __syncthreads();                                   // X = sigma0 of every stage is in place: backward pass
         __syncthreads();                                   // X = hh
-        // ---- kappa = Mh^-1 hh - kg ---------------------------------------------------------------------
-        if (tact) {
-            const float2 h0 = *reinterpret_cast<const float2 *>(myX);
-            const float4 h1 = *reinterpret_cast<const float4 *>(myX + 4);
-            const float h[6] = { h0.x, h0.y, h1.x, h1.y, h1.z, h1.w };
-            float kp[6];
-            symv6(Mi, h, kp);
-            *reinterpret_cast<float2 *>(myX) = make_float2(kp[0] - Mi[21], kp[1] - Mi[22]);
-            *reinterpret_cast<float4 *>(myX + 4) = make_float4(kp[2] - Mi[23], kp[3] - Mi[24], kp[4] - Mi[25], kp[5] - Mi[26]);
-        }
+        if (tact) stage_kappa(W, st, ts0, myX0);
+        if (act1) stage_kappa(W, st, ts1, myX1);
         __syncthreads();                                   // X = kappa: forward pass
         __syncthreads();                                   // X = w
-        // ---- u from w, projection (S4), dual update (S5), residuals (S6) ----------------------------
-        // ---- u from w, projection (S4), dual update (S5), residuals (S6), contact by contact -------------
-        if (tact && !frozen) {
-            float wv[6], dl[6], lam[6];
-            {
-                const float2 w0 = *reinterpret_cast<const float2 *>(myX);
-                const float4 w1 = *reinterpret_cast<const float4 *>(myX + 4);
-                wv[0] = w0.x; wv[1] = w0.y; wv[2] = w1.x; wv[3] = w1.y; wv[4] = w1.z; wv[5] = w1.w;
-            }
-            dinv_apply(Iw, idt, m_dt, wv, dl);
-#pragma unroll
-            for (int a = 0; a < 6; a++) dl[a] -= G0[a];
-            lam_inv_apply<NU>(P, TI, r, dl, lam);
-            float Gn[6] = { 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f };
-            float rp = 0.0f, rd = 0.0f, un = 0.0f, znm = 0.0f, ynm = 0.0f;
-            float *ou = o.u + ts * NU;
-#pragma unroll
-            for (int i = 0; i < NC; i++) {
-                const bool on = (bits >> i) & 1;
-                const int fc = fcol(i), mc = mcol(i);
-                const float rx = r[3 * i], ry = r[3 * i + 1], rz = r[3 * i + 2];
-                constexpr int NV = 6;                       // f (3) and, for a foot, m (3)
-                const int nv = i < NW ? 6 : 3;
-                int col[NV];
-                float zo[NV], yo[NV], uu[NV], zn[NV];
-#pragma unroll
-                for (int a = 0; a < 3; a++) { col[a] = fc + a; col[3 + a] = mc + a; }
-                // u = u0 + Rt^-1 Gh^T lam :  f_i += lam_tau x r_i + lam_F ;  m_i += lam_tau
-                const float g[NV] = { lam[1] * rz - lam[2] * ry + lam[3], lam[2] * rx - lam[0] * rz + lam[4],
-                                      lam[0] * ry - lam[1] * rx + lam[5], lam[0], lam[1], lam[2] };
-#pragma unroll
-                for (int a = 0; a < NV; a++)
-                    if (a < nv) {
-                        zo[a] = myZ[col[a] * N]; yo[a] = myZ[(NU + col[a]) * N];
-                        const float u0 = fmaf(P.rtR[col[a]], zo[a] - yo[a], ru[col[a]]);
-                        uu[a] = fmaf(P.tR[col[a]], g[a], u0);
-                    }
-                if (i < NW) {
-                    float a0, a1, a2, a3, a4, a5;
-                    project_wrench(P, uu[0] + yo[0], uu[1] + yo[1], uu[2] + yo[2], uu[3] + yo[3], uu[4] + yo[4], uu[5] + yo[5],
-                                   a0, a1, a2, a3, a4, a5);
-                    zn[0] = on ? a0 : 0.0f; zn[1] = on ? a1 : 0.0f; zn[2] = on ? a2 : 0.0f;
-                    zn[3] = on ? a3 : 0.0f; zn[4] = on ? a4 : 0.0f; zn[5] = on ? a5 : 0.0f;
-                } else {
-#pragma unroll
-                    for (int a = 0; a < 3; a++) zn[a] = on ? fminf(fmaxf(uu[a] + yo[a], -P.hand_fmax), P.hand_fmax) : 0.0f;
-                }
-                float u0n[NV];
-#pragma unroll
-                for (int a = 0; a < NV; a++)
-                    if (a < nv) {
-                        const float yn = yo[a] + uu[a] - zn[a];
-                        myZ[col[a] * N] = zn[a]; myZ[(NU + col[a]) * N] = yn;
-                        if (emit) {
-                            rp = fmaxf(rp, fabsf(uu[a] - zn[a]));
-                            rd = fmaxf(rd, fabsf(zn[a] - zo[a]));
-                            un = fmaxf(un, fabsf(uu[a])); znm = fmaxf(znm, fabsf(zn[a]));
-                            ynm = fmaxf(ynm, fabsf(yn));
-                            ou[col[a]] = uu[a];
-                        }
-                        u0n[a] = fmaf(P.rtR[col[a]], zn[a] - yn, ru[col[a]]);       // u0 of the next iteration
-                    }
-                Gn[0] += ry * u0n[2] - rz * u0n[1]; Gn[1] += rz * u0n[0] - rx * u0n[2]; Gn[2] += rx * u0n[1] - ry * u0n[0];
-                Gn[3] += u0n[0]; Gn[4] += u0n[1]; Gn[5] += u0n[2];
-                if (i < NW) { Gn[0] += u0n[3]; Gn[1] += u0n[4]; Gn[2] += u0n[5]; }
-            }
-#pragma unroll
-            for (int a = 0; a < 6; a++) G0[a] = Gn[a];
-            if (emit) {
+        {
+            float res[5] = { 0.0f, 0.0f, 0.0f, 0.0f, 0.0f };
+            if (tact) stage_update<NU>(P, W, st, ts0, S0, idt, m_dt, myX0, !frozen, emit, next, o.u + ts0 * NU, res);
+            if (act1) stage_update<NU>(P, W, st, ts1, S1, idt, m_dt, myX1, !frozen, emit, next, o.u + ts1 * NU, res);
+            if (emit && tact && !frozen) {
                 // non-negative floats order like their bit patterns
-                atomicMax(&red[te * 5 + 0], __float_as_uint(rp)); atomicMax(&red[te * 5 + 1], __float_as_uint(rd));
-                atomicMax(&red[te * 5 + 2], __float_as_uint(un)); atomicMax(&red[te * 5 + 3], __float_as_uint(znm));
-                atomicMax(&red[te * 5 + 4], __float_as_uint(ynm));
+                atomicMax(&red[te * 5 + 0], __float_as_uint(res[0])); atomicMax(&red[te * 5 + 1], __float_as_uint(res[1]));
+                atomicMax(&red[te * 5 + 2], __float_as_uint(res[2])); atomicMax(&red[te * 5 + 3], __float_as_uint(res[3]));
+                atomicMax(&red[te * 5 + 4], __float_as_uint(res[4]));
             }
         }
         if (emit) {
@@ -934,15 +982,18 @@ __global__ void __launch_bounds__(ITER_MAX_THREADS) k_iterate_srb(SolveParams P,
                 if (tact) frozen = done[te] != 0;
             }
         }
-        if (tact && it + 1 < P.iters) stage_sigma0();      // frozen envs keep a well-defined (constant) sigma0
     }
     if (tact) {
-        float *oz = o.z + ts * NU, *oy = o.y + ts * NU;
+        float *oz = o.z + ts0 * NU, *oy = o.y + ts0 * NU;
 #pragma unroll
-        for (int j = 0; j < NU; j++) { oz[j] = myZ[j * N]; oy[j] = myZ[(NU + j) * N]; }
+        for (int j = 0; j < NU; j++) { oz[j] = S0.z[j]; oy[j] = S0.y[j]; }
+    }
+    if (act1) {
+        float *oz = o.z + ts1 * NU, *oy = o.y + ts1 * NU;
+#pragma unroll
+        for (int j = 0; j < NU; j++) { oz[j] = S1.z[j]; oy[j] = S1.y[j]; }
     }
 }
-
 
 // ---------------------------------------------------------------------------------------------
 // launcher
@@ -961,8 +1012,8 @@ size_t iterate_smem_bytes(int N, int G, int ext, int nu)
 
 int iterate_threads(int N, int G)
 {
-    const int pw = (G + PASS_ENVS - 1) / PASS_ENVS, sw = (G * N + 31) / 32;
-    return 32 * (pw + sw);
+    const int pw = (G + PASS_ENVS - 1) / PASS_ENVS, H = (N + STAGES_PER_THREAD - 1) / STAGES_PER_THREAD;
+    return 32 * (pw + (G * H + 31) / 32);
 }
 
 // envs per CTA: fewest rounds of the batch over the device first (envs resident per SM, limited by
