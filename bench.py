@@ -48,6 +48,7 @@ def parse():
     ap.add_argument("--method", default="auto", choices=["auto", "srb", "dense"])
     ap.add_argument("--B", type=int, default=None)
     ap.add_argument("--N", type=int, default=None)
+    ap.add_argument("--envs-per-cta", type=int, default=0, help="tuning knob of the structured solver (0 = auto)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -169,6 +170,8 @@ def main():
     s = Solver(w.nu, w.N, w.B, layout=lay, rho=w.rho, iters=w.iters, Qdiag=w.Qdiag, Rdiag=w.Rdiag, dt=w.dt,
                method=method, device=dev)
     s.set_workload(w)
+    if args.envs_per_cta:
+        s.set_tuning(args.envs_per_cta)
     stream = torch.cuda.current_stream(dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
 

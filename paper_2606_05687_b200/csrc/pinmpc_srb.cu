@@ -688,10 +688,11 @@ __device__ __forceinline__ void forward_pass(const PassLane &p, int N, float dt,
 // 58 words per stage) are streamed from the L2-resident workspace whenever a phase needs them.
 constexpr int STAGES_PER_THREAD = 2;
 
-template <int NU> struct StageState { float z[NU], y[NU], G0[6]; };
+template <int NU> struct StageState { float z[NU], y[NU]; };
 
 template <int NU> struct StageGeom {
-    float TI[6], Iw[6], r[3 * (NW + (NU - 12) / 3)];
+    float TI[6], Iw[6], r[3 * (NW + (NU - 12) / 3)], ru[NU];
+    int bits;
 };
 
 template <int NU> __device__ __forceinline__ void load_geom(const SrbWs &W, long st, long ts, StageGeom<NU> &g)
@@ -701,6 +702,9 @@ template <int NU> __device__ __forceinline__ void load_geom(const SrbWs &W, long
     for (int c = 0; c < 6; c++) { g.TI[c] = __ldg(W.LI + c * st + ts); g.Iw[c] = __ldg(W.IW + c * st + ts); }
 #pragma unroll
     for (int c = 0; c < 3 * NC; c++) g.r[c] = __ldg(W.RR + c * st + ts);
+#pragma unroll
+    for (int c = 0; c < NU; c++) g.ru[c] = __ldg(W.RU + c * st + ts);
+    g.bits = __ldg(W.bits + ts);
 }
 
 // X_k = sigma0 = D^-1 Lam^-1 G0
@@ -714,32 +718,18 @@ __device__ __forceinline__ void write_sigma0(const SolveParams &P, const StageGe
     *reinterpret_cast<float4 *>(myX + 4) = make_float4(s0[2], s0[3], s0[4], s0[5]);
 }
 
-// start of a solve: z = y = 0, u0 = ubar', G0 = Gh u0, sigma0 -> X
+// start of a solve: z = y = 0, u0 = ubar', sigma0 -> X
 template <int NU>
 __device__ __forceinline__ void stage_init(const SolveParams &P, const SrbWs &W, long st, long ts, StageState<NU> &S, float idt, float m_dt,
                                            float *myX)
 {
-    constexpr int NC = NW + (NU - 12) / 3;
     StageGeom<NU> g;
     load_geom<NU>(W, st, ts, g);
 #pragma unroll
     for (int j = 0; j < NU; j++) { S.z[j] = 0.0f; S.y[j] = 0.0f; }
-#pragma unroll
-    for (int a = 0; a < 6; a++) S.G0[a] = 0.0f;
-#pragma unroll
-    for (int i = 0; i < NC; i++) {
-        const float rx = g.r[3 * i], ry = g.r[3 * i + 1], rz = g.r[3 * i + 2];
-        const int fc = fcol(i);
-        const float f0 = __ldg(W.RU + (long)fc * st + ts), f1 = __ldg(W.RU + (long)(fc + 1) * st + ts), f2 = __ldg(W.RU + (long)(fc + 2) * st + ts);
-        S.G0[0] += ry * f2 - rz * f1; S.G0[1] += rz * f0 - rx * f2; S.G0[2] += rx * f1 - ry * f0;
-        S.G0[3] += f0; S.G0[4] += f1; S.G0[5] += f2;
-        if (i < NW) {
-            const int mc = mcol(i);
-            S.G0[0] += __ldg(W.RU + (long)mc * st + ts); S.G0[1] += __ldg(W.RU + (long)(mc + 1) * st + ts);
-            S.G0[2] += __ldg(W.RU + (long)(mc + 2) * st + ts);
-        }
-    }
-    write_sigma0<NU>(P, g, S.G0, idt, m_dt, myX);
+    float u0[NU], G0[6];
+    stage_u0<NU>(P, g.ru, S.z, S.y, g.r, u0, G0);
+    write_sigma0<NU>(P, g, G0, idt, m_dt, myX);
 }
 
 // kappa = Mh^-1 hh - kg  (X: hh -> kappa)
@@ -768,8 +758,13 @@ __device__ __forceinline__ void stage_update(const SolveParams &P, const SrbWs &
     constexpr int NC = NW + (NU - 12) / 3;
     StageGeom<NU> g;
     load_geom<NU>(W, st, ts, g);
+    float G0[6];
+    {
+        float u0[NU];
+        stage_u0<NU>(P, g.ru, S.z, S.y, g.r, u0, G0);       // G0 = Gh u0 of the current z, y
+    }
     if (update) {
-        const int bits = __ldg(W.bits + ts);
+        const int bits = g.bits;
         float wv[6], dl[6], lam[6];
         {
             const float2 w0 = *reinterpret_cast<const float2 *>(myX);
@@ -778,7 +773,7 @@ __device__ __forceinline__ void stage_update(const SolveParams &P, const SrbWs &
         }
         dinv_apply(g.Iw, idt, m_dt, wv, dl);
 #pragma unroll
-        for (int a = 0; a < 6; a++) dl[a] -= S.G0[a];
+        for (int a = 0; a < 6; a++) dl[a] -= G0[a];
         lam_inv_apply<NU>(P, g.TI, g.r, dl, lam);
         float Gn[6] = { 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f };
 #pragma unroll
@@ -791,10 +786,12 @@ __device__ __forceinline__ void stage_update(const SolveParams &P, const SrbWs &
             int col[NV];
             float ru[NV], uu[NV], zn[NV], u0n[NV];
 #pragma unroll
+            for (int a = 0; a < NV; a++) ru[a] = 0.0f;
+#pragma unroll
             for (int a = 0; a < 3; a++) { col[a] = fc + a; col[3 + a] = mc + a; }
 #pragma unroll
             for (int a = 0; a < NV; a++)
-                if (a < nv) ru[a] = __ldg(W.RU + (long)col[a] * st + ts);
+                if (a < nv) ru[a] = g.ru[col[a]];
             // u = u0 + Rt^-1 Gh^T lam :  f_i += lam_tau x r_i + lam_F ;  m_i += lam_tau
             const float gl[NV] = { lam[1] * rz - lam[2] * ry + lam[3], lam[2] * rx - lam[0] * rz + lam[4],
                                    lam[0] * ry - lam[1] * rx + lam[5], lam[0], lam[1], lam[2] };
@@ -833,9 +830,9 @@ __device__ __forceinline__ void stage_update(const SolveParams &P, const SrbWs &
             if (i < NW) { Gn[0] += u0n[3]; Gn[1] += u0n[4]; Gn[2] += u0n[5]; }
         }
 #pragma unroll
-        for (int a = 0; a < 6; a++) S.G0[a] = Gn[a];
+        for (int a = 0; a < 6; a++) G0[a] = Gn[a];
     }
-    if (next) write_sigma0<NU>(P, g, S.G0, idt, m_dt, myX);   // frozen envs keep a well-defined (constant) sigma0
+    if (next) write_sigma0<NU>(P, g, G0, idt, m_dt, myX);   // frozen envs keep a well-defined (constant) sigma0
 }
 
 template <int NU>
@@ -953,6 +950,7 @@ __global__ void __launch_bounds__(ITER_MAX_THREADS) k_iterate_srb(SolveParams P,
         {
             float res[5] = { 0.0f, 0.0f, 0.0f, 0.0f, 0.0f };
             if (tact) stage_update<NU>(P, W, st, ts0, S0, idt, m_dt, myX0, !frozen, emit, next, o.u + ts0 * NU, res);
+            asm volatile("" ::: "memory");              // one stage after the other (register pressure)
             if (act1) stage_update<NU>(P, W, st, ts1, S1, idt, m_dt, myX1, !frozen, emit, next, o.u + ts1 * NU, res);
             if (emit && tact && !frozen) {
                 // non-negative floats order like their bit patterns
