@@ -891,6 +891,14 @@ __global__ void __launch_bounds__(ITER_MAX_THREADS) k_iterate_srb(SolveParams P,
         }
         pl.nb = lane ^ 1;
         pl.m = pi < 2 ? 1.0f : 0.0f; pl.om = 1.0f - pl.m; pl.sg = pi == 0 ? -1.0f : (pi == 1 ? 1.0f : 0.0f);
+        // keep the lane constants in registers: opaque to the compiler, so that it cannot rematerialise them
+        // from the lane index inside the pass loops (that costs ~15 instructions per stage of a latency-bound chain)
+#pragma unroll
+        for (int r = 0; r < 6; r++) asm volatile("" : "+r"(pl.src[r]));
+        asm volatile("" : "+r"(pl.nb)); asm volatile("" : "+r"(pl.q));
+        asm volatile("" : "+f"(pl.m)); asm volatile("" : "+f"(pl.om)); asm volatile("" : "+f"(pl.sg));
+        asm volatile("" : "+r"(pl.aK_b)); asm volatile("" : "+r"(pl.aK_f)); asm volatile("" : "+r"(pl.aXr));
+        asm volatile("" : "+r"(pl.aXo)); asm volatile("" : "+r"(pl.aXq)); asm volatile("" : "+r"(pl.aC));
     }
     float *oxe = o.x + (long)(b0 + pe) * N * NX;
 
