@@ -1023,8 +1023,8 @@ int iterate_threads(int N, int G)
 }
 
 // envs per CTA: fewest rounds of the batch over the device first (envs resident per SM, limited by
-// shared memory, registers and thread slots), then at least two CTAs per SM (their pass and stage
-// phases overlap), then full pass warps (multiples of PASS_ENVS), then the smaller CTA.
+// shared memory, registers and thread slots), then full pass warps (multiples of PASS_ENVS: a pass
+// step costs the same for one env as for five), then the larger CTA (fewer pass warps per SM).
 int choose_G(const pinmpc_ctx *h, int regs, int ext)
 {
     int best = 0;
@@ -1044,7 +1044,7 @@ int choose_G(const pinmpc_ctx *h, int regs, int ext)
         const long per_round = (long)ctas * G * h->sm_count;
         const long rounds = (h->B + per_round - 1) / per_round;
         const int pw = (G + PASS_ENVS - 1) / PASS_ENVS;
-        const long score = -rounds * 1000000 + (ctas >= 2 ? 100000 : 0) + (G * 1000L) / (pw * PASS_ENVS) * 10 - G;
+        const long score = -rounds * 1000000 + (G * 1000L) / (pw * PASS_ENVS) * 10 + G;
         if (best == 0 || score > best_score) { best_score = score; best = G; }
     }
     return best;
