@@ -321,7 +321,7 @@ __device__ __forceinline__ float atx(const float *X, int i, int j, float dt, flo
     return a;
 }
 
-__global__ void __launch_bounds__(FAC_WARPS * 32) k_factor_srb(SolveParams P, const float *__restrict__ x0, SrbWs W, int has_ext)
+__global__ void __launch_bounds__(FAC_WARPS * 32, 8) k_factor_srb(SolveParams P, const float *__restrict__ x0, SrbWs W, int has_ext)
 {
     __shared__ __align__(16) float sm_all[FAC_WARPS * FAC_SMEM];
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
