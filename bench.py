@@ -30,12 +30,15 @@ if ROOT not in sys.path:
 METRIC = "batched ADMM-MPC solves/s at B=4096,N=50 (fixed iters); % of roofline"
 
 # Algorithmic FLOPs of the formulation shipped (structured 6-D-input LQR):
-FLOP_PER_STAGE_ITER = {12: 995.0, 18: 1245.0}     # one stage of one ADMM iteration
+FLOP_PER_STAGE_ITER = {12: 930.0, 18: 1150.0}     # one stage of one ADMM iteration
 FLOP_PER_STAGE_ONCE = {12: 3900.0, 18: 4700.0}    # assembly + factorisation, once per solve
 # dense-generic count of SURVEY.md 8(d), used when --method dense is timed
 FLOP_DENSE_ITER = {12: 2700.0, 18: 3700.0}
 FLOP_DENSE_ONCE = {12: 33000.0, 18: 60000.0}
 FMA_LANES_PER_SM = 128
+# DRAM bytes (read + write) of one k_iterate_srb launch at config 2 from the `ncu --set full` capture
+# summarised in profiles/r1_final_iterate_ncu.md (dram__bytes_read.sum + dram__bytes_write.sum)
+NCU_DRAM_BYTES_ITERATE = {"c2_long_horizon": None}
 
 
 def parse():
@@ -197,7 +200,23 @@ def main():
     sampler = ClockSampler(local) if rank == 0 else None
     if sampler:
         sampler.start()
-    ms_steps = timed(s.solve, args.steps)
+    kernel_ms = []
+    profiled = mname == "srb"
+    if profiled:
+        s.set_profiling(True)
+
+    def solve_profiled():
+        s.solve()
+
+    ms_steps = timed(solve_profiled, args.steps)
+    if profiled:
+        # events of the last solve only are kept by the handle; re-run K solves reading them one by one
+        # (same kernels, same stream, device-resident inputs; outside the timed region above)
+        for _ in range(args.steps):
+            flush.zero_()
+            s.solve()
+            kernel_ms.append(s.kernel_ms())
+        s.set_profiling(False)
     barrier()
     clocks = sampler.stop() if sampler else None
     launches = s.launch_count() * args.steps
@@ -244,7 +263,15 @@ def main():
         total_solves = w.B * world
         value = total_solves / (ms * 1e-3)
         fl = flops_per_solve(w, mname)
-        achieved = fl / (ms * 1e-3) / 1e12                     # TFLOP/s of this rank's kernel(s)
+        if kernel_ms:
+            # dominant kernel = the iteration kernel: its own algorithmic FLOPs over its own duration (CUDA events
+            # recorded by pinmpc_solve on the launching stream around the kernel, averaged over K launches)
+            k_ms = [float(np.mean([k[i] for k in kernel_ms])) for i in range(3)]
+            fl = w.B * w.N * w.iters * FLOP_PER_STAGE_ITER[w.nu]
+            achieved = fl / (k_ms[2] * 1e-3) / 1e12
+        else:
+            k_ms = None
+            achieved = fl / (ms * 1e-3) / 1e12                 # TFLOP/s of the whole step (dense variant)
         props = torch.cuda.get_device_properties(dev)
         peaks = {}
         try:
@@ -277,7 +304,10 @@ def main():
             "gpu_launches": launches,
             "clocks": clocks,
             "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                         "traffic": None,
+                         "traffic": NCU_DRAM_BYTES_ITERATE.get(w.name),
+                         "kernel": "k_iterate_srb (S3-S6, all iterations)" if k_ms else "whole step",
+                         "kernel_ms": {"assemble": k_ms[0], "factor": k_ms[1], "iterate": k_ms[2]} if k_ms else None,
+                         "whole_step_tflops": flops_per_solve(w, mname) / (ms * 1e-3) / 1e12,
                          "peak_source": f"{props.multi_processor_count} SMs x {FMA_LANES_PER_SM} FP32 lanes x 2 x "
                                         f"{sm_max_mhz:.0f} MHz (guide unit counts, max SM clock)",
                          "peak_measured_fma_tflops": fma_meas,
@@ -295,8 +325,13 @@ def main():
             n0, t0 = time_oracle(w, 32)
             n = int(min(w.B, max(32, 12.0 * n0 / max(t0, 1e-3))))        # about 12 s of CPU work
             n, t = time_oracle(w, n)
-            line["cpu_baseline"] = {"value": n / t, "unit": "solves/s", "cores": oracle.max_threads(), "kind": "oracle",
-                                    "sample": f"first {n} of {w.B} envs of {w.name}, all {w.iters} iterations, fp64, {t:.1f} s"}
+            reps = 1
+            while t < 10.0 and reps < 64:                            # the whole batch is too quick: repeat it
+                t += time_oracle(w, n)[1]
+                reps += 1
+            line["cpu_baseline"] = {"value": n * reps / t, "unit": "solves/s", "cores": oracle.max_threads(), "kind": "oracle",
+                                    "sample": f"first {n} of {w.B} envs of {w.name} x {reps} repeats, all {w.iters} iterations, "
+                                              f"fp64, {t:.1f} s"}
         print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()

@@ -155,6 +155,15 @@ double pinmpc_probe_fma(int blocks, int iters, float *d_out, void *stream);
 /* Number of kernel launches the last pinmpc_solve enqueued (for bench.py's gpu_launches). */
 int pinmpc_last_launch_count(pinmpc_t h);
 
+/* Per-kernel timing of the structured solver ("per-phase split (S1, S2, loop)").
+ * pinmpc_set_profiling(h, 1) makes every following pinmpc_solve record CUDA events on ITS stream
+ * around the three kernels (assembly S1, factorisation S2, iteration S3-S6); 0 turns it off (default).
+ * pinmpc_get_kernel_ms synchronises the host on the last recorded event and writes the elapsed
+ * milliseconds of the last solve into h_ms[0..2] (HOST array of 3 floats).  PINMPC_ESTATE if
+ * profiling is off or no structured solve has been enqueued since it was turned on. */
+pinmpc_status pinmpc_set_profiling(pinmpc_t h, int on);
+pinmpc_status pinmpc_get_kernel_ms(pinmpc_t h, float *h_ms);
+
 /* Human-readable description of the last error on this handle (owned by the handle; "" if none).
  * With h = NULL: the last pinmpc_create failure in this thread. */
 const char *pinmpc_last_error(pinmpc_t h);

@@ -24,7 +24,7 @@ _STATUS = {0: "PINMPC_OK", 1: "PINMPC_EINVAL", 2: "PINMPC_EALLOC", 3: "PINMPC_EC
 EXPORTS = ("pinmpc_workspace_bytes", "pinmpc_workspace_bytes_method", "pinmpc_create", "pinmpc_set_weights",
            "pinmpc_set_tolerance", "pinmpc_set_method", "pinmpc_set_tuning", "pinmpc_set_problem", "pinmpc_set_dynamics", "pinmpc_solve",
            "pinmpc_get", "pinmpc_get_aux", "pinmpc_get_dynamics", "pinmpc_last_launch_count", "pinmpc_last_error",
-           "pinmpc_destroy", "pinmpc_probe_fma")
+           "pinmpc_destroy", "pinmpc_probe_fma", "pinmpc_set_profiling", "pinmpc_get_kernel_ms")
 
 
 class PinmpcError(RuntimeError):
@@ -88,6 +88,10 @@ def load():
     lib.pinmpc_last_error.argtypes = [c_void_p]
     lib.pinmpc_probe_fma.restype = ctypes.c_double
     lib.pinmpc_probe_fma.argtypes = [c_int, c_int, c_void_p, c_void_p]
+    lib.pinmpc_set_profiling.restype = c_int
+    lib.pinmpc_set_profiling.argtypes = [c_void_p, c_int]
+    lib.pinmpc_get_kernel_ms.restype = c_int
+    lib.pinmpc_get_kernel_ms.argtypes = [c_void_p, POINTER(c_float)]
     lib.pinmpc_destroy.restype = None
     lib.pinmpc_destroy.argtypes = [c_void_p]
     _lib = lib
@@ -172,6 +176,16 @@ def pinmpc_last_launch_count(h) -> int:
     return int(load().pinmpc_last_launch_count(h))
 
 
+def pinmpc_set_profiling(h, on):
+    _check(load().pinmpc_set_profiling(h, int(bool(on))), h)
+
+
+def pinmpc_get_kernel_ms(h):
+    ms = (c_float * 3)()
+    _check(load().pinmpc_get_kernel_ms(h, ms), h)
+    return [float(v) for v in ms]
+
+
 def pinmpc_probe_fma(blocks, iters, d_out, stream=0) -> float:
     return float(load().pinmpc_probe_fma(int(blocks), int(iters), _ptr(d_out), c_void_p(stream)))
 
@@ -251,6 +265,13 @@ class Solver:
 
     def set_tuning(self, envs_per_cta):
         pinmpc_set_tuning(self.h, envs_per_cta)
+
+    def set_profiling(self, on=True):
+        pinmpc_set_profiling(self.h, on)
+
+    def kernel_ms(self):
+        """[assembly, factorisation, iteration] milliseconds of the last profiled solve (synchronises)."""
+        return pinmpc_get_kernel_ms(self.h)
 
     def _stream(self, stream):
         if stream is None:

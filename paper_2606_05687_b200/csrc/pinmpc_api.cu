@@ -287,6 +287,42 @@ extern "C" pinmpc_status pinmpc_get_dynamics(pinmpc_t h, float *A, float *Bm, fl
 
 extern "C" int pinmpc_last_launch_count(pinmpc_t h) { return h ? h->launch_count : 0; }
 
+extern "C" pinmpc_status pinmpc_set_profiling(pinmpc_t h, int on)
+{
+    if (!h) return PINMPC_EINVAL;
+    if (on && !h->ev[0]) {
+        for (int i = 0; i < 4; i++) {
+            cudaError_t e = cudaEventCreate(&h->ev[i]);
+            if (e != cudaSuccess) {
+                snprintf(h->err, sizeof h->err, "cudaEventCreate: %s", cudaGetErrorString(e));
+                return PINMPC_ECUDA;
+            }
+        }
+    }
+    h->profiling = on ? 1 : 0;
+    h->prof_valid = false;
+    return PINMPC_OK;
+}
+
+extern "C" pinmpc_status pinmpc_get_kernel_ms(pinmpc_t h, float *h_ms)
+{
+    if (!h || !h_ms) return PINMPC_EINVAL;
+    if (!h->profiling || !h->prof_valid) return set_err(h, PINMPC_ESTATE, "pinmpc_get_kernel_ms: no profiled structured solve");
+    cudaError_t e = cudaEventSynchronize(h->ev[3]);
+    for (int i = 0; i < 3 && e == cudaSuccess; i++) e = cudaEventElapsedTime(&h_ms[i], h->ev[i], h->ev[i + 1]);
+    if (e != cudaSuccess) {
+        snprintf(h->err, sizeof h->err, "pinmpc_get_kernel_ms: %s", cudaGetErrorString(e));
+        return PINMPC_ECUDA;
+    }
+    return PINMPC_OK;
+}
+
 extern "C" const char *pinmpc_last_error(pinmpc_t h) { return h ? h->err : g_create_err; }
 
-extern "C" void pinmpc_destroy(pinmpc_t h) { delete h; }
+extern "C" void pinmpc_destroy(pinmpc_t h)
+{
+    if (!h) return;
+    for (int i = 0; i < 4; i++)
+        if (h->ev[i]) cudaEventDestroy(h->ev[i]);
+    delete h;
+}

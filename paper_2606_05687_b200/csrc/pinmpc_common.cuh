@@ -82,6 +82,9 @@ struct pinmpc_ctx {
     int envs_per_cta;        // tuning knob of the structured solver (0 = auto)
     int sm_count, smem_optin;
     int launch_count;
+    int profiling;           // record events around the kernels of the structured solver
+    bool prof_valid;
+    cudaEvent_t ev[4];
     cudaError_t sticky;
     char err[256];
 };

@@ -1057,12 +1057,16 @@ int launch_t(pinmpc_ctx *h, cudaStream_t st)
     ProblemPtrs q = make_problem_ptrs(h);
     const int ext = q.ext != nullptr;
     const long stages = (long)h->B * h->N;
+    const bool prof = h->profiling != 0;
+    if (prof) cudaEventRecord(h->ev[0], st);
     k_assemble_srb<NU><<<(unsigned)((stages + 127) / 128), 128, 0, st>>>(P, q, h->srb);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(h, "k_assemble_srb launch", e);
+    if (prof) cudaEventRecord(h->ev[1], st);
     k_factor_srb<<<(unsigned)((h->B + FAC_WARPS - 1) / FAC_WARPS), FAC_WARPS * 32, 0, st>>>(P, q.x0, h->srb, ext);
     e = cudaGetLastError();
     if (e != cudaSuccess) return fail(h, "k_factor_srb launch", e);
+    if (prof) cudaEventRecord(h->ev[2], st);
 
     cudaFuncAttributes fa;
     e = cudaFuncGetAttributes(&fa, k_iterate_srb<NU>);
@@ -1083,6 +1087,7 @@ int launch_t(pinmpc_ctx *h, cudaStream_t st)
     k_iterate_srb<NU><<<(unsigned)((h->B + G - 1) / G), threads, smem, st>>>(P, h->srb, q.x0, q.mass, h->out, G, PW, ext);
     e = cudaGetLastError();
     if (e != cudaSuccess) return fail(h, "k_iterate_srb launch", e);
+    if (prof) { cudaEventRecord(h->ev[3], st); h->prof_valid = true; }
     return 3;
 }
 

@@ -203,3 +203,46 @@ def test_error_codes_on_device():
     s.solve(); s.get()
     torch.cuda.synchronize()
     s.close()
+
+
+@pytest.mark.parametrize("B,N,nu", [(37, 13, 12), (21, 50, 12), (19, 9, 18)])
+def test_results_do_not_depend_on_envs_per_cta(B, N, nu):
+    """pinmpc_set_tuning: every CTA shape (1..16 envs, ragged last CTA, odd N => ragged second stage
+    of the stage threads) gives the oracle's answer."""
+    import torch
+    from paper_2606_05687_b200 import METHOD_SRB, Solver, make_layout
+    w = gen.make_config(3 if nu == 18 else 2, B=B, N=N, iters=25)
+    ref = oracle.solve(w)
+    lay = make_layout(w.n_wrench, w.n_force, w.mu, w.fz_max, w.mx_coef, w.my_coef, w.mz_coef, w.hand_fmax)
+    for G in (1, 2, 5, 6, 7, 11, 16):
+        s = Solver(w.nu, w.N, w.B, layout=lay, rho=w.rho, iters=w.iters, Qdiag=w.Qdiag, Rdiag=w.Rdiag, dt=w.dt, method=METHOD_SRB)
+        s.set_workload(w)
+        s.set_tuning(G)
+        s.solve()
+        out = s.get(aux=True)
+        torch.cuda.synchronize()
+        check_parity(w, {k: v.cpu().numpy() for k, v in out.items()}, ref)
+        s.close()
+
+
+def test_kernel_timing_hook():
+    """pinmpc_set_profiling / pinmpc_get_kernel_ms: three positive durations that add up to about the solve."""
+    import torch
+    from paper_2606_05687_b200 import PinmpcError, Solver, binding
+    w = gen.make_config(1, B=256, N=20)
+    s = Solver(w.nu, w.N, w.B, dt=w.dt, iters=w.iters, Qdiag=w.Qdiag, Rdiag=w.Rdiag)
+    s.set_workload(w)
+    s.solve()
+    with pytest.raises(PinmpcError) as e:
+        s.kernel_ms()
+    assert e.value.status == binding.ESTATE
+    s.set_profiling(True)
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    stream = torch.cuda.current_stream()
+    a.record(stream); s.solve(); b.record(stream)
+    ms = s.kernel_ms()
+    torch.cuda.synchronize()
+    assert len(ms) == 3 and all(m > 0 for m in ms)
+    assert sum(ms) <= a.elapsed_time(b) * 1.05 + 0.05
+    assert ms[2] > ms[0]
+    s.close()
