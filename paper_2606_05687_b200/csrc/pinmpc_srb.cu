@@ -485,7 +485,10 @@ struct ArenaLay { int oX, oC, stride; };
 
 constexpr int ITER_MAX_THREADS = 512;  // 16 warps x 128 registers: four warps per SM sub-partition
 constexpr int PASS_ENVS = 5;           // envs per pass warp (6 lanes each)
-constexpr int ARENA_PAD_MOD = 12;      // arena stride mod 32 (bank spread of the 6-lane groups)
+#ifndef PINMPC_ARENA_PAD_MOD
+#define PINMPC_ARENA_PAD_MOD 12
+#endif
+constexpr int ARENA_PAD_MOD = PINMPC_ARENA_PAD_MOD;      // arena stride mod 32 (bank spread of the 6-lane groups)
 constexpr int G_MAX = 16;              // envs per CTA
 constexpr int CTL_INTS = 32 + 5 * G_MAX;   // done[16] | ndone | pad[15] | red[16][5]
 
@@ -878,14 +881,17 @@ __global__ void __launch_bounds__(ITER_MAX_THREADS) k_iterate_srb(SolveParams P,
         pi = lane - 6 * eloc;
         const int e = warp * PASS_ENVS + eloc;
         pl.act = pass_warp && eloc < PASS_ENVS && e < Gv;
-        pe = pl.act ? e : (pass_warp ? warp * PASS_ENVS : 0);      // idle lanes shadow the warp's first env
+        // idle lanes shadow the warp's LAST env (the same addresses as its lanes, in the same half-warp: broadcast,
+        // no extra shared-memory wavefront)
+        const int elast = min(Gv, (warp + 1) * PASS_ENVS) - 1;
+        pe = pl.act ? e : (pass_warp ? elast : 0);
         const unsigned ar = (unsigned)__cvta_generic_to_shared(smem + pe * L.stride);
         pl.aK_b = ar + 8 * pi; pl.aK_f = ar + 48 * pi;
         pl.aXr = ar + 4 * L.oX; pl.aXo = pl.aXr + 4 * xslot(pi); pl.aXq = pl.aXr + (pi < 2 ? 0 : 16);
         pl.q = pi < 2 ? pi : pi - 2;
         pl.aC = ar + 4 * (L.oC + pi);
         {
-            const int base = pl.act ? 6 * eloc : 0;
+            const int base = pl.act ? 6 * eloc : 6 * (pass_warp ? elast - warp * PASS_ENVS : 0);
 #pragma unroll
             for (int r = 0; r < 6; r++) pl.src[r] = base + r;
         }
