@@ -52,6 +52,7 @@ def parse():
     ap.add_argument("--B", type=int, default=None)
     ap.add_argument("--N", type=int, default=None)
     ap.add_argument("--envs-per-cta", type=int, default=0, help="tuning knob of the structured solver (0 = auto)")
+    ap.add_argument("--sweep", action="store_true", help="BASELINE.json config 4: B x N table (one JSON line per point)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -144,10 +145,52 @@ def run_reference(args):
         "gpu_launches": 0}))
 
 
+def run_sweep(args):
+    """BASELINE.json config 4: B in {1024, 4096, 16384, 65536} x N in {10, 25, 50, 100}, 100 iterations, fp32:
+    solves/s, achieved FP32 and HBM rates and the device-memory footprint of every point."""
+    import numpy as np
+    import torch
+    import gen
+    from paper_2606_05687_b200 import METHOD_SRB, Solver, make_layout
+    dev = torch.device("cuda", 0)
+    stream = torch.cuda.current_stream(dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    for B in (1024, 4096, 16384, 65536):
+        for N in (10, 25, 50, 100):
+            w = gen.make_config(4, B=B, N=N)
+            lay = make_layout(w.n_wrench, w.n_force, w.mu, w.fz_max, w.mx_coef, w.my_coef, w.mz_coef, w.hand_fmax)
+            s = Solver(w.nu, w.N, w.B, layout=lay, rho=w.rho, iters=w.iters, Qdiag=w.Qdiag, Rdiag=w.Rdiag, dt=w.dt,
+                       method=METHOD_SRB, device=dev)
+            s.set_workload(w)
+            for _ in range(3):
+                s.solve()
+            torch.cuda.synchronize(dev)
+            ts = []
+            for _ in range(max(args.steps // 4, 3)):
+                flush.zero_()
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(stream); s.solve(); b.record(stream)
+                torch.cuda.synchronize(dev)
+                ts.append(a.elapsed_time(b))
+            ms = float(np.median(ts))
+            inputs = sum(getattr(w, n).nbytes for n in gen.Workload.ARRAYS if getattr(w, n) is not None)
+            io_bytes = inputs + w.B * w.N * (13 + 3 * w.nu) * 4 + w.B * 12
+            print(json.dumps({"sweep": w.name, "B": B, "N": N, "iters": w.iters, "ms_per_solve": ms,
+                              "solves_per_s": B / (ms * 1e-3), "stage_iters_per_s": B * N * w.iters / (ms * 1e-3),
+                              "tflops": flops_per_solve(w, "srb") / (ms * 1e-3) / 1e12,
+                              "hbm_gbs_algorithmic": io_bytes / (ms * 1e-3) / 1e9,
+                              "footprint_mb": (s.workspace_bytes + inputs) / 2 ** 20}), flush=True)
+            s.close()
+            del s, w
+            torch.cuda.empty_cache()
+
+
 def main():
     args = parse()
     if args.impl == "reference":
         return run_reference(args)
+    if args.sweep:
+        return run_sweep(args)
 
     import numpy as np
     import torch
