@@ -756,7 +756,7 @@ __device__ __forceinline__ void stage_kappa(const SrbWs &W, long st, long ts, fl
 // the next iteration.  res = running maxima (r_prim, |dz|, |u|, |z|, |y|) of this thread's env.
 template <int NU>
 __device__ __forceinline__ void stage_update(const SolveParams &P, const SrbWs &W, long st, long ts, StageState<NU> &S, float idt, float m_dt,
-                                             float *myX, bool update, bool emit, bool next, float *ou, float *res)
+                                             float *myX, bool update, bool emit, bool next, float *ou, float *res, bool two_feet)
 {
     constexpr int NC = NW + (NU - 12) / 3;
     StageGeom<NU> g;
@@ -779,6 +779,43 @@ __device__ __forceinline__ void stage_update(const SolveParams &P, const SrbWs &
         for (int a = 0; a < 6; a++) dl[a] -= G0[a];
         lam_inv_apply<NU>(P, g.TI, g.r, dl, lam);
         float Gn[6] = { 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f };
+        // The feet: u of both, then ONE exact projection when no thread of the warp has both feet in stance
+        // (a swing foot projects to 0): the wrench of the stance foot is selected, projected and scattered.
+        float uf[NW][6], zf[NW][6];
+#pragma unroll
+        for (int i = 0; i < NW; i++) {
+            const float rx = g.r[3 * i], ry = g.r[3 * i + 1], rz = g.r[3 * i + 2];
+            const float gl[6] = { lam[1] * rz - lam[2] * ry + lam[3], lam[2] * rx - lam[0] * rz + lam[4],
+                                  lam[0] * ry - lam[1] * rx + lam[5], lam[0], lam[1], lam[2] };
+#pragma unroll
+            for (int a = 0; a < 6; a++) {
+                const int c = a < 3 ? fcol(i) + a : mcol(i) + a - 3;
+                uf[i][a] = fmaf(P.tR[c], gl[a], fmaf(P.rtR[c], S.z[c] - S.y[c], g.ru[c]));
+            }
+        }
+        {
+            const bool on0 = bits & 1, on1 = (bits >> 1) & 1;
+            float v0[6], v1[6];
+#pragma unroll
+            for (int a = 0; a < 6; a++) {
+                v0[a] = uf[0][a] + S.y[a < 3 ? fcol(0) + a : mcol(0) + a - 3];
+                v1[a] = uf[1][a] + S.y[a < 3 ? fcol(1) + a : mcol(1) + a - 3];
+            }
+            if (two_feet) {                                 // warp-uniform
+                project_wrench(P, v0[0], v0[1], v0[2], v0[3], v0[4], v0[5], zf[0][0], zf[0][1], zf[0][2], zf[0][3], zf[0][4], zf[0][5]);
+                project_wrench(P, v1[0], v1[1], v1[2], v1[3], v1[4], v1[5], zf[1][0], zf[1][1], zf[1][2], zf[1][3], zf[1][4], zf[1][5]);
+#pragma unroll
+                for (int a = 0; a < 6; a++) { zf[0][a] = on0 ? zf[0][a] : 0.0f; zf[1][a] = on1 ? zf[1][a] : 0.0f; }
+            } else {
+                const bool sel = on1;                       // at most one foot is on
+                float vs[6], zs[6];
+#pragma unroll
+                for (int a = 0; a < 6; a++) vs[a] = sel ? v1[a] : v0[a];
+                project_wrench(P, vs[0], vs[1], vs[2], vs[3], vs[4], vs[5], zs[0], zs[1], zs[2], zs[3], zs[4], zs[5]);
+#pragma unroll
+                for (int a = 0; a < 6; a++) { zf[0][a] = on0 ? zs[a] : 0.0f; zf[1][a] = on1 ? zs[a] : 0.0f; }
+            }
+        }
 #pragma unroll
         for (int i = 0; i < NC; i++) {
             const bool on = (bits >> i) & 1;
@@ -795,24 +832,19 @@ __device__ __forceinline__ void stage_update(const SolveParams &P, const SrbWs &
 #pragma unroll
             for (int a = 0; a < NV; a++)
                 if (a < nv) ru[a] = g.ru[col[a]];
-            // u = u0 + Rt^-1 Gh^T lam :  f_i += lam_tau x r_i + lam_F ;  m_i += lam_tau
-            const float gl[NV] = { lam[1] * rz - lam[2] * ry + lam[3], lam[2] * rx - lam[0] * rz + lam[4],
-                                   lam[0] * ry - lam[1] * rx + lam[5], lam[0], lam[1], lam[2] };
+            if (i < NW) {
 #pragma unroll
-            for (int a = 0; a < NV; a++)
-                if (a < nv) {
+                for (int a = 0; a < 6; a++) { uu[a] = uf[i < NW ? i : 0][a]; zn[a] = zf[i < NW ? i : 0][a]; }
+            } else {
+                // u = u0 + Rt^-1 Gh^T lam :  f_i += lam_tau x r_i + lam_F
+                const float gl[3] = { lam[1] * rz - lam[2] * ry + lam[3], lam[2] * rx - lam[0] * rz + lam[4],
+                                      lam[0] * ry - lam[1] * rx + lam[5] };
+#pragma unroll
+                for (int a = 0; a < 3; a++) {
                     const float u0 = fmaf(P.rtR[col[a]], S.z[col[a]] - S.y[col[a]], ru[a]);
                     uu[a] = fmaf(P.tR[col[a]], gl[a], u0);
+                    zn[a] = on ? fminf(fmaxf(uu[a] + S.y[col[a]], -P.hand_fmax), P.hand_fmax) : 0.0f;
                 }
-            if (i < NW) {
-                float a0, a1, a2, a3, a4, a5;
-                project_wrench(P, uu[0] + S.y[col[0]], uu[1] + S.y[col[1]], uu[2] + S.y[col[2]], uu[3] + S.y[col[3]],
-                               uu[4] + S.y[col[4]], uu[5] + S.y[col[5]], a0, a1, a2, a3, a4, a5);
-                zn[0] = on ? a0 : 0.0f; zn[1] = on ? a1 : 0.0f; zn[2] = on ? a2 : 0.0f;
-                zn[3] = on ? a3 : 0.0f; zn[4] = on ? a4 : 0.0f; zn[5] = on ? a5 : 0.0f;
-            } else {
-#pragma unroll
-                for (int a = 0; a < 3; a++) zn[a] = on ? fminf(fmaxf(uu[a] + S.y[col[a]], -P.hand_fmax), P.hand_fmax) : 0.0f;
             }
 #pragma unroll
             for (int a = 0; a < NV; a++)
@@ -947,6 +979,9 @@ __global__ void __launch_bounds__(ITER_MAX_THREADS) k_iterate_srb(SolveParams P,
     StageState<NU> S0, S1;
     if (tact) stage_init<NU>(P, W, st, ts0, S0, idt, m_dt, myX0);
     if (act1) stage_init<NU>(P, W, st, ts1, S1, idt, m_dt, myX1);
+    // does any thread of this warp own a stage with both feet in stance?  (then two projections per stage)
+    const bool two_feet0 = __any_sync(FULL, tact && (__ldg(W.bits + ts0) & 3) == 3);
+    const bool two_feet1 = __any_sync(FULL, act1 && (__ldg(W.bits + ts1) & 3) == 3);
     bool frozen = false;          // this thread's env has met the tolerances (tolerance mode only)
 
     for (int it = 0; it < P.iters; it++) {
@@ -963,9 +998,9 @@ __global__ void __launch_bounds__(ITER_MAX_THREADS) k_iterate_srb(SolveParams P,
         __syncthreads();                                   // X = w
         {
             float res[5] = { 0.0f, 0.0f, 0.0f, 0.0f, 0.0f };
-            if (tact) stage_update<NU>(P, W, st, ts0, S0, idt, m_dt, myX0, !frozen, emit, next, o.u + ts0 * NU, res);
+            if (tact) stage_update<NU>(P, W, st, ts0, S0, idt, m_dt, myX0, !frozen, emit, next, o.u + ts0 * NU, res, two_feet0);
             asm volatile("" ::: "memory");              // one stage after the other (register pressure)
-            if (act1) stage_update<NU>(P, W, st, ts1, S1, idt, m_dt, myX1, !frozen, emit, next, o.u + ts1 * NU, res);
+            if (act1) stage_update<NU>(P, W, st, ts1, S1, idt, m_dt, myX1, !frozen, emit, next, o.u + ts1 * NU, res, two_feet1);
             if (emit && tact && !frozen) {
                 // non-negative floats order like their bit patterns
                 atomicMax(&red[te * 5 + 0], __float_as_uint(res[0])); atomicMax(&red[te * 5 + 1], __float_as_uint(res[1]));
