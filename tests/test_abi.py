@@ -46,6 +46,8 @@ def test_host_only_entry_points_without_a_gpu(lib):
     assert binding.pinmpc_workspace_bytes(12, 12, 50, 64, lay) == 0          # nx must be 13
     assert binding.pinmpc_workspace_bytes(13, 14, 50, 64, lay) == 0          # nu must match the layout
     assert binding.pinmpc_workspace_bytes(13, 12, 257, 64, lay) == 0         # N_MAX
+    assert binding.pinmpc_workspace_bytes(13, 12, 10, 0, lay) == 0           # empty batch
+    assert binding.pinmpc_workspace_bytes(13, 12, 0, 4, lay) == 0            # empty horizon
     assert binding.pinmpc_workspace_bytes(13, 18, 30, 64, binding.make_layout(2, 2)) > 0
     # create must refuse bad arguments before touching the device
     h = ctypes.c_void_p()

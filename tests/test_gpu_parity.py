@@ -246,3 +246,11 @@ def test_kernel_timing_hook():
     assert sum(ms) <= a.elapsed_time(b) * 1.05 + 0.05
     assert ms[2] > ms[0]
     s.close()
+
+
+def test_maximum_horizon_and_single_env():
+    """N = PINMPC_N_MAX (256) with B = 1 and B = 3: one env per CTA, arena of 82 KB per env."""
+    for B in (1, 3):
+        w = gen.make_config(1, B=B, N=256, iters=20)
+        got = run_gpu(w, "srb")
+        check_parity(w, got, oracle.solve(w))
