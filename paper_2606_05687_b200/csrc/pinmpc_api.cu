@@ -17,13 +17,12 @@ size_t pinmpc_ws_base_bytes(int nu, int N, int B)
 }
 
 // structured-solver factors (SrbWs)
-static const int SRB_NARR = 12;
+static const int SRB_NARR = 7;
 static void srb_sizes(int nu, int N, int B, size_t *f)
 {
     size_t st = (size_t)B * N;
-    int nc = 2 + (nu - 12) / 3;
-    f[0] = st * 72; f[1] = (size_t)B * (N + 1) * 12; f[2] = st * 6; f[3] = st * 6; f[4] = st * 2; f[5] = st * 21;
-    f[6] = st * 6; f[7] = st * 21; f[8] = st * 6; f[9] = st * 3 * nc; f[10] = st * nu; f[11] = st;
+    f[0] = st * 72; f[1] = (size_t)B * (N + 1) * 12; f[2] = st * 6; f[3] = st * 2; f[4] = st * 21;
+    f[5] = st * PINMPC_RA_W; f[6] = st * (size_t)pinmpc_rb_width(nu);
 }
 
 size_t pinmpc_ws_srb_bytes(int nu, int N, int B)
@@ -127,9 +126,8 @@ extern "C" pinmpc_status pinmpc_create(pinmpc_t *out, int nx, int nu, int N, int
         size_t f[SRB_NARR];
         srb_sizes(nu, N, B, f);
         h->srb.Kh = (float *)take(f[0] * 4); h->srb.qv = (float *)take(f[1] * 4); h->srb.c6 = (float *)take(f[2] * 4);
-        h->srb.HQ = (float *)take(f[3] * 4); h->srb.cs = (float *)take(f[4] * 4); h->srb.MI = (float *)take(f[5] * 4);
-        h->srb.KG = (float *)take(f[6] * 4); h->srb.LI = (float *)take(f[7] * 4); h->srb.IW = (float *)take(f[8] * 4);
-        h->srb.RR = (float *)take(f[9] * 4); h->srb.RU = (float *)take(f[10] * 4); h->srb.bits = (int *)take(f[11] * 4);
+        h->srb.cs = (float *)take(f[3] * 4); h->srb.MI = (float *)take(f[4] * 4);
+        h->srb.RA = (float *)take(f[5] * 4); h->srb.RB = (float *)take(f[6] * 4);
     }
     if (workspace_bytes >= pinmpc_ws_dense_bytes(nu, N, B)) {
         h->dA = (float *)take(st * NX * NX * 4);

@@ -49,17 +49,18 @@ struct SrbWs {
     float *Kh;     // [st][6][6][2]  gain of the 6-D-input LQR, pairs (Kh[r][j], Kh[r][6+j]), j = 0..5
     float *qv;     // [B][N+1][12]   q_k = Q xbar_k (k = 1..N), q_0 = 0
     float *c6;     // [st][6]        ch = (dt I_w^-1 tau_ext ; dt/m F_ext)   (zeros without ext_wrench)
-    float *HQ;     // [6][st]        (reserved)
     float *cs;     // [st][2]        cos, sin of the linearisation yaw
-    float *MI;     // [21][st]       S_k after assembly, Mh_k^-1 after factorisation (packed symmetric)
-    float *KG;     // [6][st]        kg_k = Kh[:,12] x_12 - Mh^-1 hq_k: gravity state's share of w and the
-                   //                iteration-invariant part of the backward pass (response to q, s)
-    float *LI;     // [21][st]       Lam_k^-1 (packed symmetric)
-    float *IW;     // [6][st]        I_w (packed symmetric 3x3)
-    float *RR;     // [3*nc][st]     contact offsets
-    float *RU;     // [nu][st]       R ubar
-    int *bits;     // [st]           contact flags
+    float *MI;     // [21][st]       S_k = D^-1 Lam^-1 D^-1 (packed symmetric): assembly -> factorisation
+    // Stage constants streamed by the stage threads of the iteration kernel every iteration: float4
+    // component-major, so that thread = stage reads them with coalesced LDG.128 (word w of stage s is
+    // at [(w / 4) * st + s] * 4 + w % 4).
+    float *RA;     // [7][st][4]     Mh_k^-1 packed symmetric (21) | kg_k = Kh[:,12] x_12 - Mh^-1 hq_k (6) | pad
+    float *RB;     // [RBW/4][st][4] T^-1 (6) | I_w (6) | r (3 nc) | Rt^-1 R ubar (nu) | contact bits | pad
 };
+#define PINMPC_RA_W 28
+__host__ __device__ constexpr int pinmpc_rb_width(int nu) { return (12 + 3 * (2 + (nu - 12) / 3) + nu + 1 + 3) & ~3; }
+__host__ __device__ inline long pinmpc_rec_index(int w, long st, long s) { return ((long)(w >> 2) * st + s) * 4 + (w & 3); }
+
 
 struct pinmpc_ctx {
     int nx, nu, N, B;

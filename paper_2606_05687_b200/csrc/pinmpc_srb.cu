@@ -182,7 +182,11 @@ __global__ void __launch_bounds__(128) k_assemble_srb(SolveParams P, ProblemPtrs
     world_inertia_inv(Ib, cs, sn, Iwf);
     const float iw[6] = { Iwf[0], Iwf[1], Iwf[2], Iwf[4], Iwf[5], Iwf[8] };
 #pragma unroll
-    for (int i = 0; i < 6; i++) W.IW[i * st + s] = iw[i];
+    float rb[pinmpc_rb_width(NU)];
+#pragma unroll
+    for (int i = 0; i < pinmpc_rb_width(NU); i++) rb[i] = 0.0f;
+#pragma unroll
+    for (int i = 0; i < 6; i++) rb[6 + i] = iw[i];
 
     int bits = 0;
     float r[3 * NC];
@@ -192,12 +196,12 @@ __global__ void __launch_bounds__(128) k_assemble_srb(SolveParams P, ProblemPtrs
 #pragma unroll
         for (int a = 0; a < 3; a++) {
             r[3 * i + a] = q.foot_r[(s * NC + i) * 3 + a];
-            W.RR[(3 * i + a) * st + s] = r[3 * i + a];
+            rb[12 + 3 * i + a] = r[3 * i + a];
         }
     }
-    W.bits[s] = bits;
+    rb[12 + 3 * NC + NU] = __int_as_float(bits);
 #pragma unroll
-    for (int j = 0; j < NU; j++) W.RU[j * st + s] = q.u_ref ? P.tR[j] * P.Rd[j] * q.u_ref[s * NU + j] : 0.0f;
+    for (int j = 0; j < NU; j++) rb[12 + 3 * NC + j] = q.u_ref ? P.tR[j] * P.Rd[j] * q.u_ref[s * NU + j] : 0.0f;
     // q_{k+1} = Q xbar_{k+1}  (x_ref[b,k] holds xbar_{k+1});  q_0 = 0
     {
         float *qv = W.qv + ((long)b * (N + 1) + k + 1) * 12;
@@ -248,7 +252,7 @@ __global__ void __launch_bounds__(128) k_assemble_srb(SolveParams P, ProblemPtrs
         TI[3] = (T[0] * T[5] - T[2] * T[2]) * id; TI[4] = (T[1] * T[2] - T[0] * T[4]) * id;
         TI[5] = (T[0] * T[3] - T[1] * T[1]) * id;
 #pragma unroll
-        for (int i = 0; i < 6; i++) W.LI[i * st + s] = TI[i];
+        for (int i = 0; i < 6; i++) rb[i] = TI[i];
     }
     spd_inv6(Lam);                                   // Lam^-1 (for S below)
     // S = D^-1 Lam^-1 D^-1,  D^-1 = blkdiag(I_w / dt, m/dt I)
@@ -288,6 +292,13 @@ __global__ void __launch_bounds__(128) k_assemble_srb(SolveParams P, ProblemPtrs
             for (int y = x; y < 3; y++) S[sidx(3 + x, 3 + y)] = Lam[sidx(3 + x, 3 + y)] * m_dt * m_dt;
 #pragma unroll
         for (int i = 0; i < 21; i++) W.MI[i * st + s] = S[i];
+    }
+    // the stage record of the iteration kernel: float4 component-major
+    {
+        float4 *RB4 = reinterpret_cast<float4 *>(W.RB);
+#pragma unroll
+        for (int c = 0; c < pinmpc_rb_width(NU) / 4; c++)
+            RB4[(long)c * st + s] = make_float4(rb[4 * c], rb[4 * c + 1], rb[4 * c + 2], rb[4 * c + 3]);
     }
     // ch = (dt I_w^-1 tau_ext ; dt/m F_ext): the part of c_k in rows 6..11
     if (q.ext != nullptr) {
@@ -407,7 +418,7 @@ __global__ void __launch_bounds__(FAC_WARPS * 32, 8) k_factor_srb(SolveParams P,
             else M = fmaf(-a * id, c, M);
         }
         M = -M;
-        if (lane < 21) { sM[lane] = M; W.MI[(long)lane * st + s] = M; }
+        if (lane < 21) { sM[lane] = M; W.RA[pinmpc_rec_index(lane, st, s)] = M; }
         __syncwarp();
         // Kh = Mh^-1 X[6:12,:]
 #pragma unroll
@@ -439,7 +450,7 @@ __global__ void __launch_bounds__(FAC_WARPS * 32, 8) k_factor_srb(SolveParams P,
                 mh = fmaf(sM[sidx(il, r)], hr, mh);
             }
             // constant part of kappa_k = Mh^-1 hh_k - Kh[:,12] x_12 :  kg_k = Kh[:,12] x_12 - Mh^-1 hq_k
-            if (lane < 6) W.KG[(long)lane * st + s] = fmaf(sK[lane * NX + 12], x12, -mh);
+            if (lane < 6) W.RA[pinmpc_rec_index(21 + lane, st, s)] = fmaf(sK[lane * NX + 12], x12, -mh);
             float atg = g;
             if (lane == 6) atg = fmaf(dt, cs * g_lo - sn * g_nb, g);
             else if (lane == 7) atg = fmaf(dt, cs * g_lo + sn * g_nb, g);
@@ -700,14 +711,21 @@ template <int NU> struct StageGeom {
 
 template <int NU> __device__ __forceinline__ void load_geom(const SrbWs &W, long st, long ts, StageGeom<NU> &g)
 {
-    constexpr int NC = NW + (NU - 12) / 3;
+    constexpr int NC = NW + (NU - 12) / 3, RBW = pinmpc_rb_width(NU);
+    const float4 *rec = reinterpret_cast<const float4 *>(W.RB) + ts;
+    float v[RBW];
 #pragma unroll
-    for (int c = 0; c < 6; c++) { g.TI[c] = __ldg(W.LI + c * st + ts); g.Iw[c] = __ldg(W.IW + c * st + ts); }
+    for (int c = 0; c < RBW / 4; c++) {
+        const float4 q = __ldg(rec + (long)c * st);
+        v[4 * c] = q.x; v[4 * c + 1] = q.y; v[4 * c + 2] = q.z; v[4 * c + 3] = q.w;
+    }
 #pragma unroll
-    for (int c = 0; c < 3 * NC; c++) g.r[c] = __ldg(W.RR + c * st + ts);
+    for (int c = 0; c < 6; c++) { g.TI[c] = v[c]; g.Iw[c] = v[6 + c]; }
 #pragma unroll
-    for (int c = 0; c < NU; c++) g.ru[c] = __ldg(W.RU + c * st + ts);
-    g.bits = __ldg(W.bits + ts);
+    for (int c = 0; c < 3 * NC; c++) g.r[c] = v[12 + c];
+#pragma unroll
+    for (int c = 0; c < NU; c++) g.ru[c] = v[12 + 3 * NC + c];
+    g.bits = __float_as_int(v[12 + 3 * NC + NU]);
 }
 
 // X_k = sigma0 = D^-1 Lam^-1 G0
@@ -738,11 +756,13 @@ __device__ __forceinline__ void stage_init(const SolveParams &P, const SrbWs &W,
 // kappa = Mh^-1 hh - kg  (X: hh -> kappa)
 __device__ __forceinline__ void stage_kappa(const SrbWs &W, long st, long ts, float *myX)
 {
-    float Mi[27];
+    float Mi[28];
+    const float4 *rec = reinterpret_cast<const float4 *>(W.RA) + ts;
 #pragma unroll
-    for (int c = 0; c < 21; c++) Mi[c] = __ldg(W.MI + c * st + ts);
-#pragma unroll
-    for (int c = 0; c < 6; c++) Mi[21 + c] = __ldg(W.KG + c * st + ts);
+    for (int c = 0; c < 7; c++) {
+        const float4 q = __ldg(rec + (long)c * st);
+        Mi[4 * c] = q.x; Mi[4 * c + 1] = q.y; Mi[4 * c + 2] = q.z; Mi[4 * c + 3] = q.w;
+    }
     const float2 h0 = *reinterpret_cast<const float2 *>(myX);
     const float4 h1 = *reinterpret_cast<const float4 *>(myX + 4);
     const float h[6] = { h0.x, h0.y, h1.x, h1.y, h1.z, h1.w };
@@ -980,8 +1000,8 @@ __global__ void __launch_bounds__(ITER_MAX_THREADS) k_iterate_srb(SolveParams P,
     if (tact) stage_init<NU>(P, W, st, ts0, S0, idt, m_dt, myX0);
     if (act1) stage_init<NU>(P, W, st, ts1, S1, idt, m_dt, myX1);
     // does any thread of this warp own a stage with both feet in stance?  (then two projections per stage)
-    const bool two_feet0 = __any_sync(FULL, tact && (__ldg(W.bits + ts0) & 3) == 3);
-    const bool two_feet1 = __any_sync(FULL, act1 && (__ldg(W.bits + ts1) & 3) == 3);
+    const bool two_feet0 = __any_sync(FULL, tact && (__float_as_int(__ldg(W.RB + pinmpc_rec_index(12 + 3 * NC + NU, st, ts0))) & 3) == 3);
+    const bool two_feet1 = __any_sync(FULL, act1 && (__float_as_int(__ldg(W.RB + pinmpc_rec_index(12 + 3 * NC + NU, st, ts1))) & 3) == 3);
     bool frozen = false;          // this thread's env has met the tolerances (tolerance mode only)
 
     for (int it = 0; it < P.iters; it++) {

@@ -38,8 +38,8 @@ def test_host_only_entry_points_without_a_gpu(lib):
     base = binding.pinmpc_workspace_bytes(13, 12, 50, 4096, lay)
     dense = binding.pinmpc_workspace_bytes(13, 12, 50, 4096, lay, binding.METHOD_DENSE)
     st = 4096 * 50
-    # outputs x,u,z,y (13 + 36 floats per stage) + the structured solver's factors (192 per stage + q_0)
-    per_stage = (13 + 36) + (72 + 12 + 6 + 6 + 2 + 21 + 6 + 21 + 6 + 6 + 12 + 1)
+    # outputs x,u,z,y (13 + 36 floats per stage) + the structured solver's factors (175 per stage + q_0)
+    per_stage = (13 + 36) + (72 + 12 + 6 + 2 + 21 + 28 + 32)
     lo = (st * per_stage + 4096 * 12) * 4
     assert base >= lo and base < lo + 20 * 256 + 3 * 4096 * 4
     assert dense > base + st * (169 + 156 + 156 + 144) * 4
