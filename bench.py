@@ -38,7 +38,7 @@ FLOP_DENSE_ONCE = {12: 33000.0, 18: 60000.0}
 FMA_LANES_PER_SM = 128
 # DRAM bytes (read + write) of one k_iterate_srb launch at config 2 from the `ncu --set full` capture
 # summarised in profiles/r1_final_iterate_ncu.md (dram__bytes_read.sum + dram__bytes_write.sum)
-NCU_DRAM_BYTES_ITERATE = {"c2_long_horizon": 108795648 + 15324928}
+NCU_DRAM_BYTES_ITERATE = {"c2_long_horizon": 110317568 + 13498368}
 
 
 def parse():
