@@ -43,7 +43,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     subprocess.check_call([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", tmp] + objs + ["-lcudart"])
     os.replace(tmp, LIB)
     with open(os.path.join(CSRC, "ptxas_v.log"), "w") as f:
-        f.write("\n".join(log))
+        # without ptxas' wall-clock lines, so that the committed log changes only when the code does
+        f.write("\n".join(l for l in "\n".join(log).splitlines() if "Compile time" not in l) + "\n")
     if verbose:
         print("\n".join(log))
     return LIB
