@@ -100,6 +100,22 @@ class ClockSampler:
                 "samples": len(sm)}
 
 
+def max_over_ranks(values, dist, device):
+    """Replicas only: the one collective of a multi-GPU run is this MAX of the per-rank
+    step times; `value` is then (envs of all ranks) / (the slowest rank's time)."""
+    import torch
+    if dist is None:
+        return [float(v) for v in values]
+    t = torch.tensor([float(v) for v in values], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t]
+
+
+def aggregate_value(envs_per_rank, world, ms):
+    """Whole-job throughput of `world` replicas of `envs_per_rank` envs that all finished within `ms`."""
+    return envs_per_rank * world / (ms * 1e-3)
+
+
 def flops_per_solve(w, method):
     st = w.B * w.N
     if method == "dense":
@@ -298,13 +314,12 @@ def main():
 
     # ---- max over ranks ---------------------------------------------------------------------------
     if dist is not None:
-        t = torch.tensor([ms, e2e[0] if e2e else 0.0], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t[0]); e2e = (float(t[1]), e2e[1], e2e[2]) if e2e else None
+        ms, e2e_ms = max_over_ranks([ms, e2e[0] if e2e else 0.0], dist, dev)
+        e2e = (e2e_ms, e2e[1], e2e[2]) if e2e else None
 
     if rank == 0:
         total_solves = w.B * world
-        value = total_solves / (ms * 1e-3)
+        value = aggregate_value(w.B, world, ms)
         fl = flops_per_solve(w, mname)
         if kernel_ms:
             # dominant kernel = the iteration kernel: its own algorithmic FLOPs over its own duration (CUDA events
