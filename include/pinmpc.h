@@ -98,6 +98,13 @@ pinmpc_status pinmpc_set_weights(pinmpc_t h, const float *h_Qdiag /*[nx]*/, cons
  *   r_prim <= eps_abs + eps_rel max(|u|_inf,|z|_inf)  and  r_dual <= eps_abs + eps_rel rho |y|_inf. */
 pinmpc_status pinmpc_set_tolerance(pinmpc_t h, float eps_abs, float eps_rel, int check_every);
 
+/* Warm start of the ADMM iteration (the paper re-solves the MPC at 5-50 Hz inside RL
+ * training, so consecutive solves differ by one shifted stage).  d_z0, d_y0: DEVICE arrays
+ * [B,N,nu] holding the start values z^0 (constraint copy) and y^0 (scaled dual), e.g. the z, y of the previous
+ * solve from pinmpc_get_aux shifted by the caller; borrowed until the next call.  Both NULL (default) = cold
+ * start z^0 = y^0 = 0.  The arrays must not alias the library workspace.  One of them NULL: PINMPC_EINVAL. */
+pinmpc_status pinmpc_set_warm_start(pinmpc_t h, const float *d_z0, const float *d_y0);
+
 /* Force a solver variant (default PINMPC_METHOD_AUTO). */
 pinmpc_status pinmpc_set_method(pinmpc_t h, pinmpc_method m);
 

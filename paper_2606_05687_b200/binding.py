@@ -24,7 +24,8 @@ _STATUS = {0: "PINMPC_OK", 1: "PINMPC_EINVAL", 2: "PINMPC_EALLOC", 3: "PINMPC_EC
 EXPORTS = ("pinmpc_workspace_bytes", "pinmpc_workspace_bytes_method", "pinmpc_create", "pinmpc_set_weights",
            "pinmpc_set_tolerance", "pinmpc_set_method", "pinmpc_set_tuning", "pinmpc_set_problem", "pinmpc_set_dynamics", "pinmpc_solve",
            "pinmpc_get", "pinmpc_get_aux", "pinmpc_get_dynamics", "pinmpc_last_launch_count", "pinmpc_last_error",
-           "pinmpc_destroy", "pinmpc_probe_fma", "pinmpc_set_profiling", "pinmpc_get_kernel_ms")
+           "pinmpc_destroy", "pinmpc_probe_fma", "pinmpc_set_profiling", "pinmpc_get_kernel_ms",
+           "pinmpc_set_warm_start")
 
 
 class PinmpcError(RuntimeError):
@@ -88,6 +89,8 @@ def load():
     lib.pinmpc_last_error.argtypes = [c_void_p]
     lib.pinmpc_probe_fma.restype = ctypes.c_double
     lib.pinmpc_probe_fma.argtypes = [c_int, c_int, c_void_p, c_void_p]
+    lib.pinmpc_set_warm_start.restype = c_int
+    lib.pinmpc_set_warm_start.argtypes = [c_void_p, c_void_p, c_void_p]
     lib.pinmpc_set_profiling.restype = c_int
     lib.pinmpc_set_profiling.argtypes = [c_void_p, c_int]
     lib.pinmpc_get_kernel_ms.restype = c_int
@@ -174,6 +177,10 @@ def pinmpc_get_dynamics(h, A=None, Bm=None, c=None, stream=0):
 
 def pinmpc_last_launch_count(h) -> int:
     return int(load().pinmpc_last_launch_count(h))
+
+
+def pinmpc_set_warm_start(h, z0=None, y0=None):
+    _check(load().pinmpc_set_warm_start(h, _ptr(z0), _ptr(y0)), h)
 
 
 def pinmpc_set_profiling(h, on):
@@ -265,6 +272,16 @@ class Solver:
 
     def set_tuning(self, envs_per_cta):
         pinmpc_set_tuning(self.h, envs_per_cta)
+
+    def set_warm_start(self, z0=None, y0=None):
+        """Start the next solves from z0, y0 [B,N,nu] (None, None: cold start)."""
+        f = self.torch.float32
+        z0, y0 = self._dev(z0, f), self._dev(y0, f)
+        for v in (z0, y0):
+            if v is not None and tuple(v.shape) != (self.B, self.N, self.nu):
+                raise ValueError(f"warm start: shape {tuple(v.shape)} != {(self.B, self.N, self.nu)}")
+        self._keep.update(warm_z=z0, warm_y=y0)
+        pinmpc_set_warm_start(self.h, z0, y0)
 
     def set_profiling(self, on=True):
         pinmpc_set_profiling(self.h, on)

@@ -163,6 +163,14 @@ extern "C" pinmpc_status pinmpc_set_tolerance(pinmpc_t h, float eps_abs, float e
     return PINMPC_OK;
 }
 
+extern "C" pinmpc_status pinmpc_set_warm_start(pinmpc_t h, const float *d_z0, const float *d_y0)
+{
+    if (!h) return PINMPC_EINVAL;
+    if ((d_z0 == nullptr) != (d_y0 == nullptr)) return set_err(h, PINMPC_EINVAL, "pinmpc_set_warm_start: give both z0 and y0, or neither");
+    h->warm_z = d_z0; h->warm_y = d_y0;
+    return PINMPC_OK;
+}
+
 extern "C" pinmpc_status pinmpc_set_method(pinmpc_t h, pinmpc_method m)
 {
     if (!h) return PINMPC_EINVAL;

@@ -29,6 +29,7 @@ struct ProblemPtrs {
     const float *x0, *x_ref, *u_ref;
     const uint8_t *contact;
     const float *foot_r, *yaw, *mass, *inertia, *ext;
+    const float *z0, *y0;      // warm start [B,N,nu] (both NULL: cold start)
 };
 
 struct OutPtrs {
@@ -74,6 +75,7 @@ struct pinmpc_ctx {
     bool have_problem, have_dynamics, solved;
     pinmpc_problem prob;
     const float *userA, *userB, *userC;
+    const float *warm_z, *warm_y;
     char *ws;
     size_t ws_bytes;
     // carved from the workspace
@@ -129,6 +131,7 @@ static inline ProblemPtrs make_problem_ptrs(const pinmpc_ctx *h)
     q.x0 = h->prob.x0; q.x_ref = h->prob.x_ref; q.u_ref = h->prob.u_ref; q.contact = h->prob.contact;
     q.foot_r = h->prob.foot_r; q.yaw = h->prob.yaw; q.mass = h->prob.mass; q.inertia = h->prob.inertia;
     q.ext = h->prob.ext_wrench;
+    q.z0 = h->warm_z; q.y0 = h->warm_y;
     return q;
 }
 

@@ -248,7 +248,10 @@ __global__ void __launch_bounds__(128) k_iterate_dense(SolveParams P, ProblemPtr
     const float *ur = q.u_ref ? q.u_ref + (long)b * N * NU : nullptr;
 
     for (int k = 0; k < N; k++)
-        if (lane < NU) { zb[k * NU + lane] = 0.0f; yb[k * NU + lane] = 0.0f; }
+        if (lane < NU) {
+            zb[k * NU + lane] = q.z0 ? q.z0[((long)b * N + k) * NU + lane] : 0.0f;
+            yb[k * NU + lane] = q.y0 ? q.y0[((long)b * N + k) * NU + lane] : 0.0f;
+        }
     __syncwarp();
 
     float rp = 0.0f, rd = 0.0f;

@@ -739,15 +739,18 @@ __device__ __forceinline__ void write_sigma0(const SolveParams &P, const StageGe
     *reinterpret_cast<float4 *>(myX + 4) = make_float4(s0[2], s0[3], s0[4], s0[5]);
 }
 
-// start of a solve: z = y = 0, u0 = ubar', sigma0 -> X
+// start of a solve: z, y = the start values, u0 from them, sigma0 -> X
 template <int NU>
 __device__ __forceinline__ void stage_init(const SolveParams &P, const SrbWs &W, long st, long ts, StageState<NU> &S, float idt, float m_dt,
-                                           float *myX)
+                                           float *myX, const float *z0, const float *y0)
 {
     StageGeom<NU> g;
     load_geom<NU>(W, st, ts, g);
 #pragma unroll
-    for (int j = 0; j < NU; j++) { S.z[j] = 0.0f; S.y[j] = 0.0f; }
+    for (int j = 0; j < NU; j++) {
+        S.z[j] = z0 ? __ldg(z0 + ts * NU + j) : 0.0f;       // warm start (pinmpc_set_warm_start) or cold start
+        S.y[j] = y0 ? __ldg(y0 + ts * NU + j) : 0.0f;
+    }
     float u0[NU], G0[6];
     stage_u0<NU>(P, g.ru, S.z, S.y, g.r, u0, G0);
     write_sigma0<NU>(P, g, G0, idt, m_dt, myX);
@@ -890,9 +893,9 @@ __device__ __forceinline__ void stage_update(const SolveParams &P, const SrbWs &
     if (next) write_sigma0<NU>(P, g, G0, idt, m_dt, myX);   // frozen envs keep a well-defined (constant) sigma0
 }
 
-template <int NU>
+template <int NU, bool WARM>
 __global__ void __launch_bounds__(ITER_MAX_THREADS) k_iterate_srb(SolveParams P, SrbWs W, const float *__restrict__ x0g,
-                                                                  const float *__restrict__ massg, OutPtrs o, int G, int PW, int has_ext)
+                                                                  const float *__restrict__ massg, OutPtrs o, int G, int PW, int has_ext, const float *__restrict__ z0g, const float *__restrict__ y0g)
 {
     constexpr int NC = NW + (NU - 12) / 3;
     extern __shared__ __align__(16) float smem[];
@@ -997,8 +1000,8 @@ __global__ void __launch_bounds__(ITER_MAX_THREADS) k_iterate_srb(SolveParams P,
     const float m_dt = massg[bb] / dt;
 
     StageState<NU> S0, S1;
-    if (tact) stage_init<NU>(P, W, st, ts0, S0, idt, m_dt, myX0);
-    if (act1) stage_init<NU>(P, W, st, ts1, S1, idt, m_dt, myX1);
+    if (tact) stage_init<NU>(P, W, st, ts0, S0, idt, m_dt, myX0, WARM ? z0g : nullptr, WARM ? y0g : nullptr);
+    if (act1) stage_init<NU>(P, W, st, ts1, S1, idt, m_dt, myX1, WARM ? z0g : nullptr, WARM ? y0g : nullptr);
     // does any thread of this warp own a stage with both feet in stance?  (then two projections per stage)
     const bool two_feet0 = __any_sync(FULL, tact && (__float_as_int(__ldg(W.RB + pinmpc_rec_index(12 + 3 * NC + NU, st, ts0))) & 3) == 3);
     const bool two_feet1 = __any_sync(FULL, act1 && (__float_as_int(__ldg(W.RB + pinmpc_rec_index(12 + 3 * NC + NU, st, ts1))) & 3) == 3);
@@ -1129,8 +1132,10 @@ int launch_t(pinmpc_ctx *h, cudaStream_t st)
     if (e != cudaSuccess) return fail(h, "k_factor_srb launch", e);
     if (prof) cudaEventRecord(h->ev[2], st);
 
+    // the cold-start kernel carries no warm-start code (same registers and schedule as without the feature)
+    auto kern = q.z0 ? k_iterate_srb<NU, true> : k_iterate_srb<NU, false>;
     cudaFuncAttributes fa;
-    e = cudaFuncGetAttributes(&fa, k_iterate_srb<NU>);
+    e = cudaFuncGetAttributes(&fa, kern);
     if (e != cudaSuccess) return fail(h, "k_iterate_srb attributes", e);
     int G = h->envs_per_cta;
     if (G > 0 && (iterate_threads(h->N, G) > ITER_MAX_THREADS || iterate_smem_bytes(h->N, G, ext, h->nu) > (size_t)h->smem_optin)) G = 0;
@@ -1142,10 +1147,10 @@ int launch_t(pinmpc_ctx *h, cudaStream_t st)
     }
     const int threads = iterate_threads(h->N, G), PW = (G + PASS_ENVS - 1) / PASS_ENVS;
     const size_t smem = iterate_smem_bytes(h->N, G, ext, h->nu);
-    e = cudaFuncSetAttribute(k_iterate_srb<NU>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_iterate_srb<NU>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+    e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
     if (e != cudaSuccess) return fail(h, "k_iterate_srb smem attribute", e);
-    k_iterate_srb<NU><<<(unsigned)((h->B + G - 1) / G), threads, smem, st>>>(P, h->srb, q.x0, q.mass, h->out, G, PW, ext);
+    kern<<<(unsigned)((h->B + G - 1) / G), threads, smem, st>>>(P, h->srb, q.x0, q.mass, h->out, G, PW, ext, q.z0, q.y0);
     e = cudaGetLastError();
     if (e != cudaSuccess) return fail(h, "k_iterate_srb launch", e);
     if (prof) { cudaEventRecord(h->ev[3], st); h->prof_valid = true; }

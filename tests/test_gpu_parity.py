@@ -254,3 +254,52 @@ def test_maximum_horizon_and_single_env():
         w = gen.make_config(1, B=B, N=256, iters=20)
         got = run_gpu(w, "srb")
         check_parity(w, got, oracle.solve(w))
+
+
+@pytest.mark.parametrize("method", METHODS)
+def test_warm_start(method):
+    """pinmpc_set_warm_start.  (a) The ADMM state is (z, y): 30 cold iterations, then 20
+    from their z, y = 50 cold iterations of the oracle.  (b) Receding horizon: a new problem started from the
+    previous z, y shifted by one stage vs the oracle started from the same values."""
+    import torch
+    from paper_2606_05687_b200 import Solver, make_layout
+    w = gen.make_config(1, B=48, N=21, iters=50)
+    lay = make_layout(w.n_wrench, w.n_force, w.mu, w.fz_max, w.mx_coef, w.my_coef, w.mz_coef, w.hand_fmax)
+
+    def solve(work, iters, z0=None, y0=None):
+        s = Solver(work.nu, work.N, work.B, layout=lay, rho=work.rho, iters=iters, Qdiag=work.Qdiag, Rdiag=work.Rdiag,
+                   dt=work.dt, method=_method(method), dense_workspace=(method == "dense"))
+        s.set_workload(work)
+        s.set_warm_start(z0, y0)
+        s.solve()
+        out = s.get(aux=True)
+        torch.cuda.synchronize()
+        res = {k: v.cpu().numpy() for k, v in out.items()}
+        s.close()
+        return res
+
+    first = solve(w, 30)
+    second = solve(w, 20, first["z"], first["y"])
+    ref = oracle.solve(w, iters=50)
+    second["iters_done"] = second["iters_done"] + 30
+    check_parity(w, second, ref)
+    # (b) the next MPC problem (another seed of the same generator), started from the shifted previous solution
+    w2 = gen.make_config(2, B=48, N=21, iters=15)
+    z0 = np.concatenate([first["z"][:, 1:], first["z"][:, -1:]], axis=1)
+    y0 = np.concatenate([first["y"][:, 1:], first["y"][:, -1:]], axis=1)
+    got = solve(w2, 15, np.ascontiguousarray(z0), np.ascontiguousarray(y0))
+    check_parity(w2, got, oracle.solve(w2, iters=15, z0=z0, y0=y0))
+    # and back to a cold start on the same handle semantics: None, None
+    cold = solve(w2, 15, None, None)
+    check_parity(w2, cold, oracle.solve(w2, iters=15))
+
+
+def test_warm_start_argument_check():
+    import torch
+    from paper_2606_05687_b200 import PinmpcError, Solver, binding
+    w = gen.make_config(0, B=4, N=5)
+    s = Solver(w.nu, w.N, w.B, dt=w.dt)
+    with pytest.raises(PinmpcError) as e:
+        binding.pinmpc_set_warm_start(s.h, torch.zeros(4, 5, 12, device="cuda"), None)
+    assert e.value.status == binding.EINVAL
+    s.close()
