@@ -315,22 +315,13 @@ __global__ void __launch_bounds__(128) k_assemble_srb(SolveParams P, ProblemPtrs
 }
 
 // ---------------------------------------------------------------------------------------------
-// S2  factorisation: one warp per env, sequential over stages, P (13x13) in shared memory
+// S2  factorisation: one warp per env, sequential over stages.  Lane i < 13 owns row i of the 13x13
+// matrices P and X = P A (rows padded to 16 floats in shared memory, float4 accesses, no index
+// arithmetic in the loop); lanes 0..20 own one packed element of the symmetric 6x6 Mh each.
 // ---------------------------------------------------------------------------------------------
-constexpr int FAC_WARPS = 4;                     // warps (envs) per CTA
-constexpr int FAC_SMEM = 172 + 172 + 80 + 24;    // floats per warp: P, X, Kh, Mh^-1
-
-// element (i,j) of A^T X for the structured A (rows 6..12 of A^T pick up dt * rows of X)
-__device__ __forceinline__ float atx(const float *X, int i, int j, float dt, float cs, float sn)
-{
-    float a = X[i * NX + j];
-    if (i == 6) a += dt * (cs * X[0 * NX + j] - sn * X[1 * NX + j]);
-    else if (i == 7) a += dt * (sn * X[0 * NX + j] + cs * X[1 * NX + j]);
-    else if (i == 8) a += dt * X[2 * NX + j];
-    else if (i >= 9 && i <= 11) a += dt * X[(i - 6) * NX + j];
-    else if (i == 12) a += dt * X[11 * NX + j];
-    return a;
-}
+constexpr int FAC_WARPS = 4;                        // warps (envs) per CTA
+constexpr int FAC_LD = 16;                          // padded row length
+constexpr int FAC_SMEM = 13 * 16 + 13 * 16 + 6 * 16 + 24;   // floats per warp: P, X, Kh, Mh^-1
 
 __global__ void __launch_bounds__(FAC_WARPS * 32, 8) k_factor_srb(SolveParams P, const float *__restrict__ x0, SrbWs W, int has_ext)
 {
@@ -338,33 +329,38 @@ __global__ void __launch_bounds__(FAC_WARPS * 32, 8) k_factor_srb(SolveParams P,
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     const int b = blockIdx.x * FAC_WARPS + wib;
     if (b >= P.B) return;
-    float *sP = sm_all + wib * FAC_SMEM, *sX = sP + 172, *sK = sX + 172, *sM = sK + 80;
+    float *sP = sm_all + wib * FAC_SMEM, *sX = sP + 13 * FAC_LD, *sK = sX + 13 * FAC_LD, *sM = sK + 6 * FAC_LD;
     const int N = P.N;
     const long st = (long)P.B * N;
     const float dt = P.dt;
     const float x12 = x0[(long)b * NX + 12];
+    const int row = lane < NX ? lane : 0;             // lanes >= 13 shadow row 0 (no stores)
+    const bool rown = lane < NX;
 
     // lane <-> (i,j) of the packed symmetric 6x6 (lanes >= 21 shadow element (0,0))
     int mi = 0, mj = 0;
     {
-        int l = lane < 21 ? lane : 0, row = 0;
-        while (l >= 6 - row) { l -= 6 - row; row++; }
-        mi = row; mj = row + l;
+        int l = lane < 21 ? lane : 0, r = 0;
+        while (l >= 6 - r) { l -= 6 - r; r++; }
+        mi = r; mj = r + l;
     }
     int la[6], lb[6];
 #pragma unroll
     for (int p = 0; p < 6; p++) { la[p] = sidx(mi, p); lb[p] = sidx(p, mj); }
-    // upper triangle of the 13x13: element t = lane + 32 r  ->  (ti, tj), ti <= tj
-    int ti[3], tj[3];
-#pragma unroll
-    for (int r = 0; r < 3; r++) {
-        int t = lane + 32 * r, row = 0;
-        if (t > 90) t = 90;
-        while (t >= NX - row) { t -= NX - row; row++; }
-        ti[r] = row; tj[r] = row + t;
-    }
+    // A^T X: row i of A^T X = X[i] + ea X[ra] + eb X[rb]  (rows 6..12 pick up dt * rows of X)
+    const int ra = row == 6 || row == 7 ? 0 : (row == 8 ? 2 : (row >= 9 && row <= 11 ? row - 6 : (row == 12 ? 11 : 0)));
+    const int rb = row == 6 || row == 7 ? 1 : ra;
+    const float qd = rown ? P.Qd[row] : 0.0f;
 
-    for (int i = lane; i < 169; i += 32) sP[i] = ((i * 79) >> 10) * 14 == i ? P.Qd[(i * 79) >> 10] : 0.0f;
+    // P_N = Q
+    if (rown) {
+#pragma unroll
+        for (int c = 0; c < 4; c++) {
+            float4 v = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+            if (row == 4 * c) v.x = qd; else if (row == 4 * c + 1) v.y = qd; else if (row == 4 * c + 2) v.z = qd; else if (row == 4 * c + 3) v.w = qd;
+            *reinterpret_cast<float4 *>(sP + row * FAC_LD + 4 * c) = v;
+        }
+    }
     __syncwarp();
     const int jl = lane < 12 ? lane : 0;
     float pc = W.qv[((long)b * (N + 1) + N) * 12 + jl];     // pc_N = q_N
@@ -382,29 +378,30 @@ __global__ void __launch_bounds__(FAC_WARPS * 32, 8) k_factor_srb(SolveParams P,
             S_n = W.MI[(long)(lane < 21 ? lane : 0) * st + s - 1];
             ch_n = (has_ext && lane < 6) ? W.c6[(s - 1) * 6 + lane] : 0.0f;
         }
-        // X = P A
-#pragma unroll
-        for (int r = 0; r < 6; r++) {
-            int e = lane + 32 * r;
-            if (e < 169) {
-                int i = (e * 79) >> 10, j = e - i * NX;
-                const float *Pi = sP + i * NX;
-                float a = Pi[j];
-                if (j == 6) a += dt * (cs * Pi[0] - sn * Pi[1]);
-                else if (j == 7) a += dt * (sn * Pi[0] + cs * Pi[1]);
-                else if (j == 8) a += dt * Pi[2];
-                else if (j >= 9 && j <= 11) a += dt * Pi[j - 6];
-                else if (j == 12) a += dt * Pi[11];
-                sX[e] = a;
+        // ---- X = P A, row `row`:  columns 6..12 pick up dt * (R_z^T | I | e_11) combinations of columns 0..5, 11
+        float xr[16];
+        {
+            const float4 *Pr = reinterpret_cast<const float4 *>(sP + row * FAC_LD);
+            const float4 p0 = Pr[0], p1 = Pr[1], p2 = Pr[2], p3 = Pr[3];
+            xr[0] = p0.x; xr[1] = p0.y; xr[2] = p0.z; xr[3] = p0.w; xr[4] = p1.x; xr[5] = p1.y;
+            xr[6] = fmaf(dt, cs * p0.x - sn * p0.y, p1.z);
+            xr[7] = fmaf(dt, sn * p0.x + cs * p0.y, p1.w);
+            xr[8] = fmaf(dt, p0.z, p2.x);
+            xr[9] = fmaf(dt, p0.w, p2.y); xr[10] = fmaf(dt, p1.x, p2.z); xr[11] = fmaf(dt, p1.y, p2.w);
+            xr[12] = fmaf(dt, p2.w, p3.x);
+            xr[13] = xr[14] = xr[15] = 0.0f;
+            if (rown) {
+                float4 *Xr = reinterpret_cast<float4 *>(sX + row * FAC_LD);
+                Xr[0] = make_float4(xr[0], xr[1], xr[2], xr[3]); Xr[1] = make_float4(xr[4], xr[5], xr[6], xr[7]);
+                Xr[2] = make_float4(xr[8], xr[9], xr[10], xr[11]); Xr[3] = make_float4(xr[12], 0.0f, 0.0f, 0.0f);
             }
         }
-        // Mh = S + P[6:12,6:12] (one packed element per lane) ; s_k = P (E ch)
-        float M = Sl + sP[(6 + mi) * NX + 6 + mj];
+        // ---- Mh = S + P[6:12,6:12] (one packed element per lane) ;  s_k = P (E ch)
+        float M = Sl + sP[(6 + mi) * FAC_LD + 6 + mj];
         float sk = 0.0f;
         if (has_ext) {
-            const int rl = lane < NX ? lane : 0;
 #pragma unroll
-            for (int a = 0; a < 6; a++) sk = fmaf(sP[rl * NX + 6 + a], __shfl_sync(FULL, chl, a), sk);
+            for (int a = 0; a < 6; a++) sk = fmaf(sP[row * FAC_LD + 6 + a], __shfl_sync(FULL, chl, a), sk);
         }
         // Mh^-1 by symmetric sweeps (-Mh^-1 after six pivots), all in registers
 #pragma unroll
@@ -420,21 +417,30 @@ __global__ void __launch_bounds__(FAC_WARPS * 32, 8) k_factor_srb(SolveParams P,
         M = -M;
         if (lane < 21) { sM[lane] = M; W.RA[pinmpc_rec_index(lane, st, s)] = M; }
         __syncwarp();
-        // Kh = Mh^-1 X[6:12,:]
+        // ---- Kh = Mh^-1 X[6:12,:], column `row`;  xc = X[6..11][row] = G[:, row] is reused for the P update
+        float xc[6], kc[6];
 #pragma unroll
-        for (int r = 0; r < 3; r++) {
-            int e = lane + 32 * r;
-            if (e < 78) {
-                int i = (e * 79) >> 10, j = e - i * NX;
-                float a = 0.0f;
+        for (int l = 0; l < 6; l++) xc[l] = sX[(6 + l) * FAC_LD + row];
+        {
+            float Mi[24];
 #pragma unroll
-                for (int l = 0; l < 6; l++) a = fmaf(sM[sidx(i, l)], sX[(6 + l) * NX + j], a);
-                sK[e] = a;
-                if (j < 12) W.Kh[s * 72 + i * 12 + (j < 6 ? 2 * j : 2 * (j - 6) + 1)] = a;
+            for (int c = 0; c < 6; c++) {
+                const float4 v = *reinterpret_cast<const float4 *>(sM + 4 * c);
+                Mi[4 * c] = v.x; Mi[4 * c + 1] = v.y; Mi[4 * c + 2] = v.z; Mi[4 * c + 3] = v.w;
+            }
+            symv6(Mi, xc, kc);
+        }
+        if (rown) {
+#pragma unroll
+            for (int r = 0; r < 6; r++) sK[r * FAC_LD + row] = kc[r];
+            if (row < 12) {
+                const int pos = row < 6 ? 2 * row : 2 * (row - 6) + 1;
+#pragma unroll
+                for (int r = 0; r < 6; r++) W.Kh[s * 72 + r * 12 + pos] = kc[r];
             }
         }
         __syncwarp();
-        // iteration-invariant part of the backward vector pass (response to q and s, sigma0 = 0):
+        // ---- iteration-invariant part of the backward vector pass (response to q and s, sigma0 = 0):
         //   g = pc - s_k ; hq_k = E^T g ; pc <- q_k + A^T g - Kh^T hq_k        (lane j < 12 holds pc_j)
         // The iteration kernel runs the sigma0-driven part only; hq_k enters kappa_k through kg_k.
         {
@@ -446,28 +452,43 @@ __global__ void __launch_bounds__(FAC_WARPS * 32, 8) k_factor_srb(SolveParams P,
 #pragma unroll
             for (int r = 0; r < 6; r++) {
                 const float hr = __shfl_sync(FULL, g, 6 + r);
-                acc = fmaf(sK[r * NX + jl], hr, acc);
+                acc = fmaf(kc[r], hr, acc);                 // kc = Kh[:, lane] for lane < 13
                 mh = fmaf(sM[sidx(il, r)], hr, mh);
             }
             // constant part of kappa_k = Mh^-1 hh_k - Kh[:,12] x_12 :  kg_k = Kh[:,12] x_12 - Mh^-1 hq_k
-            if (lane < 6) W.RA[pinmpc_rec_index(21 + lane, st, s)] = fmaf(sK[lane * NX + 12], x12, -mh);
+            if (lane < 6) W.RA[pinmpc_rec_index(21 + lane, st, s)] = fmaf(sK[lane * FAC_LD + 12], x12, -mh);
             float atg = g;
             if (lane == 6) atg = fmaf(dt, cs * g_lo - sn * g_nb, g);
             else if (lane == 7) atg = fmaf(dt, cs * g_lo + sn * g_nb, g);
             else if (lane >= 8 && lane < 12) atg = fmaf(dt, g_lo, g);
             pc = (k >= 1 ? W.qv[((long)b * (N + 1) + k) * 12 + jl] : 0.0f) + atg - acc;
         }
-        // P <- [k>=1] Q + A^T X - G^T Kh   (upper triangle, mirrored: both terms are symmetric)
+        // ---- P <- [k>=1] Q + A^T X - G^T Kh, row `row`, four columns at a time
+        {
+            const float ea = row == 6 ? dt * cs : (row == 7 ? dt * sn : (row >= 8 ? dt : 0.0f));
+            const float eb = row == 6 ? -dt * sn : (row == 7 ? dt * cs : 0.0f);
+            const float qk = k >= 1 ? qd : 0.0f;
 #pragma unroll
-        for (int r = 0; r < 3; r++) {
-            if (lane + 32 * r < 91) {
-                int i = ti[r], j = tj[r];
-                float a = atx(sX, i, j, dt, cs, sn);
+            for (int c = 0; c < 4; c++) {
+                const float4 xa = *reinterpret_cast<const float4 *>(sX + ra * FAC_LD + 4 * c);
+                const float4 xb = *reinterpret_cast<const float4 *>(sX + rb * FAC_LD + 4 * c);
+                float4 o;
+                o.x = fmaf(ea, xa.x, fmaf(eb, xb.x, xr[4 * c])); o.y = fmaf(ea, xa.y, fmaf(eb, xb.y, xr[4 * c + 1]));
+                o.z = fmaf(ea, xa.z, fmaf(eb, xb.z, xr[4 * c + 2])); o.w = fmaf(ea, xa.w, fmaf(eb, xb.w, xr[4 * c + 3]));
 #pragma unroll
-                for (int l = 0; l < 6; l++) a = fmaf(-sX[(6 + l) * NX + i], sK[l * NX + j], a);
-                if (k >= 1 && i == j) a += P.Qd[i];
-                sP[i * NX + j] = a;
-                sP[j * NX + i] = a;
+                for (int l = 0; l < 6; l++) {
+                    const float4 kv = *reinterpret_cast<const float4 *>(sK + l * FAC_LD + 4 * c);
+                    o.x = fmaf(-xc[l], kv.x, o.x); o.y = fmaf(-xc[l], kv.y, o.y);
+                    o.z = fmaf(-xc[l], kv.z, o.z); o.w = fmaf(-xc[l], kv.w, o.w);
+                }
+                if (row == 4 * c) o.x += qk; else if (row == 4 * c + 1) o.y += qk; else if (row == 4 * c + 2) o.z += qk; else if (row == 4 * c + 3) o.w += qk;
+                // upper triangle (j >= row), mirrored: P stays exactly symmetric over long horizons
+                const float ov[4] = { o.x, o.y, o.z, o.w };
+#pragma unroll
+                for (int d = 0; d < 4; d++) {
+                    const int j = 4 * c + d;
+                    if (j < NX && rown && j >= row) { sP[row * FAC_LD + j] = ov[d]; sP[j * FAC_LD + row] = ov[d]; }
+                }
             }
         }
         __syncwarp();
