@@ -171,6 +171,38 @@ int pinmpc_last_launch_count(pinmpc_t h);
 pinmpc_status pinmpc_set_profiling(pinmpc_t h, int on);
 pinmpc_status pinmpc_get_kernel_ms(pinmpc_t h, float *h_ms);
 
+/* ---- Predictive landmarks and the prediction-confidence reward (eq. (10)-(14)) ----
+ * Stateless calls on a caller-owned DEVICE ring buffer; all run asynchronously on `stream`.
+ *   eq. (10)  n_l = 1 + floor(s_l (N-1))  (float64 product of the float32 s_l), l = 0..n_landmarks-1
+ *   eq. (11)  a solve at time t stores (t + n_l, c_hat = x_{n_l}[3:6]) for every landmark
+ *   eq. (12)  e_l(t) = c_t - c_hat^{t - n_l}(n_l), omitted when that landmark was never stored
+ *   eq. (13)  r_t = exp(-sum_l alpha_l sum_j Qc_j e_{l,j}^2 / sigma_c^2)
+ * Time is an integer count of MPC steps per env (int32, restarts with the episode).  The ring holds
+ * n_landmarks x (N+1) slots of (c_x, c_y, c_z, target time) per env, addressed by target time modulo N+1;
+ * a slot is valid only while its stored target time equals the time asked for. */
+#define PINMPC_MAX_LANDMARKS 8
+typedef struct {
+    int n_landmarks;                      /* N_L in 1..PINMPC_MAX_LANDMARKS                          */
+    float s[PINMPC_MAX_LANDMARKS];        /* s_l in [0,1]; the paper sets s_0 = 0, s_{NL-1} = 1        */
+    float alpha[PINMPC_MAX_LANDMARKS];    /* prediction-confidence weights, eq. (14)                  */
+    float Qc[3];                          /* diagonal of Q_c                                         */
+    float sigma_c;                        /* > 0                                                     */
+} pinmpc_landmark_cfg;
+
+/* Bytes of the ring buffer for B envs and horizon N (0 on invalid arguments). */
+size_t pinmpc_landmark_ring_bytes(int B, int N, const pinmpc_landmark_cfg *cfg);
+/* Start of an episode: forget the landmarks of the envs with mask[b] != 0 (DEVICE uint8 [B]; NULL = all). */
+pinmpc_status pinmpc_landmark_reset(void *d_ring, int B, int N, const pinmpc_landmark_cfg *cfg, const uint8_t *mask, void *stream);
+/* eq. (11): store the landmarks of a solve.  x DEVICE [B,N,13] = x_1..x_N, t DEVICE int32 [B] = solve time. */
+pinmpc_status pinmpc_landmark_push(void *d_ring, int B, int N, const pinmpc_landmark_cfg *cfg, const float *x, const int *t, void *stream);
+/* The same, reading x straight from the solver's workspace after pinmpc_solve on the same stream (no copy). */
+pinmpc_status pinmpc_landmark_push_solver(pinmpc_t h, void *d_ring, const pinmpc_landmark_cfg *cfg, const int *t, void *stream);
+/* eq. (12)-(13): c_real DEVICE [B,3] = realised CoM at time t[b]; r DEVICE [B]; n_used DEVICE int32 [B] or NULL
+ * = number of landmarks that existed.  Errors: PINMPC_EINVAL on NULL pointers, B,N < 0, n_landmarks out of
+ * range or sigma_c <= 0; B = 0 is a no-op. */
+pinmpc_status pinmpc_landmark_reward(const void *d_ring, int B, int N, const pinmpc_landmark_cfg *cfg, const float *c_real, const int *t,
+                                     float *r, int *n_used, void *stream);
+
 /* Human-readable description of the last error on this handle (owned by the handle; "" if none).
  * With h = NULL: the last pinmpc_create failure in this thread. */
 const char *pinmpc_last_error(pinmpc_t h);

@@ -4,5 +4,5 @@
 hand-written CUDA kernels for sm_100a (csrc/).  No CPU fallback.
 """
 from . import binding  # noqa: F401
-from .binding import (METHOD_AUTO, METHOD_DENSE, METHOD_SRB, NX, Layout, PinmpcError, Solver,  # noqa: F401
-                      make_layout)
+from .binding import (METHOD_AUTO, METHOD_DENSE, METHOD_SRB, NX, LandmarkCfg, Landmarks, Layout,  # noqa: F401
+                      PinmpcError, Solver, make_landmark_cfg, make_layout)

@@ -25,7 +25,9 @@ EXPORTS = ("pinmpc_workspace_bytes", "pinmpc_workspace_bytes_method", "pinmpc_cr
            "pinmpc_set_tolerance", "pinmpc_set_method", "pinmpc_set_tuning", "pinmpc_set_problem", "pinmpc_set_dynamics", "pinmpc_solve",
            "pinmpc_get", "pinmpc_get_aux", "pinmpc_get_dynamics", "pinmpc_last_launch_count", "pinmpc_last_error",
            "pinmpc_destroy", "pinmpc_probe_fma", "pinmpc_set_profiling", "pinmpc_get_kernel_ms",
-           "pinmpc_set_warm_start")
+           "pinmpc_set_warm_start", "pinmpc_landmark_ring_bytes", "pinmpc_landmark_reset", "pinmpc_landmark_push",
+           "pinmpc_landmark_push_solver", "pinmpc_landmark_reward")
+MAX_LANDMARKS = 8
 
 
 class PinmpcError(RuntimeError):
@@ -42,6 +44,11 @@ class Layout(ctypes.Structure):
 class Problem(ctypes.Structure):
     _fields_ = [(n, c_void_p) for n in ("x0", "x_ref", "u_ref", "contact", "foot_r", "yaw", "mass", "inertia",
                                         "ext_wrench")]
+
+
+class LandmarkCfg(ctypes.Structure):
+    _fields_ = [("n_landmarks", c_int), ("s", c_float * MAX_LANDMARKS), ("alpha", c_float * MAX_LANDMARKS),
+                ("Qc", c_float * 3), ("sigma_c", c_float)]
 
 
 _lib = None
@@ -95,6 +102,16 @@ def load():
     lib.pinmpc_set_profiling.argtypes = [c_void_p, c_int]
     lib.pinmpc_get_kernel_ms.restype = c_int
     lib.pinmpc_get_kernel_ms.argtypes = [c_void_p, POINTER(c_float)]
+    lib.pinmpc_landmark_ring_bytes.restype = c_size_t
+    lib.pinmpc_landmark_ring_bytes.argtypes = [c_int, c_int, POINTER(LandmarkCfg)]
+    lib.pinmpc_landmark_reset.restype = c_int
+    lib.pinmpc_landmark_reset.argtypes = [c_void_p, c_int, c_int, POINTER(LandmarkCfg), c_void_p, c_void_p]
+    lib.pinmpc_landmark_push.restype = c_int
+    lib.pinmpc_landmark_push.argtypes = [c_void_p, c_int, c_int, POINTER(LandmarkCfg), c_void_p, c_void_p, c_void_p]
+    lib.pinmpc_landmark_push_solver.restype = c_int
+    lib.pinmpc_landmark_push_solver.argtypes = [c_void_p, c_void_p, POINTER(LandmarkCfg), c_void_p, c_void_p]
+    lib.pinmpc_landmark_reward.restype = c_int
+    lib.pinmpc_landmark_reward.argtypes = [c_void_p, c_int, c_int, POINTER(LandmarkCfg)] + [c_void_p] * 5
     lib.pinmpc_destroy.restype = None
     lib.pinmpc_destroy.argtypes = [c_void_p]
     _lib = lib
@@ -336,3 +353,51 @@ class Solver:
             self.close()
         except Exception:
             pass
+
+
+# ---- predictive landmarks + prediction-confidence reward (include/pinmpc.h, eq. (10)-(14)) ----------
+def make_landmark_cfg(s, alpha, Qc=(1.0, 1.0, 1.0), sigma_c=0.05) -> LandmarkCfg:
+    if len(s) != len(alpha) or not 1 <= len(s) <= MAX_LANDMARKS:
+        raise PinmpcError(EINVAL, "1..8 landmarks, len(s) == len(alpha)")
+    c = LandmarkCfg()
+    c.n_landmarks = len(s)
+    for i, (a, b) in enumerate(zip(s, alpha)):
+        c.s[i], c.alpha[i] = float(a), float(b)
+    for j in range(3):
+        c.Qc[j] = float(Qc[j])
+    c.sigma_c = float(sigma_c)
+    return c
+
+
+class Landmarks:
+    """Owns the device ring buffer; every method is one C-ABI call (argument marshalling only)."""
+
+    def __init__(self, B, N, cfg: LandmarkCfg, device="cuda:0"):
+        import torch
+        self.torch, self.device = torch, torch.device(device)
+        self.B, self.N, self.cfg = int(B), int(N), cfg
+        nbytes = load().pinmpc_landmark_ring_bytes(self.B, self.N, ctypes.byref(cfg))
+        if nbytes == 0 and self.B > 0:
+            raise PinmpcError(EINVAL, "invalid landmark configuration")
+        self.ring = torch.empty(max(nbytes, 16), dtype=torch.uint8, device=self.device)
+        self.reset()
+
+    def _s(self, stream):
+        return c_void_p(self.torch.cuda.current_stream(self.device).cuda_stream if stream is None else stream.cuda_stream)
+
+    def reset(self, mask=None, stream=None):
+        _check(load().pinmpc_landmark_reset(_ptr(self.ring), self.B, self.N, ctypes.byref(self.cfg), _ptr(mask), self._s(stream)))
+
+    def push(self, x, t, stream=None):
+        _check(load().pinmpc_landmark_push(_ptr(self.ring), self.B, self.N, ctypes.byref(self.cfg), _ptr(x), _ptr(t), self._s(stream)))
+
+    def push_solver(self, solver, t, stream=None):
+        _check(load().pinmpc_landmark_push_solver(solver.h, _ptr(self.ring), ctypes.byref(self.cfg), _ptr(t), self._s(stream)), solver.h)
+
+    def reward(self, c_real, t, stream=None):
+        tt = self.torch
+        r = tt.empty(self.B, dtype=tt.float32, device=self.device)
+        used = tt.empty(self.B, dtype=tt.int32, device=self.device)
+        _check(load().pinmpc_landmark_reward(_ptr(self.ring), self.B, self.N, ctypes.byref(self.cfg), _ptr(c_real), _ptr(t),
+                                             _ptr(r), _ptr(used), self._s(stream)))
+        return r, used
