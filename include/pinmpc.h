@@ -149,6 +149,13 @@ pinmpc_status pinmpc_get(pinmpc_t h, float *x, float *u, float *r_prim, float *r
 /* The splitting variables after the last solve: z [B,N,nu] (feasible copy), y [B,N,nu] (scaled dual). */
 pinmpc_status pinmpc_get_aux(pinmpc_t h, float *z, float *y, void *stream);
 
+/* Receding-horizon shift for the next MPC update (the MPC is re-solved every few control
+ * steps): z0[b,k] = z[b,min(k+shift,N-1)] and y0 likewise from the z, y of the last solve (the last stage is
+ * repeated), written into caller DEVICE buffers z0, y0 [B,N,nu] that can be handed to pinmpc_set_warm_start.
+ * 0 <= shift <= N; asynchronous on `stream` (the solve's stream, or ordered after it).  PINMPC_ESTATE before
+ * the first solve and after a pinmpc_set_problem that no solve has followed (shift first, then set the next problem), PINMPC_EINVAL on NULL buffers or a shift out of range. */
+pinmpc_status pinmpc_shift_aux(pinmpc_t h, int shift, float *z0, float *y0, void *stream);
+
 /* Materialise the assembled dynamics of the current problem into caller DEVICE buffers
  * A [B,N,nx,nx], Bm [B,N,nx,nu], c [B,N,nx] (any may be NULL); runs the assembly kernel on `stream`. */
 pinmpc_status pinmpc_get_dynamics(pinmpc_t h, float *A, float *Bm, float *c, void *stream);

@@ -25,7 +25,7 @@ EXPORTS = ("pinmpc_workspace_bytes", "pinmpc_workspace_bytes_method", "pinmpc_cr
            "pinmpc_set_tolerance", "pinmpc_set_method", "pinmpc_set_tuning", "pinmpc_set_problem", "pinmpc_set_dynamics", "pinmpc_solve",
            "pinmpc_get", "pinmpc_get_aux", "pinmpc_get_dynamics", "pinmpc_last_launch_count", "pinmpc_last_error",
            "pinmpc_destroy", "pinmpc_probe_fma", "pinmpc_set_profiling", "pinmpc_get_kernel_ms",
-           "pinmpc_set_warm_start", "pinmpc_landmark_ring_bytes", "pinmpc_landmark_reset", "pinmpc_landmark_push",
+           "pinmpc_set_warm_start", "pinmpc_shift_aux", "pinmpc_landmark_ring_bytes", "pinmpc_landmark_reset", "pinmpc_landmark_push",
            "pinmpc_landmark_push_solver", "pinmpc_landmark_reward")
 MAX_LANDMARKS = 8
 
@@ -102,6 +102,8 @@ def load():
     lib.pinmpc_set_profiling.argtypes = [c_void_p, c_int]
     lib.pinmpc_get_kernel_ms.restype = c_int
     lib.pinmpc_get_kernel_ms.argtypes = [c_void_p, POINTER(c_float)]
+    lib.pinmpc_shift_aux.restype = c_int
+    lib.pinmpc_shift_aux.argtypes = [c_void_p, c_int, c_void_p, c_void_p, c_void_p]
     lib.pinmpc_landmark_ring_bytes.restype = c_size_t
     lib.pinmpc_landmark_ring_bytes.argtypes = [c_int, c_int, POINTER(LandmarkCfg)]
     lib.pinmpc_landmark_reset.restype = c_int
@@ -198,6 +200,10 @@ def pinmpc_last_launch_count(h) -> int:
 
 def pinmpc_set_warm_start(h, z0=None, y0=None):
     _check(load().pinmpc_set_warm_start(h, _ptr(z0), _ptr(y0)), h)
+
+
+def pinmpc_shift_aux(h, shift, z0, y0, stream=None):
+    _check(load().pinmpc_shift_aux(h, int(shift), _ptr(z0), _ptr(y0), stream), h)
 
 
 def pinmpc_set_profiling(h, on):
@@ -299,6 +305,17 @@ class Solver:
                 raise ValueError(f"warm start: shape {tuple(v.shape)} != {(self.B, self.N, self.nu)}")
         self._keep.update(warm_z=z0, warm_y=y0)
         pinmpc_set_warm_start(self.h, z0, y0)
+
+    def shift_warm_start(self, shift=1, stream=None):
+        """Receding-horizon update: shift z, y of the last solve by `shift` stages on the device and use them as
+        the start of the next solves.  Call it before handing over the next problem (set_problem forgets the solve)."""
+        t = self.torch
+        z0 = t.empty((self.B, self.N, self.nu), dtype=t.float32, device=self.device)
+        y0 = t.empty_like(z0)
+        pinmpc_shift_aux(self.h, shift, z0, y0, self._stream(stream))
+        self._keep.update(warm_z=z0, warm_y=y0)
+        pinmpc_set_warm_start(self.h, z0, y0)
+        return z0, y0
 
     def set_profiling(self, on=True):
         pinmpc_set_profiling(self.h, on)

@@ -281,6 +281,36 @@ extern "C" pinmpc_status pinmpc_get_aux(pinmpc_t h, float *z, float *y, void *st
     return PINMPC_OK;
 }
 
+// receding-horizon shift of the splitting variables: dst[b,k,:] = src[b,min(k+shift,N-1),:]
+__global__ void k_shift_stages(const float *__restrict__ src, float *__restrict__ dst, int B, int N, int nu, int shift)
+{
+    const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= (long)B * N * nu) return;
+    const int j = (int)(i % nu);
+    const long bk = i / nu;
+    const int k = (int)(bk % N);
+    const long b = bk / N;
+    const int ks = min(k + shift, N - 1);
+    dst[i] = src[(b * N + ks) * nu + j];
+}
+
+extern "C" pinmpc_status pinmpc_shift_aux(pinmpc_t h, int shift, float *z0, float *y0, void *stream)
+{
+    if (!h) return PINMPC_EINVAL;
+    if (h->sticky != cudaSuccess) return PINMPC_ECUDA;
+    if (!h->solved) return set_err(h, PINMPC_ESTATE, "pinmpc_shift_aux: no solve has been enqueued");
+    if (shift < 0 || shift > h->N || !z0 || !y0) return set_err(h, PINMPC_EINVAL, "pinmpc_shift_aux: 0 <= shift <= N, z0 and y0 non-NULL");
+    if (z0 == h->out.z || y0 == h->out.y) return set_err(h, PINMPC_EINVAL, "pinmpc_shift_aux: z0, y0 must not alias the workspace");
+    const long n = (long)h->B * h->N * h->nu;
+    if (n == 0) return PINMPC_OK;
+    const unsigned blocks = (unsigned)((n + 255) / 256);
+    k_shift_stages<<<blocks, 256, 0, (cudaStream_t)stream>>>(h->out.z, z0, h->B, h->N, h->nu, shift);
+    k_shift_stages<<<blocks, 256, 0, (cudaStream_t)stream>>>(h->out.y, y0, h->B, h->N, h->nu, shift);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) { h->sticky = e; return set_err(h, PINMPC_ECUDA, cudaGetErrorString(e)); }
+    return PINMPC_OK;
+}
+
 extern "C" pinmpc_status pinmpc_get_dynamics(pinmpc_t h, float *A, float *Bm, float *c, void *stream)
 {
     if (!h) return PINMPC_EINVAL;

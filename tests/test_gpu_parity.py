@@ -303,3 +303,58 @@ def test_warm_start_argument_check():
         binding.pinmpc_set_warm_start(s.h, torch.zeros(4, 5, 12, device="cuda"), None)
     assert e.value.status == binding.EINVAL
     s.close()
+
+
+def _stage_window(w, a, N, x0):
+    from dataclasses import replace
+    kw = {}
+    for f in ("x_ref", "u_ref", "contact", "foot_r", "yaw", "ext_wrench"):
+        v = getattr(w, f)
+        kw[f] = None if v is None else np.ascontiguousarray(v[:, a:a + N])
+    return replace(w, N=N, x0=np.ascontiguousarray(x0, dtype=np.float32), name=f"{w.name}_win{a}", **kw)
+
+
+def test_receding_horizon_shift():
+    """pinmpc_shift_aux: z0[b,k] = z[b,min(k+shift,N-1)] bit for bit (a copy), and what it is for: the next MPC
+    problem (window moved by one stage, x0 = the predicted x_1) started from the shifted z, y meets the same
+    tolerance in fewer iterations than from a cold start."""
+    import torch
+    from paper_2606_05687_b200 import PinmpcError, Solver, binding, make_layout
+    N = 20
+    long = gen.make_config(1, B=96, N=N + 1, iters=3000)
+    lay = make_layout(long.n_wrench, long.n_force, long.mu, long.fz_max, long.mx_coef, long.my_coef, long.mz_coef, long.hand_fmax)
+    w0 = _stage_window(long, 0, N, long.x0)
+    s = Solver(w0.nu, N, w0.B, layout=lay, rho=1e-2, iters=3000, Qdiag=w0.Qdiag, Rdiag=w0.Rdiag, dt=w0.dt)   # well-scaled rho
+    zbuf = torch.empty((w0.B, N, w0.nu), device="cuda"); ybuf = torch.empty_like(zbuf)
+    with pytest.raises(PinmpcError) as e:                     # nothing solved yet
+        binding.pinmpc_shift_aux(s.h, 1, zbuf, ybuf, None)
+    assert e.value.status == binding.ESTATE
+    s.set_tolerance(1e-2, 1e-3, 5)
+    s.set_workload(w0)
+    s.solve()
+    first = {k: v.cpu().numpy() for k, v in s.get(aux=True).items()}
+    for bad in (-1, N + 1):
+        with pytest.raises(PinmpcError) as e:
+            binding.pinmpc_shift_aux(s.h, bad, zbuf, ybuf, None)
+        assert e.value.status == binding.EINVAL
+    for shift in (0, 1, 3, N):
+        binding.pinmpc_shift_aux(s.h, shift, zbuf, ybuf, None)
+        idx = np.minimum(np.arange(N) + shift, N - 1)
+        assert np.array_equal(zbuf.cpu().numpy(), first["z"][:, idx])
+        assert np.array_equal(ybuf.cpu().numpy(), first["y"][:, idx])
+    # the next MPC update
+    w1 = _stage_window(long, 1, N, first["x"][:, 0])
+    s.shift_warm_start(1)                                     # before set_problem: it reads the last solve's z, y
+    s.set_workload(w1)
+    s.solve()
+    warm = {k: v.cpu().numpy() for k, v in s.get().items()}
+    s.set_warm_start(None, None)
+    s.solve()
+    cold = {k: v.cpu().numpy() for k, v in s.get().items()}
+    s.close()
+    assert cold["iters_done"].max() < 3000                    # both converged to the tolerance
+    assert warm["iters_done"].mean() < 0.8 * cold["iters_done"].mean(), (warm["iters_done"].mean(), cold["iters_done"].mean())
+    # (u itself is not compared: with R = 1e-5 the optimum is nearly flat in u, so two runs stopped at the same
+    # tolerance differ by far more than the tolerance)
+    for run in (warm, cold):
+        assert np.all(run["r_prim"] <= 1e-2 + 1e-3 * np.abs(run["u"]).max(axis=(1, 2)) * 1.01)
