@@ -210,6 +210,39 @@ pinmpc_status pinmpc_landmark_push_solver(pinmpc_t h, void *d_ring, const pinmpc
 pinmpc_status pinmpc_landmark_reward(const void *d_ring, int B, int N, const pinmpc_landmark_cfg *cfg, const float *c_real, const int *t,
                                      float *r, int *n_used, void *stream);
 
+/* ---- The paper's own stage-local ADMM (eq. (18)-(22)): second method -----------------------
+ * Velocity form with the lifted state xi_k = [x_k ; u_{k-1}] (n = 13 + nu), copies z_{k+1} = xi_{k+1} and
+ * v_k = Bb_k du_k, the dynamics relaxed with a third scaled dual; every update is local to a stage (no recursion
+ * over the horizon).  Same QP (16)-(17) as pinmpc_solve, generic dense LTV data.  Per iteration, for every k:
+ *   du_k = J_k (v_k - beta_k);  xi_{k+1} = H_k h_k;  gamma_k, gamma~_k;  z_{k+1} = Proj_{R^nx x U_k}((2 gamma~_k +
+ *   gamma_k)/3);  v_k = (z_{k+1} + gamma_k)/2;  theta_k, beta_k, lambda_k updates         (eq. (22))
+ * with J_k = (Bb_k^T Bb_k)^-1 Bb_k^T and H_k = (Qb + rho I + rho Ab_{k+1}^T Ab_{k+1})^-1 computed once on the
+ * device.  All iterates start at 0; `iters` iterations, no acceleration.  Stateless: everything lives in the
+ * caller's workspace.  All problem pointers are DEVICE pointers, float32, contiguous. */
+typedef struct {
+    const float *A;            /* [B,N,13,13]                                                        */
+    const float *Bm;           /* [B,N,13,nu]                                                        */
+    const float *c;            /* [B,N,13]   offset e_k; NULL => 0                                   */
+    const float *x0;           /* [B,13]                                                             */
+    const float *u_prev;       /* [B,nu]     u_{-1} of the velocity form; NULL => 0                  */
+    const float *x_ref;        /* [B,N,13]   xbar_1..xbar_N                                          */
+    const float *u_ref;        /* [B,N,nu]   ubar_0..ubar_{N-1}; NULL => 0                           */
+    const uint8_t *contact;    /* [B,N,nc]                                                           */
+} pinmpc_split_problem;
+
+/* Bytes of device workspace pinmpc_split_solve needs (0 on unsupported sizes): H_k, G_k and seven lifted vectors
+ * per stage, about 4 KB per stage at nu = 12. */
+size_t pinmpc_split_workspace_bytes(int nu, int N, int B);
+
+/* Factorise and run `iters` iterations, asynchronously on `stream`.  Outputs (DEVICE, any may be NULL):
+ * xi [B,N,13+nu] = xi_1..xi_N = [x_{k+1} ; u_k] of the last (21a) step, z [B,N,13+nu] = the feasible copy,
+ * r_prim [B] = max_k |xi_{k+1} - z_{k+1}|_inf of the last iteration.  h_Qdiag [13], h_Rdiag [nu]: HOST.
+ * PINMPC_EUNSUPPORTED: nu not in {12,18}, layout not (2,0)/(2,2), N outside 1..PINMPC_N_MAX; PINMPC_EINVAL: NULL
+ * required pointer, rho <= 0, iters < 1, negative weight; PINMPC_EALLOC: workspace too small; B = 0: no-op. */
+pinmpc_status pinmpc_split_solve(int nu, int N, int B, const pinmpc_layout *layout, const float *h_Qdiag, const float *h_Rdiag,
+                                 float rho, int iters, const pinmpc_split_problem *p, void *d_workspace, size_t workspace_bytes,
+                                 float *xi, float *z, float *r_prim, void *stream);
+
 /* Human-readable description of the last error on this handle (owned by the handle; "" if none).
  * With h = NULL: the last pinmpc_create failure in this thread. */
 const char *pinmpc_last_error(pinmpc_t h);

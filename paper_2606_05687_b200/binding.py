@@ -26,7 +26,7 @@ EXPORTS = ("pinmpc_workspace_bytes", "pinmpc_workspace_bytes_method", "pinmpc_cr
            "pinmpc_get", "pinmpc_get_aux", "pinmpc_get_dynamics", "pinmpc_last_launch_count", "pinmpc_last_error",
            "pinmpc_destroy", "pinmpc_probe_fma", "pinmpc_set_profiling", "pinmpc_get_kernel_ms",
            "pinmpc_set_warm_start", "pinmpc_shift_aux", "pinmpc_landmark_ring_bytes", "pinmpc_landmark_reset", "pinmpc_landmark_push",
-           "pinmpc_landmark_push_solver", "pinmpc_landmark_reward")
+           "pinmpc_landmark_push_solver", "pinmpc_landmark_reward", "pinmpc_split_workspace_bytes", "pinmpc_split_solve")
 MAX_LANDMARKS = 8
 
 
@@ -44,6 +44,10 @@ class Layout(ctypes.Structure):
 class Problem(ctypes.Structure):
     _fields_ = [(n, c_void_p) for n in ("x0", "x_ref", "u_ref", "contact", "foot_r", "yaw", "mass", "inertia",
                                         "ext_wrench")]
+
+
+class SplitProblem(ctypes.Structure):
+    _fields_ = [(n, c_void_p) for n in ("A", "Bm", "c", "x0", "u_prev", "x_ref", "u_ref", "contact")]
 
 
 class LandmarkCfg(ctypes.Structure):
@@ -114,6 +118,11 @@ def load():
     lib.pinmpc_landmark_push_solver.argtypes = [c_void_p, c_void_p, POINTER(LandmarkCfg), c_void_p, c_void_p]
     lib.pinmpc_landmark_reward.restype = c_int
     lib.pinmpc_landmark_reward.argtypes = [c_void_p, c_int, c_int, POINTER(LandmarkCfg)] + [c_void_p] * 5
+    lib.pinmpc_split_workspace_bytes.restype = c_size_t
+    lib.pinmpc_split_workspace_bytes.argtypes = [c_int, c_int, c_int]
+    lib.pinmpc_split_solve.restype = c_int
+    lib.pinmpc_split_solve.argtypes = [c_int, c_int, c_int, POINTER(Layout), POINTER(c_float), POINTER(c_float), c_float, c_int,
+                                       POINTER(SplitProblem), c_void_p, c_size_t, c_void_p, c_void_p, c_void_p, c_void_p]
     lib.pinmpc_destroy.restype = None
     lib.pinmpc_destroy.argtypes = [c_void_p]
     _lib = lib
@@ -418,3 +427,26 @@ class Landmarks:
         _check(load().pinmpc_landmark_reward(_ptr(self.ring), self.B, self.N, ctypes.byref(self.cfg), _ptr(c_real), _ptr(t),
                                              _ptr(r), _ptr(used), self._s(stream)))
         return r, used
+
+
+# ---- the paper's own stage-local ADMM (include/pinmpc.h, eq. (18)-(22)) ---------------------------------
+def split_solve(A, Bm, c, x0, u_prev, x_ref, u_ref, contact, layout, Qdiag, Rdiag, rho, iters, stream=None):
+    """One pinmpc_split_solve call on torch CUDA tensors (float32, contiguous; c, u_prev, u_ref may be None).
+    Returns (xi [B,N,13+nu], z [B,N,13+nu], r_prim [B]) as new device tensors; the workspace is allocated here."""
+    import torch
+    B, N, _, nu = Bm.shape
+    dev = Bm.device
+    nbytes = load().pinmpc_split_workspace_bytes(nu, N, B)
+    if nbytes == 0:
+        raise PinmpcError(EUNSUPPORTED, "unsupported sizes")
+    ws = torch.empty(nbytes, dtype=torch.uint8, device=dev)
+    xi = torch.empty((B, N, NX + nu), dtype=torch.float32, device=dev)
+    z = torch.empty_like(xi)
+    r = torch.empty(B, dtype=torch.float32, device=dev)
+    prob = SplitProblem(*[None if t is None else t.data_ptr() for t in (A, Bm, c, x0, u_prev, x_ref, u_ref, contact)])
+    Qd = (c_float * NX)(*[float(v) for v in Qdiag]); Rd = (c_float * nu)(*[float(v) for v in Rdiag])
+    st = c_void_p(torch.cuda.current_stream(dev).cuda_stream if stream is None else stream.cuda_stream)
+    _check(load().pinmpc_split_solve(nu, N, B, ctypes.byref(layout), Qd, Rd, float(rho), int(iters), ctypes.byref(prob),
+                                     _ptr(ws), nbytes, _ptr(xi), _ptr(z), _ptr(r), st))
+    torch.cuda.current_stream(dev).synchronize()      # the workspace dies with this frame
+    return xi, z, r

@@ -1,0 +1,307 @@
+// The paper's own stage-local ADMM (pi^n MPC proper), eq. (18)-(22); SURVEY 8(f) rank 1.
+// Second method next to the exact-dynamics solver: no recursion over the horizon, every update is local to a
+// stage and reads at most the neighbouring stage.  Generic dense LTV data (A_k, B_k, c_k), nx = 13.
+//
+// Lifted state xi_k = [x_k ; u_{k-1}] (n = 13 + nu <= 31), Ab = [[A, B],[0, I]], Bb = [B ; I], eb = [c ; 0].
+// One warp per stage, lane i = component i of the lifted vectors; matrices are read so that consecutive lanes
+// touch consecutive words (H and G are symmetric, so "column i" is read as row-major [j][i]).
+//   k_split_factor  G_k = (B_k^T B_k + I)^-1 (J_k = G_k Bb_k^T) and H_k = (Qb + rho I + rho Ab_{k+1}^T Ab_{k+1})^-1,
+//                   Gauss-Jordan in shared memory without pivoting (both SPD)
+//   k_split_a       (21a): du_k = J_k (v_k - beta_k), xi_{k+1} = H_k h_k from the previous z, v, theta, beta, lambda
+//   k_split_b       (21b), (21c): gamma, gamma~, z = Proj((2 gamma~ + gamma)/3), v = (z + gamma)/2, dual updates
+// This first version streams H, G, A, B from HBM every iteration (about 5.5 KB + 2 KB per stage-iteration): it is
+// HBM-bound by construction and is reported as such.
+#include "pinmpc_common.cuh"
+
+namespace {
+
+constexpr unsigned FULL = 0xffffffffu;
+constexpr int SPLIT_WARPS = 8;
+constexpr int NW_FEET = 2;              // 6-D wrench contacts (supported layouts: (2,0) and (2,2))
+
+struct SplitPtrs {
+    const float *A, *Bm, *c, *x0, *u_prev, *x_ref, *u_ref;
+    const uint8_t *contact;
+    float *H, *G;                          // [st][n][n], [st][nu][nu]
+    float *xi, *du, *z, *v, *th, *be, *la; // [st][n] (du: [st][nu])
+    float *rs;                             // [st] per-stage primal residual of the last iteration
+};
+
+// in-place inverse of the SPD m x m matrix M (row stride ld) held in shared memory; lane = row
+__device__ __forceinline__ void spd_inverse_smem(float *M, int m, int ld, int lane)
+{
+    for (int p = 0; p < m; p++) {
+        const float d = 1.0f / M[p * ld + p];
+        __syncwarp();
+        if (lane == p) {
+            for (int j = 0; j < m; j++) M[p * ld + j] = (j == p) ? d : M[p * ld + j] * d;
+        }
+        __syncwarp();
+        if (lane < m && lane != p) {
+            const float f = M[lane * ld + p];
+            for (int j = 0; j < m; j++) M[lane * ld + j] = (j == p) ? -f * d : fmaf(-f, M[p * ld + j], M[lane * ld + j]);
+        }
+        __syncwarp();
+    }
+}
+
+template <int NU>
+__global__ void __launch_bounds__(SPLIT_WARPS * 32) k_split_factor(SolveParams P, SplitPtrs q)
+{
+    constexpr int n = NX + NU, LD = n + 1;
+    __shared__ float sm[SPLIT_WARPS][n * LD];
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    const long s = (long)blockIdx.x * SPLIT_WARPS + wib, st = (long)P.B * P.N;
+    if (s >= st) return;
+    const int k = (int)(s % P.N);
+    float *M = sm[wib];
+    // ---- G = (B^T B + I)^-1
+    {
+        const float *Bk = q.Bm + s * NX * NU;
+        if (lane < NU) {
+            for (int j = 0; j < NU; j++) {
+                float acc = lane == j ? 1.0f : 0.0f;
+                for (int a = 0; a < NX; a++) acc = fmaf(Bk[a * NU + lane], Bk[a * NU + j], acc);
+                M[lane * LD + j] = acc;
+            }
+        }
+        __syncwarp();
+        spd_inverse_smem(M, NU, LD, lane);
+        if (lane < NU)
+            for (int j = 0; j < NU; j++) q.G[s * NU * NU + j * NU + lane] = M[j * LD + lane];
+        __syncwarp();
+    }
+    // ---- H = (Qb + rho I [+ rho Ab_{k+1}^T Ab_{k+1}])^-1 ;  Ab^T Ab = [[A^T A, A^T B],[B^T A, B^T B + I]]
+    if (lane < n) {
+        const float qd = lane < NX ? P.Qd[lane] : P.Rd[lane - NX];
+        if (k == P.N - 1) {
+            for (int j = 0; j < n; j++) M[lane * LD + j] = lane == j ? qd + P.rho : 0.0f;
+        } else {
+            const float *A1 = q.A + (s + 1) * NX * NX, *B1 = q.Bm + (s + 1) * NX * NU;
+            for (int j = 0; j < n; j++) {
+                float acc = (lane == j && lane >= NX) ? 1.0f : 0.0f;
+                for (int a = 0; a < NX; a++) {
+                    const float li = lane < NX ? A1[a * NX + lane] : B1[a * NU + lane - NX];
+                    const float lj = j < NX ? A1[a * NX + j] : B1[a * NU + j - NX];
+                    acc = fmaf(li, lj, acc);
+                }
+                M[lane * LD + j] = fmaf(P.rho, acc, lane == j ? qd + P.rho : 0.0f);
+            }
+        }
+    }
+    __syncwarp();
+    spd_inverse_smem(M, n, LD, lane);
+    if (lane < n)
+        for (int j = 0; j < n; j++) q.H[s * n * n + j * n + lane] = M[j * LD + lane];
+}
+
+// (21a)
+template <int NU>
+__global__ void __launch_bounds__(SPLIT_WARPS * 32) k_split_a(SolveParams P, SplitPtrs q)
+{
+    constexpr int n = NX + NU;
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    const long s = (long)blockIdx.x * SPLIT_WARPS + wib, st = (long)P.B * P.N;
+    if (s >= st) return;
+    const int k = (int)(s % P.N);
+    const bool on = lane < n, isx = lane < NX;
+    const int ju = isx ? 0 : (on ? lane - NX : 0);
+    const float *Bk = q.Bm + s * NX * NU;
+    // du = G (B^T r_x + r_u),  r = v - beta
+    const float r = on ? q.v[s * n + lane] - q.be[s * n + lane] : 0.0f;
+    float t = __shfl_sync(FULL, r, NX + (lane < NU ? lane : 0));            // r_u[lane] on lanes < NU
+#pragma unroll
+    for (int a = 0; a < NX; a++) {
+        const float ra = __shfl_sync(FULL, r, a);
+        if (lane < NU) t = fmaf(Bk[a * NU + lane], ra, t);
+    }
+    float du = 0.0f;
+    const float *Gk = q.G + s * NU * NU;
+#pragma unroll
+    for (int l = 0; l < NU; l++) {
+        const float tl = __shfl_sync(FULL, t, l);
+        if (lane < NU) du = fmaf(Gk[l * NU + lane], tl, du);
+    }
+    if (lane < NU) q.du[s * NU + lane] = du;
+    // h = qb + rho (z - theta) + rho Ab_{k+1}^T (z_{k+1} - v_{k+1} - eb_{k+1} + lam_{k+1})
+    float h = 0.0f;
+    if (on) {
+        const float ref = isx ? q.x_ref[s * NX + lane] : (q.u_ref ? q.u_ref[s * NU + ju] : 0.0f);
+        const float qd = isx ? P.Qd[lane] : P.Rd[ju];
+        h = fmaf(P.rho, q.z[s * n + lane] - q.th[s * n + lane], qd * ref);
+    }
+    if (k < P.N - 1) {
+        const long s1 = s + 1;
+        float w = 0.0f;
+        if (on) {
+            w = q.z[s1 * n + lane] - q.v[s1 * n + lane] + q.la[s1 * n + lane];
+            if (isx && q.c) w -= q.c[s1 * NX + lane];
+        }
+        const float *A1 = q.A + s1 * NX * NX, *B1 = q.Bm + s1 * NX * NU;
+        float acc = isx ? 0.0f : w;
+#pragma unroll
+        for (int a = 0; a < NX; a++) {
+            const float wa = __shfl_sync(FULL, w, a);
+            if (on) acc = fmaf(isx ? A1[a * NX + lane] : B1[a * NU + ju], wa, acc);
+        }
+        h = fmaf(P.rho, acc, h);
+    }
+    // xi = H h
+    const float *Hk = q.H + s * n * n;
+    float xi = 0.0f;
+#pragma unroll
+    for (int j = 0; j < n; j++) {
+        const float hj = __shfl_sync(FULL, h, j);
+        if (on) xi = fmaf(Hk[j * n + lane], hj, xi);
+    }
+    if (on) q.xi[s * n + lane] = xi;
+}
+
+// (21b), (21c)
+template <int NU>
+__global__ void __launch_bounds__(SPLIT_WARPS * 32) k_split_b(SolveParams P, SplitPtrs q, int last)
+{
+    constexpr int n = NX + NU, NC = 2 + (NU - 12) / 3;
+    __shared__ float su[SPLIT_WARPS][NU_MAX + 2];
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    const long s = (long)blockIdx.x * SPLIT_WARPS + wib, st = (long)P.B * P.N;
+    if (s >= st) return;
+    const long b = s / P.N;
+    const int k = (int)(s - b * P.N);
+    const bool on = lane < n, isx = lane < NX;
+    const int ju = isx ? 0 : (on ? lane - NX : 0);
+    const float *Ak = q.A + s * NX * NX, *Bk = q.Bm + s * NX * NU;
+    // xi_k (the lifted state entering stage k): data for k = 0
+    float xp = 0.0f;
+    if (on) {
+        if (k == 0) xp = isx ? q.x0[b * NX + lane] : (q.u_prev ? q.u_prev[b * NU + ju] : 0.0f);
+        else xp = q.xi[(s - 1) * n + lane];
+    }
+    const float du = (on && !isx) ? q.du[s * NU + ju] : 0.0f;
+    // Ab xi_k and Bb du
+    float Axi = isx ? 0.0f : xp, Bdu = isx ? 0.0f : du;
+#pragma unroll
+    for (int a = 0; a < n; a++) {
+        const float xa = __shfl_sync(FULL, xp, a);
+        if (isx) Axi = fmaf(a < NX ? Ak[lane * NX + a] : Bk[lane * NU + a - NX], xa, Axi);
+    }
+#pragma unroll
+    for (int j = 0; j < NU; j++) {
+        const float dj = __shfl_sync(FULL, du, NX + j);
+        if (isx) Bdu = fmaf(Bk[lane * NU + j], dj, Bdu);
+    }
+    float xi = 0.0f, th = 0.0f, be = 0.0f, la = 0.0f, e = 0.0f;
+    if (on) {
+        xi = q.xi[s * n + lane]; th = q.th[s * n + lane]; be = q.be[s * n + lane]; la = q.la[s * n + lane];
+        if (isx && q.c) e = q.c[s * NX + lane];
+    }
+    const float gamma = Bdu + be - Axi - e + la;
+    const float gammat = xi + th + Axi + e - la;
+    const float w = (2.0f * gammat + gamma) * (1.0f / 3.0f);
+    // projection of the u part onto U_k (the x part is free): through shared memory, one lane per contact
+    float *uw = su[wib];
+    if (on && !isx) uw[ju] = w;
+    __syncwarp();
+    if (lane < NC) {
+        const bool in_contact = q.contact[s * NC + lane] != 0;
+        if (lane < NW_FEET) {
+            const int f0 = 3 * lane, m0 = 3 * NW_FEET + 3 * lane;
+            float o[6] = { 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f };
+            if (in_contact) project_wrench(P, uw[f0], uw[f0 + 1], uw[f0 + 2], uw[m0], uw[m0 + 1], uw[m0 + 2], o[0], o[1], o[2], o[3], o[4], o[5]);
+            uw[f0] = o[0]; uw[f0 + 1] = o[1]; uw[f0 + 2] = o[2]; uw[m0] = o[3]; uw[m0 + 1] = o[4]; uw[m0 + 2] = o[5];
+        } else {
+            const int f0 = 6 * NW_FEET + 3 * (lane - NW_FEET);
+#pragma unroll
+            for (int a = 0; a < 3; a++) uw[f0 + a] = in_contact ? fminf(fmaxf(uw[f0 + a], -P.hand_fmax), P.hand_fmax) : 0.0f;
+        }
+    }
+    __syncwarp();
+    const float z = isx ? w : (on ? uw[ju] : 0.0f);
+    const float v = 0.5f * (z + gamma);
+    if (on) {
+        q.z[s * n + lane] = z;
+        q.v[s * n + lane] = v;
+        q.th[s * n + lane] = th + xi - z;
+        q.be[s * n + lane] = be + Bdu - v;
+        q.la[s * n + lane] = la + z - Axi - v - e;
+    }
+    if (last) {
+        const float rmax = warp_max(on ? fabsf(xi - z) : 0.0f);
+        if (lane == 0) q.rs[s] = rmax;
+    }
+}
+
+__global__ void k_split_residual(const float *rs, float *r_prim, int B, int N)
+{
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= B) return;
+    float m = 0.0f;
+    for (int k = 0; k < N; k++) m = fmaxf(m, rs[(long)b * N + k]);
+    r_prim[b] = m;
+}
+
+size_t split_floats(int nu, long st)
+{
+    const long n = NX + nu;
+    return (size_t)st * (n * n + nu * nu + 7 * n + nu + 1);
+}
+
+template <int NU>
+pinmpc_status run(const SolveParams &P, SplitPtrs q, int iters, float *r_prim, cudaStream_t stream)
+{
+    const long st = (long)P.B * P.N;
+    const unsigned blocks = (unsigned)((st + SPLIT_WARPS - 1) / SPLIT_WARPS);
+    k_split_factor<NU><<<blocks, SPLIT_WARPS * 32, 0, stream>>>(P, q);
+    for (int it = 0; it < iters; it++) {
+        k_split_a<NU><<<blocks, SPLIT_WARPS * 32, 0, stream>>>(P, q);
+        k_split_b<NU><<<blocks, SPLIT_WARPS * 32, 0, stream>>>(P, q, it == iters - 1 && r_prim != nullptr);
+    }
+    if (r_prim) k_split_residual<<<(P.B + 127) / 128, 128, 0, stream>>>(q.rs, r_prim, P.B, P.N);
+    return cudaGetLastError() == cudaSuccess ? PINMPC_OK : PINMPC_ECUDA;
+}
+
+}   // namespace
+
+extern "C" size_t pinmpc_split_workspace_bytes(int nu, int N, int B)
+{
+    if ((nu != 12 && nu != 18) || N < 1 || N > PINMPC_N_MAX || B < 0) return 0;
+    return split_floats(nu, (long)B * N) * sizeof(float) + 256;
+}
+
+extern "C" pinmpc_status pinmpc_split_solve(int nu, int N, int B, const pinmpc_layout *layout, const float *h_Qdiag, const float *h_Rdiag,
+                                            float rho, int iters, const pinmpc_split_problem *p, void *d_ws, size_t ws_bytes,
+                                            float *xi, float *z, float *r_prim, void *stream)
+{
+    if ((nu != 12 && nu != 18) || N < 1 || N > PINMPC_N_MAX) return PINMPC_EUNSUPPORTED;
+    if (!layout || layout->n_wrench != 2 || 6 * layout->n_wrench + 3 * layout->n_force != nu) return PINMPC_EUNSUPPORTED;
+    if (B < 0 || !(rho > 0.0f) || iters < 1 || !h_Qdiag || !h_Rdiag || !p) return PINMPC_EINVAL;
+    if (B == 0) return PINMPC_OK;
+    if (!p->A || !p->Bm || !p->x0 || !p->x_ref || !p->contact || !d_ws) return PINMPC_EINVAL;
+    if (ws_bytes < pinmpc_split_workspace_bytes(nu, N, B)) return PINMPC_EALLOC;
+    cudaStream_t st_ = (cudaStream_t)stream;
+    SolveParams P;
+    memset(&P, 0, sizeof P);
+    P.B = B; P.N = N; P.nu = nu; P.nw = layout->n_wrench; P.nf = layout->n_force; P.iters = iters; P.rho = rho;
+    P.mu = layout->mu; P.fz_max = layout->fz_max; P.cx = layout->mx_coef; P.cy = layout->my_coef; P.cz = layout->mz_coef;
+    P.hand_fmax = layout->hand_fmax;
+    for (int i = 0; i < NX; i++) { if (!(h_Qdiag[i] >= 0.0f)) return PINMPC_EINVAL; P.Qd[i] = h_Qdiag[i]; }
+    for (int i = 0; i < nu; i++) { if (!(h_Rdiag[i] >= 0.0f)) return PINMPC_EINVAL; P.Rd[i] = h_Rdiag[i]; }
+    P.iw[0] = P.iw[1] = 1.0f / P.mu; P.iw[2] = 1.0f / P.cx; P.iw[3] = 1.0f / P.cy; P.iw[4] = 1.0f / P.cz;
+    const long stg = (long)B * N, n = NX + nu;
+    float *w = reinterpret_cast<float *>(((uintptr_t)d_ws + 255) & ~(uintptr_t)255);
+    SplitPtrs q;
+    q.A = p->A; q.Bm = p->Bm; q.c = p->c; q.x0 = p->x0; q.u_prev = p->u_prev; q.x_ref = p->x_ref; q.u_ref = p->u_ref; q.contact = p->contact;
+    q.H = w; w += stg * n * n;
+    q.G = w; w += stg * nu * nu;
+    q.xi = w; w += stg * n; q.z = w; w += stg * n; q.v = w; w += stg * n; q.th = w; w += stg * n; q.be = w; w += stg * n; q.la = w; w += stg * n;
+    q.du = w; w += stg * nu;
+    q.rs = w; w += stg;
+    // all iterates start at 0 (z, v, theta, beta, lambda are contiguous)
+    if (cudaMemsetAsync(q.z, 0, (size_t)stg * n * 5 * sizeof(float), st_) != cudaSuccess) return PINMPC_ECUDA;
+    pinmpc_status rc = nu == 12 ? run<12>(P, q, iters, r_prim, st_) : run<18>(P, q, iters, r_prim, st_);
+    if (rc != PINMPC_OK) return rc;
+    const size_t bytes = (size_t)stg * n * sizeof(float);
+    if (xi && cudaMemcpyAsync(xi, q.xi, bytes, cudaMemcpyDeviceToDevice, st_) != cudaSuccess) return PINMPC_ECUDA;
+    if (z && cudaMemcpyAsync(z, q.z, bytes, cudaMemcpyDeviceToDevice, st_) != cudaSuccess) return PINMPC_ECUDA;
+    return PINMPC_OK;
+}

@@ -1,0 +1,106 @@
+"""GPU parity of the paper's own stage-local ADMM (pinmpc_split_solve, eq. (18)-(22)) against
+oracle/split.py, through the C ABI, after the same number of iterations from the same start.
+
+Inputs: the SRB workloads of gen/ (dynamics assembled by the fp64 oracle and rounded to float32 once, so that both
+sides consume identical A_k, B_k, c_k) and random well-scaled LTV problems.  Tolerances as for the main path
+(north_star): |d xi_x| <= 1e-4 (1 + |x|_inf), |d xi_u| <= 1e-3 (1 + |u|_inf) per env, same for z.
+"""
+import numpy as np
+import pytest
+
+import gen
+import oracle
+from oracle import split
+
+pytestmark = pytest.mark.gpu
+
+
+def gpu_split(w, A, Bm, c, u_prev, rho, iters):
+    import torch
+    from paper_2606_05687_b200 import binding, make_layout
+    lay = make_layout(w.n_wrench, w.n_force, w.mu, w.fz_max, w.mx_coef, w.my_coef, w.mz_coef, w.hand_fmax)
+    d = lambda a, t=np.float32: None if a is None else torch.from_numpy(np.ascontiguousarray(a, dtype=t)).cuda()
+    xi, z, r = binding.split_solve(d(A), d(Bm), d(c), d(w.x0), d(u_prev), d(w.x_ref), d(w.u_ref), d(w.contact, np.uint8), lay,
+                                   w.Qdiag, w.Rdiag, rho, iters)
+    return xi.cpu().numpy(), z.cpu().numpy(), r.cpu().numpy()
+
+
+def oracle_split(w, A, Bm, c, u_prev, rho, iters, envs):
+    lay = oracle.layout_of(w)
+    out = []
+    for b in envs:
+        proj = lambda k, v, b=b: oracle.project(lay, w.contact[b, k:k + 1], v[None])[0]
+        cb = np.zeros((w.N, 13)) if c is None else c[b]
+        up = np.zeros(w.nu) if u_prev is None else u_prev[b]
+        out.append(split.solve_env(A[b], Bm[b], cb, w.Qdiag, w.Rdiag, rho, iters, w.x0[b], up, w.x_ref[b], w.u_ref[b], proj))
+    return out
+
+
+def check(w, got, ref, envs):
+    xi, z, r = got
+    nx = 13
+    for i, b in enumerate(envs):
+        o = ref[i]
+        tx = 1e-4 * (1 + np.abs(o["xi"][:, :nx]).max()); tu = 1e-3 * (1 + np.abs(o["xi"][:, nx:]).max())
+        for name, g in (("xi", xi[b]), ("z", z[b])):
+            dx = np.abs(g[:, :nx] - o[name][:, :nx]).max(); du = np.abs(g[:, nx:] - o[name][:, nx:]).max()
+            assert dx <= tx, f"env {b} {name} x: {dx / tx:.2f} tol"
+            assert du <= tu, f"env {b} {name} u: {du / tu:.2f} tol"
+        assert abs(r[b] - o["r_prim"]) <= 1e-3 * o["r_prim"] + tu
+
+
+@pytest.mark.parametrize("cfg,B,N,iters", [(0, 24, 10, 40), (1, 9, 21, 25), (3, 7, 12, 30)])
+def test_srb_workloads(cfg, B, N, iters):
+    w = gen.make_config(cfg, B=B, N=N)
+    A, Bm, c = oracle.assemble(w.nu, w.n_wrench, w.n_force, w.dt, w.yaw, w.foot_r, w.mass, w.inertia, w.ext_wrench)
+    A = A.astype(np.float32); Bm = Bm.astype(np.float32); c = None if c is None else c.astype(np.float32)
+    rng = np.random.default_rng(cfg)
+    u_prev = (w.u_ref[:, 0] + rng.normal(size=(B, w.nu))).astype(np.float32)
+    envs = list(range(B))
+    got = gpu_split(w, A, Bm, c, u_prev, w.rho, iters)
+    ref = oracle_split(w, A.astype(np.float64), Bm.astype(np.float64), None if c is None else c.astype(np.float64), u_prev, w.rho, iters, envs)
+    check(w, got, ref, envs)
+    assert np.all(got[2] > 0)
+
+
+def test_random_ltv_converges_to_the_same_point_as_the_oracle():
+    """A well-scaled problem where the iteration converges: after 3000 iterations both sides sit at the optimum."""
+    from dataclasses import replace
+    w = gen.make_config(0, B=5, N=6)
+    rng = np.random.default_rng(4)
+    A = (np.eye(13) + 0.1 * rng.normal(size=(w.B, w.N, 13, 13))).astype(np.float32)
+    Bm = (0.3 * rng.normal(size=(w.B, w.N, 13, w.nu))).astype(np.float32)
+    c = (0.1 * rng.normal(size=(w.B, w.N, 13))).astype(np.float32)
+    w = replace(w, Qdiag=np.ones(13, dtype=np.float32), Rdiag=np.full(w.nu, 0.2, dtype=np.float32),
+                x0=rng.normal(size=(w.B, 13)).astype(np.float32), x_ref=rng.normal(size=(w.B, w.N, 13)).astype(np.float32),
+                u_ref=rng.normal(size=(w.B, w.N, w.nu)).astype(np.float32),
+                contact=np.ones((w.B, w.N, 2), dtype=np.uint8))
+    envs = list(range(w.B))
+    got = gpu_split(w, A, Bm, c, None, 1.0, 3000)
+    ref = oracle_split(w, A.astype(np.float64), Bm.astype(np.float64), c.astype(np.float64), None, 1.0, 3000, envs)
+    check(w, got, ref, envs)
+    assert got[2].max() < 1e-4                                    # converged: xi = z
+
+
+def test_argument_checks():
+    import ctypes
+    import torch
+    from paper_2606_05687_b200 import binding as b, make_layout
+    lib = b.load()
+    assert lib.pinmpc_split_workspace_bytes(12, 10, 4) >= 4 * 10 * 4 * (25 * 25 + 144 + 7 * 25 + 12 + 1)
+    assert lib.pinmpc_split_workspace_bytes(13, 10, 4) == 0 and lib.pinmpc_split_workspace_bytes(12, 0, 4) == 0
+    lay = make_layout(2, 0)
+    Qd = (ctypes.c_float * 13)(*([1.0] * 13)); Rd = (ctypes.c_float * 12)(*([1.0] * 12))
+    prob = b.SplitProblem()
+    ws = torch.empty(1024, dtype=torch.uint8, device="cuda")
+    call = lambda nu, N, B, rho, iters, p, wsb: lib.pinmpc_split_solve(nu, N, B, ctypes.byref(lay), Qd, Rd, rho, iters, p, ctypes.c_void_p(ws.data_ptr()),
+                                                                     wsb, None, None, None, None)
+    assert call(13, 10, 4, 1.0, 5, ctypes.byref(prob), 1024) == b.EUNSUPPORTED
+    assert call(12, 10, 4, 0.0, 5, ctypes.byref(prob), 1024) == b.EINVAL
+    assert call(12, 10, 4, 1.0, 0, ctypes.byref(prob), 1024) == b.EINVAL
+    assert call(12, 10, 4, 1.0, 5, ctypes.byref(prob), 1024) == b.EINVAL          # NULL problem pointers
+    assert call(12, 10, 0, 1.0, 5, ctypes.byref(prob), 1024) == b.OK              # B = 0: no-op
+    x = torch.zeros(4 * 10 * 13 * 13, device="cuda")
+    u8 = torch.zeros(4 * 10 * 2, dtype=torch.uint8, device="cuda")
+    full = b.SplitProblem(x.data_ptr(), x.data_ptr(), None, x.data_ptr(), None, x.data_ptr(), None, u8.data_ptr())
+    assert call(12, 10, 4, 1.0, 5, ctypes.byref(full), 1024) == b.EALLOC          # workspace too small
