@@ -53,6 +53,8 @@ def parse():
     ap.add_argument("--N", type=int, default=None)
     ap.add_argument("--envs-per-cta", type=int, default=0, help="tuning knob of the structured solver (0 = auto)")
     ap.add_argument("--sweep", action="store_true", help="BASELINE.json config 4: B x N table (one JSON line per point)")
+    ap.add_argument("--split", action="store_true",
+                    help="time the paper's own stage-local ADMM (pinmpc_split_solve) on the config instead (one JSON line)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -161,6 +163,57 @@ def run_reference(args):
         "gpu_launches": 0}))
 
 
+def run_split(args):
+    """The paper's own stage-local ADMM (eq. (18)-(22), pinmpc_split_solve) on the same workload: dynamics
+    assembled on the device once (untimed), then factorisation + iters x (two stage-parallel kernels).  HBM-bound by
+    construction in this first version: H_k, G_k, A_k, B_k are streamed every iteration."""
+    import numpy as np
+    import torch
+    import gen
+    from paper_2606_05687_b200 import Solver, SplitSolver, make_layout
+    dev = torch.device("cuda", 0)
+    stream = torch.cuda.current_stream(dev)
+    w = gen.make_config(args.config, B=args.B, N=args.N)
+    lay = make_layout(w.n_wrench, w.n_force, w.mu, w.fz_max, w.mx_coef, w.my_coef, w.mz_coef, w.hand_fmax)
+    s = Solver(w.nu, w.N, w.B, layout=lay, rho=w.rho, iters=w.iters, Qdiag=w.Qdiag, Rdiag=w.Rdiag, dt=w.dt, device=dev)
+    s.set_workload(w)
+    A, Bm, c = s.get_dynamics()
+    d = lambda a, t=torch.float32: None if a is None else torch.from_numpy(np.ascontiguousarray(a)).to(dev, t)
+    x0, x_ref, u_ref, contact = d(w.x0), d(w.x_ref), d(w.u_ref), d(w.contact, torch.uint8)
+    sp = SplitSolver(w.nu, w.N, w.B, lay, w.Qdiag, w.Rdiag, w.rho, w.iters, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    run = lambda: sp.solve(A, Bm, c if w.ext_wrench is not None else None, x0, None, x_ref, u_ref, contact)
+    for _ in range(max(args.warmup, 3)):
+        run()
+    torch.cuda.synchronize(dev)
+    ts = []
+    for _ in range(args.steps):
+        flush.zero_()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream); run(); b.record(stream)
+        torch.cuda.synchronize(dev)
+        ts.append(a.elapsed_time(b))
+    ms = float(np.mean(ts))
+    n = 13 + w.nu
+    st = w.B * w.N
+    # algorithmic bytes per stage-iteration: H (n^2) + G (nu^2) + A_k, B_k twice and A_{k+1}, B_{k+1} once
+    # (3 x (169 + 13 nu)) + lifted vectors (5 read + 5 written in (21b,c); 6 read + xi, du written in (21a)) ...
+    per_stage_iter = 4 * (n * n + w.nu * w.nu + 3 * (169 + 13 * w.nu) + 18 * n)
+    gbs = per_stage_iter * st * w.iters / (ms * 1e-3) / 1e9
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except OSError:
+        peaks = {"hbm_gbs": 6540.0}                            # fallback of the profiling guide
+    print(json.dumps({"metric": "stage-local ADMM (paper eq. 22) solves/s", "value": w.B / (ms * 1e-3), "unit": "solves/s",
+                      "ms_per_step": ms, "steps": args.steps, "n_gpus": 1, "dtype": "f32", "data": "synthetic",
+                      "config": {"workload": w.name, "B": w.B, "N": w.N, "iters": w.iters, "nu": w.nu, "method": "split"},
+                      "stage_iters_per_s": st * w.iters / (ms * 1e-3), "gpu_launches": 2 + 2 * w.iters,
+                      "roofline": {"bound": "hbm", "achieved": gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                                   "frac": gbs / peaks["hbm_gbs"], "traffic": None,
+                                   "bytes_per_stage_iter": per_stage_iter},
+                      "workspace_mb": sp.workspace_bytes / 1e6, "r_prim_max": float(sp.r_prim.max())}))
+
+
 def run_sweep(args):
     """BASELINE.json config 4: B in {1024, 4096, 16384, 65536} x N in {10, 25, 50, 100}, 100 iterations, fp32:
     solves/s, achieved FP32 and HBM rates and the device-memory footprint of every point."""
@@ -205,6 +258,8 @@ def main():
     args = parse()
     if args.impl == "reference":
         return run_reference(args)
+    if args.split:
+        return run_split(args)
     if args.sweep:
         return run_sweep(args)
 

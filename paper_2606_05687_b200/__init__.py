@@ -5,4 +5,4 @@ hand-written CUDA kernels for sm_100a (csrc/).  No CPU fallback.
 """
 from . import binding  # noqa: F401
 from .binding import (METHOD_AUTO, METHOD_DENSE, METHOD_SRB, NX, LandmarkCfg, Landmarks, Layout,  # noqa: F401
-                      PinmpcError, Solver, make_landmark_cfg, make_layout)
+                      PinmpcError, Solver, SplitSolver, make_landmark_cfg, make_layout)

@@ -430,23 +430,37 @@ class Landmarks:
 
 
 # ---- the paper's own stage-local ADMM (include/pinmpc.h, eq. (18)-(22)) ---------------------------------
+class SplitSolver:
+    """Owns the workspace and the output tensors of pinmpc_split_solve; solve() is one asynchronous C-ABI call."""
+
+    def __init__(self, nu, N, B, layout, Qdiag, Rdiag, rho, iters, device="cuda:0"):
+        import torch
+        self.torch, self.device = torch, torch.device(device)
+        self.nu, self.N, self.B, self.layout, self.rho, self.iters = int(nu), int(N), int(B), layout, float(rho), int(iters)
+        self.workspace_bytes = load().pinmpc_split_workspace_bytes(self.nu, self.N, self.B)
+        if self.workspace_bytes == 0:
+            raise PinmpcError(EUNSUPPORTED, "unsupported sizes")
+        self.ws = torch.empty(self.workspace_bytes, dtype=torch.uint8, device=self.device)
+        self.xi = torch.empty((self.B, self.N, NX + self.nu), dtype=torch.float32, device=self.device)
+        self.z = torch.empty_like(self.xi)
+        self.r_prim = torch.empty(self.B, dtype=torch.float32, device=self.device)
+        self.Qd = (c_float * NX)(*[float(v) for v in Qdiag]); self.Rd = (c_float * self.nu)(*[float(v) for v in Rdiag])
+
+    def solve(self, A, Bm, c, x0, u_prev, x_ref, u_ref, contact, stream=None):
+        prob = SplitProblem(*[None if t is None else t.data_ptr() for t in (A, Bm, c, x0, u_prev, x_ref, u_ref, contact)])
+        st = c_void_p(self.torch.cuda.current_stream(self.device).cuda_stream if stream is None else stream.cuda_stream)
+        _check(load().pinmpc_split_solve(self.nu, self.N, self.B, ctypes.byref(self.layout), self.Qd, self.Rd, self.rho, self.iters,
+                                         ctypes.byref(prob), _ptr(self.ws), self.workspace_bytes, _ptr(self.xi), _ptr(self.z),
+                                         _ptr(self.r_prim), st))
+        return self.xi, self.z, self.r_prim
+
+
 def split_solve(A, Bm, c, x0, u_prev, x_ref, u_ref, contact, layout, Qdiag, Rdiag, rho, iters, stream=None):
     """One pinmpc_split_solve call on torch CUDA tensors (float32, contiguous; c, u_prev, u_ref may be None).
-    Returns (xi [B,N,13+nu], z [B,N,13+nu], r_prim [B]) as new device tensors; the workspace is allocated here."""
+    Returns (xi [B,N,13+nu], z [B,N,13+nu], r_prim [B]); synchronises the stream."""
     import torch
     B, N, _, nu = Bm.shape
-    dev = Bm.device
-    nbytes = load().pinmpc_split_workspace_bytes(nu, N, B)
-    if nbytes == 0:
-        raise PinmpcError(EUNSUPPORTED, "unsupported sizes")
-    ws = torch.empty(nbytes, dtype=torch.uint8, device=dev)
-    xi = torch.empty((B, N, NX + nu), dtype=torch.float32, device=dev)
-    z = torch.empty_like(xi)
-    r = torch.empty(B, dtype=torch.float32, device=dev)
-    prob = SplitProblem(*[None if t is None else t.data_ptr() for t in (A, Bm, c, x0, u_prev, x_ref, u_ref, contact)])
-    Qd = (c_float * NX)(*[float(v) for v in Qdiag]); Rd = (c_float * nu)(*[float(v) for v in Rdiag])
-    st = c_void_p(torch.cuda.current_stream(dev).cuda_stream if stream is None else stream.cuda_stream)
-    _check(load().pinmpc_split_solve(nu, N, B, ctypes.byref(layout), Qd, Rd, float(rho), int(iters), ctypes.byref(prob),
-                                     _ptr(ws), nbytes, _ptr(xi), _ptr(z), _ptr(r), st))
-    torch.cuda.current_stream(dev).synchronize()      # the workspace dies with this frame
-    return xi, z, r
+    s = SplitSolver(nu, N, B, layout, Qdiag, Rdiag, rho, iters, device=Bm.device)
+    out = s.solve(A, Bm, c, x0, u_prev, x_ref, u_ref, contact, stream)
+    torch.cuda.current_stream(Bm.device).synchronize()
+    return out

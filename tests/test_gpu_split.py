@@ -104,3 +104,20 @@ def test_argument_checks():
     u8 = torch.zeros(4 * 10 * 2, dtype=torch.uint8, device="cuda")
     full = b.SplitProblem(x.data_ptr(), x.data_ptr(), None, x.data_ptr(), None, x.data_ptr(), None, u8.data_ptr())
     assert call(12, 10, 4, 1.0, 5, ctypes.byref(full), 1024) == b.EALLOC          # workspace too small
+
+
+def test_full_size_config2_sampled():
+    """BASELINE.json config 2 (B = 4096, N = 50, 100 iterations) in the launch configuration bench.py --split
+    times; the oracle follows 6 sampled envs."""
+    w = gen.make_config(2)
+    A, Bm, c = oracle.assemble(w.nu, w.n_wrench, w.n_force, w.dt, w.yaw, w.foot_r, w.mass, w.inertia, w.ext_wrench)
+    A = A.astype(np.float32); Bm = Bm.astype(np.float32)
+    got = gpu_split(w, A, Bm, None, None, w.rho, w.iters)
+    envs = [0, 1, 777, 2048, 4094, 4095]
+    lay = oracle.layout_of(w)
+    ref = []
+    for b in envs:
+        proj = lambda k, v, b=b: oracle.project(lay, w.contact[b, k:k + 1], v[None])[0]
+        ref.append(split.solve_env(A[b].astype(np.float64), Bm[b].astype(np.float64), np.zeros((w.N, 13)), w.Qdiag, w.Rdiag, w.rho,
+                                   w.iters, w.x0[b], np.zeros(w.nu), w.x_ref[b], w.u_ref[b], proj))
+    check(w, got, ref, envs)
