@@ -55,6 +55,8 @@ def parse():
     ap.add_argument("--sweep", action="store_true", help="BASELINE.json config 4: B x N table (one JSON line per point)")
     ap.add_argument("--split", action="store_true",
                     help="time the paper's own stage-local ADMM (pinmpc_split_solve) on the config instead (one JSON line)")
+    ap.add_argument("--split-sweep", action="store_true",
+                    help="scalability table of the stage-local method like the paper's Fig. 3: envs x horizon up to N = 400")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -218,6 +220,63 @@ def run_split(args):
                       "workspace_mb": sp.workspace_bytes / 1e6, "r_prim_max": float(sp.r_prim.max())}))
 
 
+def device_dynamics(w, lay, dev):
+    """A_k, B_k, c_k of workload w assembled on the device by the library (pinmpc_get_dynamics).  The assembly is
+    stage-local, so horizons beyond PINMPC_N_MAX are assembled as B * ceil(N / 200) shorter pseudo-envs and viewed back."""
+    import numpy as np
+    import torch
+    from paper_2606_05687_b200 import Solver
+    B, N = w.B, w.N
+    parts = 1 if N <= 256 else -(-N // 200)
+    while N % parts:
+        parts += 1
+    n1 = N // parts
+    s = Solver(w.nu, n1, B * parts, layout=lay, rho=w.rho, iters=1, Qdiag=w.Qdiag, Rdiag=w.Rdiag, dt=w.dt, device=dev)
+    rs = lambda a: None if a is None else np.ascontiguousarray(a.reshape((B * parts, n1) + a.shape[2:]))
+    rep = lambda a: np.ascontiguousarray(np.repeat(a, parts, axis=0))
+    s.set_problem(rep(w.x0), rs(w.x_ref), rs(w.u_ref), rs(w.contact), rs(w.foot_r), rs(w.yaw), rep(w.mass), rep(w.inertia),
+                  rs(w.ext_wrench))
+    A, Bm, c = s.get_dynamics()
+    torch.cuda.synchronize(dev)
+    s.close()
+    return A.view(B, N, 13, 13), Bm.view(B, N, 13, w.nu), c.view(B, N, 13)
+
+
+def run_split_sweep(args):
+    """Scalability of the stage-local method over envs x horizon (Fig. 3: "even to N=400"; 200
+    iterations is the paper's maximum iteration count for it).  One JSON line per point."""
+    import numpy as np
+    import torch
+    import gen
+    from paper_2606_05687_b200 import SplitSolver, make_layout
+    dev = torch.device("cuda", 0)
+    stream = torch.cuda.current_stream(dev)
+    iters = 200
+    for B in (256, 1024, 4096):
+        for N in (10, 50, 100, 200, 400):
+            w = gen.make_config(4, B=B, N=N, iters=iters)
+            lay = make_layout(w.n_wrench, w.n_force, w.mu, w.fz_max, w.mx_coef, w.my_coef, w.mz_coef, w.hand_fmax)
+            A, Bm, _ = device_dynamics(w, lay, dev)
+            d = lambda a, t=torch.float32: torch.from_numpy(np.ascontiguousarray(a)).to(dev, t)
+            x0, x_ref, u_ref, contact = d(w.x0), d(w.x_ref), d(w.u_ref), d(w.contact, torch.uint8)
+            sp = SplitSolver(w.nu, N, B, lay, w.Qdiag, w.Rdiag, w.rho, iters, device=dev)
+            run = lambda: sp.solve(A, Bm, None, x0, None, x_ref, u_ref, contact)
+            run(); torch.cuda.synchronize(dev)
+            ts = []
+            for _ in range(3):
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(stream); run(); b.record(stream)
+                torch.cuda.synchronize(dev)
+                ts.append(a.elapsed_time(b))
+            ms = float(np.median(ts))
+            print(json.dumps({"split_sweep": w.name, "B": B, "N": N, "iters": iters, "ms_per_solve": ms,
+                              "solves_per_s": B / (ms * 1e-3), "stage_iters_per_s": B * N * iters / (ms * 1e-3),
+                              "workspace_mb": sp.workspace_bytes / 1e6, "dynamics_mb": (A.numel() + Bm.numel()) * 4 / 1e6,
+                              "r_prim_max": float(sp.r_prim.max())}), flush=True)
+            del sp, A, Bm
+            torch.cuda.empty_cache()
+
+
 def run_sweep(args):
     """BASELINE.json config 4: B in {1024, 4096, 16384, 65536} x N in {10, 25, 50, 100}, 100 iterations, fp32:
     solves/s, achieved FP32 and HBM rates and the device-memory footprint of every point."""
@@ -264,6 +323,8 @@ def main():
         return run_reference(args)
     if args.split:
         return run_split(args)
+    if args.split_sweep:
+        return run_split_sweep(args)
     if args.sweep:
         return run_sweep(args)
 

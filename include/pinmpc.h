@@ -40,6 +40,7 @@ extern "C" {
 
 #define PINMPC_NX 13
 #define PINMPC_N_MAX 256
+#define PINMPC_SPLIT_N_MAX 1024     /* the stage-local method has no per-horizon on-chip state (N to 400) */
 
 typedef struct pinmpc_ctx *pinmpc_t;
 
@@ -237,7 +238,7 @@ size_t pinmpc_split_workspace_bytes(int nu, int N, int B);
 /* Factorise and run `iters` iterations, asynchronously on `stream`.  Outputs (DEVICE, any may be NULL):
  * xi [B,N,13+nu] = xi_1..xi_N = [x_{k+1} ; u_k] of the last (21a) step, z [B,N,13+nu] = the feasible copy,
  * r_prim [B] = max_k |xi_{k+1} - z_{k+1}|_inf of the last iteration.  h_Qdiag [13], h_Rdiag [nu]: HOST.
- * PINMPC_EUNSUPPORTED: nu not in {12,18}, layout not (2,0)/(2,2), N outside 1..PINMPC_N_MAX; PINMPC_EINVAL: NULL
+ * PINMPC_EUNSUPPORTED: nu not in {12,18}, layout not (2,0)/(2,2), N outside 1..PINMPC_SPLIT_N_MAX; PINMPC_EINVAL: NULL
  * required pointer, rho <= 0, iters < 1, negative weight; PINMPC_EALLOC: workspace too small; B = 0: no-op. */
 pinmpc_status pinmpc_split_solve(int nu, int N, int B, const pinmpc_layout *layout, const float *h_Qdiag, const float *h_Rdiag,
                                  float rho, int iters, const pinmpc_split_problem *p, void *d_workspace, size_t workspace_bytes,

@@ -264,7 +264,7 @@ pinmpc_status run(const SolveParams &P, SplitPtrs q, int iters, float *r_prim, c
 
 extern "C" size_t pinmpc_split_workspace_bytes(int nu, int N, int B)
 {
-    if ((nu != 12 && nu != 18) || N < 1 || N > PINMPC_N_MAX || B < 0) return 0;
+    if ((nu != 12 && nu != 18) || N < 1 || N > PINMPC_SPLIT_N_MAX || B < 0) return 0;
     return split_floats(nu, (long)B * N) * sizeof(float) + 256;
 }
 
@@ -272,7 +272,7 @@ extern "C" pinmpc_status pinmpc_split_solve(int nu, int N, int B, const pinmpc_l
                                             float rho, int iters, const pinmpc_split_problem *p, void *d_ws, size_t ws_bytes,
                                             float *xi, float *z, float *r_prim, void *stream)
 {
-    if ((nu != 12 && nu != 18) || N < 1 || N > PINMPC_N_MAX) return PINMPC_EUNSUPPORTED;
+    if ((nu != 12 && nu != 18) || N < 1 || N > PINMPC_SPLIT_N_MAX) return PINMPC_EUNSUPPORTED;
     if (!layout || layout->n_wrench != 2 || 6 * layout->n_wrench + 3 * layout->n_force != nu) return PINMPC_EUNSUPPORTED;
     if (B < 0 || !(rho > 0.0f) || iters < 1 || !h_Qdiag || !h_Rdiag || !p) return PINMPC_EINVAL;
     if (B == 0) return PINMPC_OK;

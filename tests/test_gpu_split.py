@@ -49,7 +49,7 @@ def check(w, got, ref, envs):
         assert abs(r[b] - o["r_prim"]) <= 1e-3 * o["r_prim"] + tu
 
 
-@pytest.mark.parametrize("cfg,B,N,iters", [(0, 24, 10, 40), (1, 9, 21, 25), (3, 7, 12, 30), (0, 3, 1, 10), (1, 2, 256, 5)])
+@pytest.mark.parametrize("cfg,B,N,iters", [(0, 24, 10, 40), (1, 9, 21, 25), (3, 7, 12, 30), (0, 3, 1, 10), (1, 2, 256, 5), (4, 2, 400, 6)])
 def test_srb_workloads(cfg, B, N, iters):
     w = gen.make_config(cfg, B=B, N=N)
     A, Bm, c = oracle.assemble(w.nu, w.n_wrench, w.n_force, w.dt, w.yaw, w.foot_r, w.mass, w.inertia, w.ext_wrench)
