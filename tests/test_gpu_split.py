@@ -121,3 +121,19 @@ def test_full_size_config2_sampled():
         ref.append(split.solve_env(A[b].astype(np.float64), Bm[b].astype(np.float64), np.zeros((w.N, 13)), w.Qdiag, w.Rdiag, w.rho,
                                    w.iters, w.x0[b], np.zeros(w.nu), w.x_ref[b], w.u_ref[b], proj))
     check(w, got, ref, envs)
+
+
+def test_bench_long_horizon_assembly_matches_oracle():
+    """bench.device_dynamics assembles horizons beyond PINMPC_N_MAX as shorter pseudo-envs (the assembly is
+    stage-local); the result must be the oracle's assembly of the real horizon."""
+    import torch
+    import bench
+    from paper_2606_05687_b200 import make_layout
+    w = gen.make_config(4, B=3, N=400)
+    lay = make_layout(w.n_wrench, w.n_force, w.mu, w.fz_max, w.mx_coef, w.my_coef, w.mz_coef, w.hand_fmax)
+    A, Bm, c = bench.device_dynamics(w, lay, torch.device("cuda", 0))
+    Ao, Bo, co = oracle.assemble(w.nu, w.n_wrench, w.n_force, w.dt, w.yaw, w.foot_r, w.mass, w.inertia, w.ext_wrench)
+    assert A.shape == (3, 400, 13, 13) and Bm.shape == (3, 400, 13, 12)
+    assert np.abs(A.cpu().numpy() - Ao).max() <= 1e-6
+    assert np.abs(Bm.cpu().numpy() - Bo).max() <= 1e-5 * (1 + np.abs(Bo).max())
+    assert np.abs(c.cpu().numpy()).max() == 0.0
