@@ -323,7 +323,7 @@ constexpr int FAC_WARPS = 4;                        // warps (envs) per CTA
 constexpr int FAC_LD = 16;                          // padded row length
 constexpr int FAC_SMEM = 13 * 16 + 13 * 16 + 6 * 16 + 24;   // floats per warp: P, X, Kh, Mh^-1
 
-__global__ void __launch_bounds__(FAC_WARPS * 32, 8) k_factor_srb(SolveParams P, const float *__restrict__ x0, SrbWs W, int has_ext)
+__global__ void __launch_bounds__(FAC_WARPS * 32, 7) k_factor_srb(SolveParams P, const float *__restrict__ x0, SrbWs W, int has_ext)
 {
     __shared__ __align__(16) float sm_all[FAC_WARPS * FAC_SMEM];
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
