@@ -27,77 +27,91 @@ struct SplitPtrs {
     float *rs;                             // [st] per-stage primal residual of the last iteration
 };
 
-// in-place inverse of the SPD m x m matrix M (row stride ld) held in shared memory; lane = row
-__device__ __forceinline__ void spd_inverse_smem(float *M, int m, int ld, int lane)
+// In-place Gauss-Jordan inverse of an SPD m x m matrix without pivoting: lane i holds row i in registers
+// (lanes >= m hold zero rows), the pivot row is broadcast with shuffles; everything is unrolled, so the rows
+// never leave the register file.
+template <int m> __device__ __forceinline__ void spd_inverse_regs(float (&row)[m], int lane)
 {
+#pragma unroll
     for (int p = 0; p < m; p++) {
-        const float d = 1.0f / M[p * ld + p];
-        __syncwarp();
-        if (lane == p) {
-            for (int j = 0; j < m; j++) M[p * ld + j] = (j == p) ? d : M[p * ld + j] * d;
+        const float d = 1.0f / __shfl_sync(FULL, row[p], p);
+        const float f = row[p];                                  // M[lane][p] before this pivot
+#pragma unroll
+        for (int j = 0; j < m; j++) {
+            const float pj = __shfl_sync(FULL, row[j], p);
+            const float rpj = (j == p) ? d : pj * d;             // the scaled pivot row
+            row[j] = (lane == p) ? rpj : ((j == p) ? -f * d : fmaf(-f, rpj, row[j]));
         }
-        __syncwarp();
-        if (lane < m && lane != p) {
-            const float f = M[lane * ld + p];
-            for (int j = 0; j < m; j++) M[lane * ld + j] = (j == p) ? -f * d : fmaf(-f, M[p * ld + j], M[lane * ld + j]);
-        }
-        __syncwarp();
     }
 }
 
 template <int NU>
 __global__ void __launch_bounds__(SPLIT_WARPS * 32) k_split_factor(SolveParams P, SplitPtrs q)
 {
-    constexpr int n = NX + NU, LD = n + 1;
-    __shared__ float sm[SPLIT_WARPS][n * LD];
+    constexpr int n = NX + NU;
+    __shared__ float sT[SPLIT_WARPS][NX * n];
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     const long s = (long)blockIdx.x * SPLIT_WARPS + wib, st = (long)P.B * P.N;
     if (s >= st) return;
     const int k = (int)(s % P.N);
-    float *M = sm[wib];
-    // ---- G = (B^T B + I)^-1
+    float *T = sT[wib];
+    // ---- G = (B^T B + I)^-1 : B_k staged in shared memory, lane i keeps column i
     {
         const float *Bk = q.Bm + s * NX * NU;
+        for (int i = lane; i < NX * NU; i += 32) T[i] = Bk[i];
+        __syncwarp();
+        const int lu = lane < NU ? lane : 0;
+        float col[NX], g[NU];
+#pragma unroll
+        for (int a = 0; a < NX; a++) col[a] = lane < NU ? T[a * NU + lu] : 0.0f;
+#pragma unroll
+        for (int j = 0; j < NU; j++) {
+            float acc = lane == j ? 1.0f : 0.0f;
+#pragma unroll
+            for (int a = 0; a < NX; a++) acc = fmaf(col[a], T[a * NU + j], acc);
+            g[j] = acc;
+        }
+        spd_inverse_regs<NU>(g, lane);
         if (lane < NU) {
-            for (int j = 0; j < NU; j++) {
-                float acc = lane == j ? 1.0f : 0.0f;
-                for (int a = 0; a < NX; a++) acc = fmaf(Bk[a * NU + lane], Bk[a * NU + j], acc);
-                M[lane * LD + j] = acc;
-            }
+#pragma unroll
+            for (int j = 0; j < NU; j++) q.G[s * NU * NU + j * NU + lane] = g[j];
         }
         __syncwarp();
-        spd_inverse_smem(M, NU, LD, lane);
-        if (lane < NU)
-            for (int j = 0; j < NU; j++) q.G[s * NU * NU + j * NU + lane] = M[j * LD + lane];
-        __syncwarp();
     }
-    // ---- H = (Qb + rho I [+ rho Ab_{k+1}^T Ab_{k+1}])^-1 ;  Ab^T Ab = [[A^T A, A^T B],[B^T A, B^T B + I]]
-    if (lane < n) {
-        const float qd = lane < NX ? P.Qd[lane] : P.Rd[lane - NX];
-        if (k == P.N - 1) {
-            for (int j = 0; j < n; j++) M[lane * LD + j] = lane == j ? qd + P.rho : 0.0f;
-        } else {
-            const float *A1 = q.A + (s + 1) * NX * NX, *B1 = q.Bm + (s + 1) * NX * NU;
-            for (int j = 0; j < n; j++) {
-                float acc = (lane == j && lane >= NX) ? 1.0f : 0.0f;
-                for (int a = 0; a < NX; a++) {
-                    const float li = lane < NX ? A1[a * NX + lane] : B1[a * NU + lane - NX];
-                    const float lj = j < NX ? A1[a * NX + j] : B1[a * NU + j - NX];
-                    acc = fmaf(li, lj, acc);
-                }
-                M[lane * LD + j] = fmaf(P.rho, acc, lane == j ? qd + P.rho : 0.0f);
-            }
+    // ---- H = (Qb + rho I [+ rho Ab_{k+1}^T Ab_{k+1}])^-1 ;  Ab^T Ab = T^T T + [[0, 0],[0, I]],  T = [A_{k+1} B_{k+1}] (13 x n)
+    const bool nxt = k < P.N - 1;
+    if (nxt) {
+        const float *A1 = q.A + (s + 1) * NX * NX, *B1 = q.Bm + (s + 1) * NX * NU;
+        for (int i = lane; i < NX * n; i += 32) {
+            const int a = i / n, j = i - a * n;
+            T[i] = j < NX ? A1[a * NX + j] : B1[a * NU + j - NX];
         }
     }
     __syncwarp();
-    spd_inverse_smem(M, n, LD, lane);
-    if (lane < n)
-        for (int j = 0; j < n; j++) q.H[s * n * n + j * n + lane] = M[j * LD + lane];
+    const int ln = lane < n ? lane : 0;
+    const float qd = lane < NX ? P.Qd[lane] : (lane < n ? P.Rd[lane - NX] : 0.0f);
+    float h[n], col[NX];
+#pragma unroll
+    for (int a = 0; a < NX; a++) col[a] = (nxt && lane < n) ? T[a * n + ln] : 0.0f;
+#pragma unroll
+    for (int j = 0; j < n; j++) {
+        float acc = (lane == j && lane >= NX && nxt) ? 1.0f : 0.0f;
+        if (nxt) {
+#pragma unroll
+            for (int a = 0; a < NX; a++) acc = fmaf(col[a], T[a * n + j], acc);
+        }
+        h[j] = fmaf(P.rho, acc, lane == j ? qd + P.rho : 0.0f);
+    }
+    spd_inverse_regs<n>(h, lane);
+    if (lane < n) {
+#pragma unroll
+        for (int j = 0; j < n; j++) q.H[s * n * n + j * n + lane] = h[j];
+    }
 }
 
 // (21a)
 template <int NU>
-__global__ void __launch_bounds__(SPLIT_WARPS * 32) k_split_a(SolveParams P, SplitPtrs q)
+__global__ void __launch_bounds__(SPLIT_WARPS * 32, 5) k_split_a(SolveParams P, SplitPtrs q)
 {
     constexpr int n = NX + NU;
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
@@ -106,54 +120,60 @@ __global__ void __launch_bounds__(SPLIT_WARPS * 32) k_split_a(SolveParams P, Spl
     const int k = (int)(s % P.N);
     const bool on = lane < n, isx = lane < NX;
     const int ju = isx ? 0 : (on ? lane - NX : 0);
-    const float *Bk = q.Bm + s * NX * NU;
+    // The kernel is bound by memory latency, so the matrix elements a lane needs (column `lane` of B_k, G_k,
+    // Ab_{k+1}, H_k) are requested in batches of independent loads before they are used.
+    const bool nxt = k < P.N - 1;
+    const long s1 = nxt ? s + 1 : s;
+    const float *Bk = q.Bm + s * NX * NU, *Gk = q.G + s * NU * NU, *Hk = q.H + s * n * n;
+    const float *A1 = q.A + s1 * NX * NX, *B1 = q.Bm + s1 * NX * NU;
+    const int lu = lane < NU ? lane : 0, ln = on ? lane : 0;
+    float bb[NX], gb[NU];
+#pragma unroll
+    for (int a = 0; a < NX; a++) bb[a] = Bk[a * NU + lu];
+#pragma unroll
+    for (int l = 0; l < NU; l++) gb[l] = Gk[l * NU + lu];
+    const float vv = on ? q.v[s * n + lane] : 0.0f, bv = on ? q.be[s * n + lane] : 0.0f;
+    const float zv = on ? q.z[s * n + lane] : 0.0f, tv = on ? q.th[s * n + lane] : 0.0f;
+    float w = 0.0f;
+    if (on && nxt) {
+        w = q.z[s1 * n + lane] - q.v[s1 * n + lane] + q.la[s1 * n + lane];
+        if (isx && q.c) w -= q.c[s1 * NX + lane];
+    }
+    const float ref = on ? (isx ? q.x_ref[s * NX + lane] : (q.u_ref ? q.u_ref[s * NU + ju] : 0.0f)) : 0.0f;
     // du = G (B^T r_x + r_u),  r = v - beta
-    const float r = on ? q.v[s * n + lane] - q.be[s * n + lane] : 0.0f;
-    float t = __shfl_sync(FULL, r, NX + (lane < NU ? lane : 0));            // r_u[lane] on lanes < NU
+    const float r = vv - bv;
+    float t = __shfl_sync(FULL, r, NX + lu);                               // r_u[lane] on lanes < NU
 #pragma unroll
-    for (int a = 0; a < NX; a++) {
-        const float ra = __shfl_sync(FULL, r, a);
-        if (lane < NU) t = fmaf(Bk[a * NU + lane], ra, t);
-    }
+    for (int a = 0; a < NX; a++) t = fmaf(bb[a], __shfl_sync(FULL, r, a), t);
+    float ab[NX];
+#pragma unroll
+    for (int a = 0; a < NX; a++) ab[a] = isx ? A1[a * NX + lane] : B1[a * NU + ju];
     float du = 0.0f;
-    const float *Gk = q.G + s * NU * NU;
 #pragma unroll
-    for (int l = 0; l < NU; l++) {
-        const float tl = __shfl_sync(FULL, t, l);
-        if (lane < NU) du = fmaf(Gk[l * NU + lane], tl, du);
-    }
+    for (int l = 0; l < NU; l++) du = fmaf(gb[l], __shfl_sync(FULL, t, l), du);
     if (lane < NU) q.du[s * NU + lane] = du;
+    constexpr int H1 = (n + 1) / 2;
+    float ha[H1];
+#pragma unroll
+    for (int j = 0; j < H1; j++) ha[j] = Hk[j * n + ln];
     // h = qb + rho (z - theta) + rho Ab_{k+1}^T (z_{k+1} - v_{k+1} - eb_{k+1} + lam_{k+1})
     float h = 0.0f;
-    if (on) {
-        const float ref = isx ? q.x_ref[s * NX + lane] : (q.u_ref ? q.u_ref[s * NU + ju] : 0.0f);
-        const float qd = isx ? P.Qd[lane] : P.Rd[ju];
-        h = fmaf(P.rho, q.z[s * n + lane] - q.th[s * n + lane], qd * ref);
-    }
-    if (k < P.N - 1) {
-        const long s1 = s + 1;
-        float w = 0.0f;
-        if (on) {
-            w = q.z[s1 * n + lane] - q.v[s1 * n + lane] + q.la[s1 * n + lane];
-            if (isx && q.c) w -= q.c[s1 * NX + lane];
-        }
-        const float *A1 = q.A + s1 * NX * NX, *B1 = q.Bm + s1 * NX * NU;
+    if (on) h = fmaf(P.rho, zv - tv, (isx ? P.Qd[lane] : P.Rd[ju]) * ref);
+    if (nxt) {
         float acc = isx ? 0.0f : w;
 #pragma unroll
-        for (int a = 0; a < NX; a++) {
-            const float wa = __shfl_sync(FULL, w, a);
-            if (on) acc = fmaf(isx ? A1[a * NX + lane] : B1[a * NU + ju], wa, acc);
-        }
-        h = fmaf(P.rho, acc, h);
+        for (int a = 0; a < NX; a++) acc = fmaf(ab[a], __shfl_sync(FULL, w, a), acc);
+        if (on) h = fmaf(P.rho, acc, h);
     }
+    float hb[n - H1];
+#pragma unroll
+    for (int j = H1; j < n; j++) hb[j - H1] = Hk[j * n + ln];
     // xi = H h
-    const float *Hk = q.H + s * n * n;
     float xi = 0.0f;
 #pragma unroll
-    for (int j = 0; j < n; j++) {
-        const float hj = __shfl_sync(FULL, h, j);
-        if (on) xi = fmaf(Hk[j * n + lane], hj, xi);
-    }
+    for (int j = 0; j < H1; j++) xi = fmaf(ha[j], __shfl_sync(FULL, h, j), xi);
+#pragma unroll
+    for (int j = H1; j < n; j++) xi = fmaf(hb[j - H1], __shfl_sync(FULL, h, j), xi);
     if (on) q.xi[s * n + lane] = xi;
 }
 
