@@ -198,9 +198,9 @@ def run_split(args):
     ms = float(np.mean(ts))
     n = 13 + w.nu
     st = w.B * w.N
-    # algorithmic bytes per stage-iteration: H (n^2) + G (nu^2) + A_k, B_k twice and A_{k+1}, B_{k+1} once
-    # (3 x (169 + 13 nu)) + lifted vectors (5 read + 5 written in (21b,c); 6 read + xi, du written in (21a)) ...
-    per_stage_iter = 4 * (n * n + w.nu * w.nu + 3 * (169 + 13 * w.nu) + 18 * n)
+    # algorithmic bytes per stage-iteration: (21a) reads H_k (n^2), G_k (nu^2), B_k (13 nu), [A_{k+1} B_{k+1}] (13 n);
+    # (21b,c) reads [A_k B_k]^T (13 n); lifted vectors: 6 read + xi, du written in (21a), 5 read + 5 written in (21b,c)
+    per_stage_iter = 4 * (n * n + w.nu * w.nu + 13 * w.nu + 2 * 13 * n + 18 * n)
     gbs = per_stage_iter * st * w.iters / (ms * 1e-3) / 1e9
     try:
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))

@@ -23,6 +23,7 @@ struct SplitPtrs {
     const float *A, *Bm, *c, *x0, *u_prev, *x_ref, *u_ref;
     const uint8_t *contact;
     float *H, *G;                          // [st][n][n], [st][nu][nu]
+    float *Tt;                             // [st][n][13]  [A_k B_k] transposed: column-major rows for coalesced reads in (21b)
     float *xi, *du, *z, *v, *th, *be, *la; // [st][n] (du: [st][nu])
     float *rs;                             // [st] per-stage primal residual of the last iteration
 };
@@ -75,6 +76,20 @@ __global__ void __launch_bounds__(SPLIT_WARPS * 32) k_split_factor(SolveParams P
         if (lane < NU) {
 #pragma unroll
             for (int j = 0; j < NU; j++) q.G[s * NU * NU + j * NU + lane] = g[j];
+        }
+        __syncwarp();
+    }
+    // ---- Tt_k = [A_k B_k]^T for (21b)
+    {
+        const float *Ak = q.A + s * NX * NX, *Bk = q.Bm + s * NX * NU;
+        for (int i = lane; i < NX * n; i += 32) {
+            const int a = i / n, j = i - a * n;
+            T[i] = j < NX ? Ak[a * NX + j] : Bk[a * NU + j - NX];
+        }
+        __syncwarp();
+        for (int i = lane; i < NX * n; i += 32) {
+            const int c = i / NX, r = i - c * NX;
+            q.Tt[s * NX * n + i] = T[r * n + c];
         }
         __syncwarp();
     }
@@ -190,7 +205,7 @@ __global__ void __launch_bounds__(SPLIT_WARPS * 32) k_split_b(SolveParams P, Spl
     const int k = (int)(s - b * P.N);
     const bool on = lane < n, isx = lane < NX;
     const int ju = isx ? 0 : (on ? lane - NX : 0);
-    const float *Ak = q.A + s * NX * NX, *Bk = q.Bm + s * NX * NU;
+    const float *Tt = q.Tt + s * NX * n + (isx ? lane : 0);      // column-major [A_k B_k]: Tt[a * 13 + row]
     // xi_k (the lifted state entering stage k): data for k = 0
     float xp = 0.0f;
     if (on) {
@@ -203,12 +218,12 @@ __global__ void __launch_bounds__(SPLIT_WARPS * 32) k_split_b(SolveParams P, Spl
 #pragma unroll
     for (int a = 0; a < n; a++) {
         const float xa = __shfl_sync(FULL, xp, a);
-        if (isx) Axi = fmaf(a < NX ? Ak[lane * NX + a] : Bk[lane * NU + a - NX], xa, Axi);
+        if (isx) Axi = fmaf(Tt[a * NX], xa, Axi);
     }
 #pragma unroll
     for (int j = 0; j < NU; j++) {
         const float dj = __shfl_sync(FULL, du, NX + j);
-        if (isx) Bdu = fmaf(Bk[lane * NU + j], dj, Bdu);
+        if (isx) Bdu = fmaf(Tt[(NX + j) * NX], dj, Bdu);
     }
     float xi = 0.0f, th = 0.0f, be = 0.0f, la = 0.0f, e = 0.0f;
     if (on) {
@@ -263,7 +278,7 @@ __global__ void k_split_residual(const float *rs, float *r_prim, int B, int N)
 size_t split_floats(int nu, long st)
 {
     const long n = NX + nu;
-    return (size_t)st * (n * n + nu * nu + 7 * n + nu + 1);
+    return (size_t)st * (n * n + nu * nu + NX * n + 7 * n + nu + 1);
 }
 
 template <int NU>
@@ -313,6 +328,7 @@ extern "C" pinmpc_status pinmpc_split_solve(int nu, int N, int B, const pinmpc_l
     q.A = p->A; q.Bm = p->Bm; q.c = p->c; q.x0 = p->x0; q.u_prev = p->u_prev; q.x_ref = p->x_ref; q.u_ref = p->u_ref; q.contact = p->contact;
     q.H = w; w += stg * n * n;
     q.G = w; w += stg * nu * nu;
+    q.Tt = w; w += stg * NX * n;
     q.xi = w; w += stg * n; q.z = w; w += stg * n; q.v = w; w += stg * n; q.th = w; w += stg * n; q.be = w; w += stg * n; q.la = w; w += stg * n;
     q.du = w; w += stg * nu;
     q.rs = w; w += stg;
