@@ -214,7 +214,7 @@ def run_split(args):
                                    "frac": gbs / peaks["hbm_gbs"],
                                    # dram read + write of one k_split_a plus one k_split_b launch (one iteration),
                                    # ncu --set full, profiles/r1_split_ncu.md; measured at config 2 only
-                                   "traffic": (1016844000 + 31739392 + 358628352 + 81179648) if w.name == "c2_long_horizon" else None,
+                                   "traffic": (1016841000 + 31662592 + 358631936 + 81859584) if w.name == "c2_long_horizon" else None,
                                    "traffic_unit": "bytes per iteration (both kernels)",
                                    "bytes_per_stage_iter": per_stage_iter, "scope": "whole solve (factorisation + all iterations)"},
                       "workspace_mb": sp.workspace_bytes / 1e6, "r_prim_max": float(sp.r_prim.max())}))

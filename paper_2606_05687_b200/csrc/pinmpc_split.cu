@@ -5,12 +5,13 @@
 // Lifted state xi_k = [x_k ; u_{k-1}] (n = 13 + nu <= 31), Ab = [[A, B],[0, I]], Bb = [B ; I], eb = [c ; 0].
 // One warp per stage, lane i = component i of the lifted vectors; matrices are read so that consecutive lanes
 // touch consecutive words (H and G are symmetric, so "column i" is read as row-major [j][i]).
-//   k_split_factor  G_k = (B_k^T B_k + I)^-1 (J_k = G_k Bb_k^T) and H_k = (Qb + rho I + rho Ab_{k+1}^T Ab_{k+1})^-1,
-//                   Gauss-Jordan in shared memory without pivoting (both SPD)
+//   k_split_factor  G_k = (B_k^T B_k + I)^-1 (J_k = G_k Bb_k^T), H_k = (Qb + rho I + rho Ab_{k+1}^T Ab_{k+1})^-1 (both SPD:
+//                   Gauss-Jordan without pivoting, rows in registers, pivot row broadcast by shuffles) and
+//                   [A_k B_k]^T for the coalesced row reads of (21b)
 //   k_split_a       (21a): du_k = J_k (v_k - beta_k), xi_{k+1} = H_k h_k from the previous z, v, theta, beta, lambda
 //   k_split_b       (21b), (21c): gamma, gamma~, z = Proj((2 gamma~ + gamma)/3), v = (z + gamma)/2, dual updates
-// This first version streams H, G, A, B from HBM every iteration (about 5.5 KB + 2 KB per stage-iteration): it is
-// HBM-bound by construction and is reported as such.
+// The factors stream from HBM every iteration (about 8.1 KB per stage-iteration at nu = 12): the method is
+// reported against the HBM roofline.
 #include "pinmpc_common.cuh"
 
 namespace {
