@@ -115,9 +115,9 @@ __device__ __forceinline__ void stage_u0(const SolveParams &P, const float *ru, 
     for (int i = 0; i < NC; i++) {
         const float *f = u0 + fcol(i);
         float rx = r[3 * i], ry = r[3 * i + 1], rz = r[3 * i + 2];
-        G0[0] += ry * f[2] - rz * f[1];
-        G0[1] += rz * f[0] - rx * f[2];
-        G0[2] += rx * f[1] - ry * f[0];
+        G0[0] = fmaf(ry, f[2], fmaf(-rz, f[1], G0[0]));
+        G0[1] = fmaf(rz, f[0], fmaf(-rx, f[2], G0[1]));
+        G0[2] = fmaf(rx, f[1], fmaf(-ry, f[0], G0[2]));
         G0[3] += f[0]; G0[4] += f[1]; G0[5] += f[2];
         if (i < NW) {
             const float *m = u0 + mcol(i);
@@ -139,11 +139,11 @@ __device__ __forceinline__ void lam_inv_apply(const SolveParams &P, const float 
     for (int i = 0; i < NC; i++) {
         const float rx = r[3 * i], ry = r[3 * i + 1], rz = r[3 * i + 2];
         const float v0 = P.tR[fcol(i)] * q0, v1 = P.tR[fcol(i) + 1] * q1, v2 = P.tR[fcol(i) + 2] * q2;
-        e0 -= ry * v2 - rz * v1; e1 -= rz * v0 - rx * v2; e2 -= rx * v1 - ry * v0;
+        e0 = fmaf(rz, v1, fmaf(-ry, v2, e0)); e1 = fmaf(rx, v2, fmaf(-rz, v0, e1)); e2 = fmaf(ry, v0, fmaf(-rx, v1, e2));
     }
-    const float t0 = TI[0] * e0 + TI[1] * e1 + TI[2] * e2;
-    const float t1 = TI[1] * e0 + TI[3] * e1 + TI[4] * e2;
-    const float t2 = TI[2] * e0 + TI[4] * e1 + TI[5] * e2;
+    const float t0 = fmaf(TI[0], e0, fmaf(TI[1], e1, TI[2] * e2));
+    const float t1 = fmaf(TI[1], e0, fmaf(TI[3], e1, TI[4] * e2));
+    const float t2 = fmaf(TI[2], e0, fmaf(TI[4], e1, TI[5] * e2));
     float f0 = x[3], f1 = x[4], f2 = x[5];
 #pragma unroll
     for (int i = 0; i < NC; i++) {
@@ -829,8 +829,8 @@ __device__ __forceinline__ void stage_update(const SolveParams &P, const SrbWs &
 #pragma unroll
         for (int i = 0; i < NW; i++) {
             const float rx = g.r[3 * i], ry = g.r[3 * i + 1], rz = g.r[3 * i + 2];
-            const float gl[6] = { lam[1] * rz - lam[2] * ry + lam[3], lam[2] * rx - lam[0] * rz + lam[4],
-                                  lam[0] * ry - lam[1] * rx + lam[5], lam[0], lam[1], lam[2] };
+            const float gl[6] = { fmaf(lam[1], rz, fmaf(-lam[2], ry, lam[3])), fmaf(lam[2], rx, fmaf(-lam[0], rz, lam[4])),
+                                  fmaf(lam[0], ry, fmaf(-lam[1], rx, lam[5])), lam[0], lam[1], lam[2] };
 #pragma unroll
             for (int a = 0; a < 6; a++) {
                 const int c = a < 3 ? fcol(i) + a : mcol(i) + a - 3;
@@ -881,8 +881,8 @@ __device__ __forceinline__ void stage_update(const SolveParams &P, const SrbWs &
                 for (int a = 0; a < 6; a++) { uu[a] = uf[i < NW ? i : 0][a]; zn[a] = zf[i < NW ? i : 0][a]; }
             } else {
                 // u = u0 + Rt^-1 Gh^T lam :  f_i += lam_tau x r_i + lam_F
-                const float gl[3] = { lam[1] * rz - lam[2] * ry + lam[3], lam[2] * rx - lam[0] * rz + lam[4],
-                                      lam[0] * ry - lam[1] * rx + lam[5] };
+                const float gl[3] = { fmaf(lam[1], rz, fmaf(-lam[2], ry, lam[3])), fmaf(lam[2], rx, fmaf(-lam[0], rz, lam[4])),
+                                      fmaf(lam[0], ry, fmaf(-lam[1], rx, lam[5])) };
 #pragma unroll
                 for (int a = 0; a < 3; a++) {
                     const float u0 = fmaf(P.rtR[col[a]], S.z[col[a]] - S.y[col[a]], ru[a]);
@@ -904,7 +904,8 @@ __device__ __forceinline__ void stage_update(const SolveParams &P, const SrbWs &
                     S.z[col[a]] = zn[a]; S.y[col[a]] = yn;
                     u0n[a] = fmaf(P.rtR[col[a]], zn[a] - yn, ru[a]);               // u0 of the next iteration
                 }
-            Gn[0] += ry * u0n[2] - rz * u0n[1]; Gn[1] += rz * u0n[0] - rx * u0n[2]; Gn[2] += rx * u0n[1] - ry * u0n[0];
+            Gn[0] = fmaf(ry, u0n[2], fmaf(-rz, u0n[1], Gn[0])); Gn[1] = fmaf(rz, u0n[0], fmaf(-rx, u0n[2], Gn[1]));
+            Gn[2] = fmaf(rx, u0n[1], fmaf(-ry, u0n[0], Gn[2]));
             Gn[3] += u0n[0]; Gn[4] += u0n[1]; Gn[5] += u0n[2];
             if (i < NW) { Gn[0] += u0n[3]; Gn[1] += u0n[4]; Gn[2] += u0n[5]; }
         }
