@@ -187,7 +187,7 @@ __device__ __forceinline__ float wrench_height(float t0, const float a[5], const
             if (j != i) g -= w[j] * fmaxf(a[j] - w[j] * bi, 0.0f);
         if (g > 0.0f) { num = fmaf(w[i], a[i], num); den = fmaf(w[i], w[i], den); }
     }
-    return num / den;
+    return __fdividef(num, den);                     // den in [1, 1 + sum w_i^2]: the 2-ulp approximate division is safe
 }
 
 // Exact projection of one foot wrench (f, m) onto W; writes the projected 6 values.
