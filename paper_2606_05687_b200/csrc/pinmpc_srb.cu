@@ -845,19 +845,20 @@ __device__ __forceinline__ void stage_update(const SolveParams &P, const SrbWs &
                 v0[a] = uf[0][a] + S.y[a < 3 ? fcol(0) + a : mcol(0) + a - 3];
                 v1[a] = uf[1][a] + S.y[a < 3 ? fcol(1) + a : mcol(1) + a - 3];
             }
-            if (two_feet) {                                 // warp-uniform
-                project_wrench(P, v0[0], v0[1], v0[2], v0[3], v0[4], v0[5], zf[0][0], zf[0][1], zf[0][2], zf[0][3], zf[0][4], zf[0][5]);
-                project_wrench(P, v1[0], v1[1], v1[2], v1[3], v1[4], v1[5], zf[1][0], zf[1][1], zf[1][2], zf[1][3], zf[1][4], zf[1][5]);
+            // one projection of the selected foot (foot 1 if it is in stance, else foot 0) and, only when some thread
+            // of the warp has both feet in stance (warp-uniform), a second one of foot 0: two inlined copies, not three
+            const bool sel = on1;
+            float vs[6], zs[6];
 #pragma unroll
-                for (int a = 0; a < 6; a++) { zf[0][a] = on0 ? zf[0][a] : 0.0f; zf[1][a] = on1 ? zf[1][a] : 0.0f; }
-            } else {
-                const bool sel = on1;                       // at most one foot is on
-                float vs[6], zs[6];
+            for (int a = 0; a < 6; a++) vs[a] = sel ? v1[a] : v0[a];
+            project_wrench(P, vs[0], vs[1], vs[2], vs[3], vs[4], vs[5], zs[0], zs[1], zs[2], zs[3], zs[4], zs[5]);
 #pragma unroll
-                for (int a = 0; a < 6; a++) vs[a] = sel ? v1[a] : v0[a];
-                project_wrench(P, vs[0], vs[1], vs[2], vs[3], vs[4], vs[5], zs[0], zs[1], zs[2], zs[3], zs[4], zs[5]);
+            for (int a = 0; a < 6; a++) { zf[1][a] = on1 ? zs[a] : 0.0f; zf[0][a] = (on0 && !on1) ? zs[a] : 0.0f; }
+            if (two_feet) {
+                float z0p[6];
+                project_wrench(P, v0[0], v0[1], v0[2], v0[3], v0[4], v0[5], z0p[0], z0p[1], z0p[2], z0p[3], z0p[4], z0p[5]);
 #pragma unroll
-                for (int a = 0; a < 6; a++) { zf[0][a] = on0 ? zs[a] : 0.0f; zf[1][a] = on1 ? zs[a] : 0.0f; }
+                for (int a = 0; a < 6; a++) zf[0][a] = on0 ? z0p[a] : 0.0f;
             }
         }
 #pragma unroll
