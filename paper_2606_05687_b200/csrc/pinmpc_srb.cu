@@ -370,9 +370,11 @@ __global__ void __launch_bounds__(FAC_WARPS * 32, 7) k_factor_srb(SolveParams P,
     float cs_n = W.cs[s * 2], sn_n = W.cs[s * 2 + 1];
     float S_n = W.MI[(long)(lane < 21 ? lane : 0) * st + s];
     float ch_n = (has_ext && lane < 6) ? W.c6[s * 6 + lane] : 0.0f;
+    float q_n = N >= 2 ? W.qv[((long)b * (N + 1) + N - 1) * 12 + jl] : 0.0f;      // q_k of the stage being processed
     for (int k = N - 1; k >= 0; k--) {
         s = (long)b * N + k;
-        const float cs = cs_n, sn = sn_n, Sl = S_n, chl = ch_n;
+        const float cs = cs_n, sn = sn_n, Sl = S_n, chl = ch_n, qk12 = k >= 1 ? q_n : 0.0f;
+        if (k > 1) q_n = W.qv[((long)b * (N + 1) + k - 1) * 12 + jl];
         if (k > 0) {
             cs_n = W.cs[(s - 1) * 2]; sn_n = W.cs[(s - 1) * 2 + 1];
             S_n = W.MI[(long)(lane < 21 ? lane : 0) * st + s - 1];
@@ -461,7 +463,7 @@ __global__ void __launch_bounds__(FAC_WARPS * 32, 7) k_factor_srb(SolveParams P,
             if (lane == 6) atg = fmaf(dt, cs * g_lo - sn * g_nb, g);
             else if (lane == 7) atg = fmaf(dt, cs * g_lo + sn * g_nb, g);
             else if (lane >= 8 && lane < 12) atg = fmaf(dt, g_lo, g);
-            pc = (k >= 1 ? W.qv[((long)b * (N + 1) + k) * 12 + jl] : 0.0f) + atg - acc;
+            pc = qk12 + atg - acc;
         }
         // ---- P <- [k>=1] Q + A^T X - G^T Kh, row `row`, four columns at a time
         {
