@@ -109,9 +109,24 @@ pinmpc_status pinmpc_set_warm_start(pinmpc_t h, const float *d_z0, const float *
 /* Force a solver variant (default PINMPC_METHOD_AUTO). */
 pinmpc_status pinmpc_set_method(pinmpc_t h, pinmpc_method m);
 
-/* Tuning knob of the structured solver: envs solved per thread block (1..16; 0 = choose by the
- * occupancy heuristic of DESIGN.md "Kernels").  Results do not depend on it. */
+/* Tuning knob of the structured solver: envs solved per thread block (1..32; 0 = choose by the
+ * occupancy heuristic of DESIGN.md "Kernels"; a value the kernel in use cannot hold falls back to
+ * that heuristic).  Results do not depend on it. */
 pinmpc_status pinmpc_set_tuning(pinmpc_t h, int envs_per_cta);
+
+/* How the equality step (S3) is parallelised across the horizon (north_star (2); PAPER.md:L206-208 Remark 2,
+ * L23): the N stages are cut into `chunks` chunks that are swept concurrently (chunked two-sweep over the
+ * time-varying LQR recursion, gains resident in tensor memory).
+ *   0 (default) = ceil(N / 6) chunks when the shape fits the chunked kernel, else sequential passes;
+ *   1           = the sequential-pass kernel (two N-step recursions per iteration);
+ *   >= 2        = that many chunks; PINMPC_EUNSUPPORTED unless ceil(N / chunks) <= 6, chunks <= 128 and
+ *                 chunks <= ceil(N / 4) (room for the chunk operators in the workspace).
+ * Results agree to rounding for every setting. */
+pinmpc_status pinmpc_set_horizon_chunks(pinmpc_t h, int chunks);
+
+/* Launch shape the last pinmpc_solve of the structured solver used: envs per thread block and horizon
+ * chunks (1 = sequential passes).  Either pointer may be NULL.  PINMPC_ESTATE before the first solve. */
+pinmpc_status pinmpc_get_launch_shape(pinmpc_t h, int *h_envs_per_cta, int *h_chunks);
 
 /* Per-env problem data, all DEVICE pointers ("{A_k,B_k,e_k} are obtained along the
  * input periodic contact sequence" — here from these raw inputs, on the device, every solve). */

@@ -22,7 +22,7 @@ _STATUS = {0: "PINMPC_OK", 1: "PINMPC_EINVAL", 2: "PINMPC_EALLOC", 3: "PINMPC_EC
            5: "PINMPC_EUNSUPPORTED"}
 
 EXPORTS = ("pinmpc_workspace_bytes", "pinmpc_workspace_bytes_method", "pinmpc_create", "pinmpc_set_weights",
-           "pinmpc_set_tolerance", "pinmpc_set_method", "pinmpc_set_tuning", "pinmpc_set_problem", "pinmpc_set_dynamics", "pinmpc_solve",
+           "pinmpc_set_tolerance", "pinmpc_set_method", "pinmpc_set_tuning", "pinmpc_set_horizon_chunks", "pinmpc_get_launch_shape", "pinmpc_set_problem", "pinmpc_set_dynamics", "pinmpc_solve",
            "pinmpc_get", "pinmpc_get_aux", "pinmpc_get_dynamics", "pinmpc_last_launch_count", "pinmpc_last_error",
            "pinmpc_destroy", "pinmpc_probe_fma", "pinmpc_set_profiling", "pinmpc_get_kernel_ms",
            "pinmpc_set_warm_start", "pinmpc_shift_aux", "pinmpc_landmark_ring_bytes", "pinmpc_landmark_reset", "pinmpc_landmark_push",
@@ -82,6 +82,10 @@ def load():
     lib.pinmpc_set_method.argtypes = [c_void_p, c_int]
     lib.pinmpc_set_tuning.restype = c_int
     lib.pinmpc_set_tuning.argtypes = [c_void_p, c_int]
+    lib.pinmpc_set_horizon_chunks.restype = c_int
+    lib.pinmpc_set_horizon_chunks.argtypes = [c_void_p, c_int]
+    lib.pinmpc_get_launch_shape.restype = c_int
+    lib.pinmpc_get_launch_shape.argtypes = [c_void_p, POINTER(c_int), POINTER(c_int)]
     lib.pinmpc_set_problem.restype = c_int
     lib.pinmpc_set_problem.argtypes = [c_void_p, POINTER(Problem)]
     lib.pinmpc_set_dynamics.restype = c_int
@@ -175,6 +179,16 @@ def pinmpc_set_method(h, method):
 
 def pinmpc_set_tuning(h, envs_per_cta):
     _check(load().pinmpc_set_tuning(h, int(envs_per_cta)), h)
+
+
+def pinmpc_set_horizon_chunks(h, chunks):
+    _check(load().pinmpc_set_horizon_chunks(h, int(chunks)), h)
+
+
+def pinmpc_get_launch_shape(h):
+    g, c = c_int(0), c_int(0)
+    _check(load().pinmpc_get_launch_shape(h, ctypes.byref(g), ctypes.byref(c)), h)
+    return int(g.value), int(c.value)
 
 
 def pinmpc_set_problem(h, x0, x_ref, u_ref, contact, foot_r, yaw, mass, inertia, ext_wrench=None):
@@ -304,6 +318,12 @@ class Solver:
 
     def set_tuning(self, envs_per_cta):
         pinmpc_set_tuning(self.h, envs_per_cta)
+
+    def set_horizon_chunks(self, chunks):
+        pinmpc_set_horizon_chunks(self.h, chunks)
+
+    def launch_shape(self):
+        return pinmpc_get_launch_shape(self.h)
 
     def set_warm_start(self, z0=None, y0=None):
         """Start the next solves from z0, y0 [B,N,nu] (None, None: cold start)."""

@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpinmpc.so")
-SOURCES = ["pinmpc_api.cu", "pinmpc_dense.cu", "pinmpc_srb.cu", "pinmpc_probe.cu", "pinmpc_landmarks.cu", "pinmpc_split.cu"]
+SOURCES = ["pinmpc_api.cu", "pinmpc_dense.cu", "pinmpc_srb.cu", "pinmpc_tmem.cu", "pinmpc_probe.cu", "pinmpc_landmarks.cu", "pinmpc_split.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"] + os.environ.get("PINMPC_NVCC_EXTRA", "").split()
 

@@ -17,12 +17,13 @@ size_t pinmpc_ws_base_bytes(int nu, int N, int B)
 }
 
 // structured-solver factors (SrbWs)
-static const int SRB_NARR = 7;
+static const int SRB_NARR = 8;
 static void srb_sizes(int nu, int N, int B, size_t *f)
 {
     size_t st = (size_t)B * N;
     f[0] = st * 72; f[1] = (size_t)B * (N + 1) * 12; f[2] = st * 6; f[3] = st * 2; f[4] = st * 21;
     f[5] = st * PINMPC_RA_W; f[6] = st * (size_t)pinmpc_rb_width(nu);
+    f[7] = (size_t)B * pinmpc_psi_cap(N) * 144;
 }
 
 size_t pinmpc_ws_srb_bytes(int nu, int N, int B)
@@ -128,6 +129,7 @@ extern "C" pinmpc_status pinmpc_create(pinmpc_t *out, int nx, int nu, int N, int
         h->srb.Kh = (float *)take(f[0] * 4); h->srb.qv = (float *)take(f[1] * 4); h->srb.c6 = (float *)take(f[2] * 4);
         h->srb.cs = (float *)take(f[3] * 4); h->srb.MI = (float *)take(f[4] * 4);
         h->srb.RA = (float *)take(f[5] * 4); h->srb.RB = (float *)take(f[6] * 4);
+        h->psi = (float *)take(f[7] * 4); h->psi_cap = pinmpc_psi_cap(N);
     }
     if (workspace_bytes >= pinmpc_ws_dense_bytes(nu, N, B)) {
         h->dA = (float *)take(st * NX * NX * 4);
@@ -183,8 +185,32 @@ extern "C" pinmpc_status pinmpc_set_method(pinmpc_t h, pinmpc_method m)
 extern "C" pinmpc_status pinmpc_set_tuning(pinmpc_t h, int envs_per_cta)
 {
     if (!h) return PINMPC_EINVAL;
-    if (envs_per_cta < 0 || envs_per_cta > 16) return set_err(h, PINMPC_EINVAL, "pinmpc_set_tuning: envs_per_cta must be 0 (auto) .. 16");
+    if (envs_per_cta < 0 || envs_per_cta > 32) return set_err(h, PINMPC_EINVAL, "pinmpc_set_tuning: envs_per_cta must be 0 (auto) .. 32");
     h->envs_per_cta = envs_per_cta;
+    return PINMPC_OK;
+}
+
+extern "C" pinmpc_status pinmpc_set_horizon_chunks(pinmpc_t h, int chunks)
+{
+    if (!h) return PINMPC_EINVAL;
+    if (chunks < 0 || chunks > h->N) return set_err(h, PINMPC_EINVAL, "pinmpc_set_horizon_chunks: chunks must be 0 (auto), 1 (sequential) .. N");
+    if (chunks > 1) {
+        pinmpc_ctx t = *h;
+        t.chunks = chunks; t.envs_per_cta = 0;
+        int G, C;
+        if (!pinmpc_tm_config(&t, &G, &C))
+            return set_err(h, PINMPC_EUNSUPPORTED, "pinmpc_set_horizon_chunks: needs ceil(N / chunks) <= 6, chunks <= 128 and chunks - 2 <= ceil(N / 4) - 2");
+    }
+    h->chunks = chunks;
+    return PINMPC_OK;
+}
+
+extern "C" pinmpc_status pinmpc_get_launch_shape(pinmpc_t h, int *envs_per_cta, int *chunks)
+{
+    if (!h) return PINMPC_EINVAL;
+    if (!h->solved) return set_err(h, PINMPC_ESTATE, "pinmpc_get_launch_shape: no solve has been enqueued");
+    if (envs_per_cta) *envs_per_cta = h->last_G;
+    if (chunks) *chunks = h->last_C;
     return PINMPC_OK;
 }
 

@@ -83,6 +83,10 @@ struct pinmpc_ctx {
     float *dA, *dB, *dC, *dK, *dMinv, *dS, *dKappa;   // dense-only (NULL when the workspace is the small one)
     SrbWs srb;
     int envs_per_cta;        // tuning knob of the structured solver (0 = auto)
+    int chunks;              // horizon chunks of the equality step: 0 = auto, 1 = sequential passes, >= 2 forced
+    int psi_cap;             // chunk operators per env the workspace has room for
+    float *psi;              // [B][C-2][12][12] chunk operators of the chunked (TMEM) iteration kernel
+    int last_G, last_C;      // launch shape of the last structured solve (last_C = 1: sequential passes)
     int sm_count, smem_optin;
     int launch_count;
     int profiling;           // record events around the kernels of the structured solver
@@ -100,6 +104,10 @@ int pinmpc_launch_assemble_dense(pinmpc_ctx *h, float *A, float *Bm, float *c, c
 int pinmpc_launch_solve_dense(pinmpc_ctx *h, cudaStream_t st);
 int pinmpc_launch_solve_srb(pinmpc_ctx *h, cudaStream_t st);
 size_t pinmpc_ws_srb_bytes(int nu, int N, int B);
+// chunked, TMEM-resident iteration kernel (pinmpc_tmem.cu)
+bool pinmpc_tm_config(const pinmpc_ctx *h, int *G, int *C);
+int pinmpc_launch_iterate_tm(pinmpc_ctx *h, int G, int C, cudaStream_t st);
+inline int pinmpc_psi_cap(int N) { int c = (N + 3) / 4 - 2; return c > 0 ? c : 0; }
 
 static inline SolveParams make_params(const pinmpc_ctx *h)
 {

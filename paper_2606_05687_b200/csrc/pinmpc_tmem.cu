@@ -1,0 +1,930 @@
+// pinmpc_tmem.cu — the equality step solved IN PARALLEL ACROSS THE HORIZON (north_star (2)
+// Remark 2, L23: "horizon-wise recursions" are the bottleneck of GPU MPC), with the gains resident in Blackwell
+// TENSOR MEMORY.
+//
+// The exact LQR step of pinmpc_srb.cu (same formulation, same factors Kh, Mh^-1, kg from k_factor_srb) is a pair
+// of affine recursions in the 12-D (Theta, p, omega, v) state,
+//     forward   x+ = Phi_k x + E (kappa_k + c_k),           Phi_k = [[I, dt Rot_k], [Kn_a, I + Kn_b]],  Kn = -Kh_k
+//     backward  p  <- Phi_k^T p + Kn^T sigma0_k
+// The horizon is cut into C chunks of L <= 6 stages.  Each pass is a chunked TWO-SWEEP:
+//     sweep A   every chunk concurrently from a zero boundary vector (chunk 0 forward from x_0, the last chunk
+//               backward from the zero terminal costate): gives the chunk's affine offset d_c / b_c
+//     boundary  x_{k_{c+1}} = Psi_c x_{k_c} + d_c  (backward: p_{k_c} = Psi_c^T p_{k_{c+1}} + b_c), C - 2 dependent
+//               12 x 12 steps with the chunk operators Psi_c = Phi_{k_c + L - 1} ... Phi_{k_c} formed once per
+//               solve by k_chunk_ops
+//     sweep B   every chunk concurrently from its true boundary vector, producing hh -> kappa (backward) and
+//               w, x (forward)
+// so the dependent depth of a pass drops from N to 2 L + C - 2 (50 -> 19 at N = 50, C = 9).
+//
+// One CHAIN THREAD per (env, chunk) runs a sweep step alone: 72 FMAs, no shuffles, no shared-memory exchange.
+// Its operands, the 72 gains of every stage of its chunk, live in ITS lane of tensor memory (tcgen05.ld
+// 32x32b: thread t of warp w reads lane 32 (w % 4) + t; 6 x 72 = 432 of the 512 columns) next to the 6-D
+// exchange vector of every stage (sigma0 -> kappa -> w) and the external-wrench offsets.  TMEM is the only
+// on-chip store that is both large enough for 14 envs x 50 stages x 72 words (256 KB per SM next to 227 KB of
+// shared memory) and fast enough for one-use operands (measured 64 B/clk per sub-partition = 2 x the shared-memory
+// pipe of the whole SM); a sweep step is bound by that read rate (144 cycles).  The three WORKER
+// threads that share a chain's TMEM lane (warps 4+q, 8+q, 12+q for chain warp q) own two stages of the chunk
+// each: u from w, the exact projection (S4), the dual update (S5), residuals (S6) and sigma0 of the next
+// iteration, with the stage constants (Mh^-1, kg, T^-1, I_w, r, R ubar) in shared memory — nothing streams from
+// L2 after the prologue.
+#include "pinmpc_srb_math.cuh"
+
+namespace {
+
+#ifndef TM_ABL
+#define TM_ABL 0
+#endif
+
+constexpr int TM_LMAX = 6;                         // stages per chunk
+constexpr int TM_XOFF = TM_LMAX * 72;              // exchange vectors   [LMAX][6]   columns 432..467
+constexpr int TM_COFF = TM_XOFF + TM_LMAX * 6;     // ch (ext only)      [LMAX][6]   columns 468..503
+constexpr int TM_CHAINS = 128;                     // chain threads = TMEM lanes
+constexpr int TM_THREADS = 384;                    // 4 chain warps + 8 worker warps (168 registers per thread)
+constexpr int TM_GMAX = 32;                        // envs per CTA
+constexpr int TM_RAW = 28;                         // Mh^-1 (21) | kg (6) | contact bits
+constexpr int TM_CTL = 48 + 5 * TM_GMAX;           // done[32] | ndone | pad[15] | red[32][5]
+constexpr unsigned BMASK = 0x00ffffffu;            // the 24 boundary lanes of a worker warp
+
+__host__ __device__ constexpr int tm_rbw(int nu) { return 12 + 3 * (2 + (nu - 12) / 3) + nu + 2; }   // T^-1 | I_w | r | R ubar' | cos sin
+
+// shared-memory layout (offsets in floats)
+struct TmLay { int oA, oB, oPsi, oBnd, oCtl, total; };
+__host__ __device__ inline TmLay tm_layout(int N, int G, int C, int nu)
+{
+    TmLay L;
+    const int st = G * N;
+    L.oA = 0;
+    L.oB = L.oA + TM_RAW * st;
+    L.oPsi = L.oB + tm_rbw(nu) * st;
+    L.oBnd = L.oPsi + G * (C > 2 ? C - 2 : 0) * 144;
+    L.oCtl = L.oBnd + G * (C + 1) * 12;
+    L.total = L.oCtl + TM_CTL;
+    return L;
+}
+
+// ---- tensor memory ------------------------------------------------------------------------------------------
+__device__ __forceinline__ void tm_ld8(uint32_t a, float *r)
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=f"(r[0]), "=f"(r[1]), "=f"(r[2]), "=f"(r[3]), "=f"(r[4]), "=f"(r[5]), "=f"(r[6]), "=f"(r[7]) : "r"(a));
+}
+__device__ __forceinline__ void tm_ld6(uint32_t a, float *r)
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];" : "=f"(r[0]), "=f"(r[1]), "=f"(r[2]), "=f"(r[3]) : "r"(a));
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0,%1}, [%2];" : "=f"(r[4]), "=f"(r[5]) : "r"(a + 4));
+}
+__device__ __forceinline__ void tm_st8(uint32_t a, const float *r)
+{
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
+                 :: "r"(a), "f"(r[0]), "f"(r[1]), "f"(r[2]), "f"(r[3]), "f"(r[4]), "f"(r[5]), "f"(r[6]), "f"(r[7]) : "memory");
+}
+__device__ __forceinline__ void tm_st6(uint32_t a, const float *r)
+{
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1,%2,%3,%4};" :: "r"(a), "f"(r[0]), "f"(r[1]), "f"(r[2]), "f"(r[3]) : "memory");
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1,%2};" :: "r"(a + 4), "f"(r[4]), "f"(r[5]) : "memory");
+}
+__device__ __forceinline__ void tm_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tm_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+// CTA barrier that also orders tensor-memory stores of one thread before the loads of another
+__device__ __forceinline__ void tm_sync()
+{
+    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+}
+
+// chunk c of C over N stages: the first N % C chunks hold one stage more
+__host__ __device__ inline void tm_chunk(int N, int C, int c, int &k0, int &len)
+{
+    const int base = N / C, rem = N - base * C;
+    k0 = c * base + (c < rem ? c : rem);
+    len = base + (c < rem ? 1 : 0);
+}
+
+// ---------------------------------------------------------------------------------------------
+// chunk operators Psi_c = Phi_{k0+len-1} ... Phi_{k0} for the inner chunks c = 1 .. C-2, once per solve.
+// One thread per (env, chunk, row): row <- row Phi_k from the last stage of the chunk to the first.
+//   (row Phi)_a = row_a + row_b Kn_a ;  (row Phi)_b = dt row_a Rot + row_b + row_b Kn_b
+// Psi [B][C-2][12][12] row-major.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(192) k_chunk_ops(int B, int N, int C, float dt, const float *__restrict__ Kh, const float *__restrict__ cs,
+                                                   float *__restrict__ Psi)
+{
+    const long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long rows = (long)B * (C - 2) * 12;
+    if (t >= rows) return;
+    const int i = (int)(t % 12);
+    const long bc = t / 12;
+    const int c = (int)(bc % (C - 2)) + 1, b = (int)(bc / (C - 2));
+    int k0, len;
+    tm_chunk(N, C, c, k0, len);
+    float ra[6], rb[6];
+#pragma unroll
+    for (int j = 0; j < 6; j++) { ra[j] = (i == j) ? 1.0f : 0.0f; rb[j] = (i == 6 + j) ? 1.0f : 0.0f; }
+    for (int k = k0 + len - 1; k >= k0; k--) {
+        const long s = (long)b * N + k;
+        const float4 *kp = reinterpret_cast<const float4 *>(Kh + s * 72);
+        const float co = cs[s * 2], sn = cs[s * 2 + 1];
+        float na[6], nb[6];
+        // dt row_a Rot:  Rot = [[c, s], [-s, c]] (+) I_4   (Theta+ = Theta + dt R_z^T omega, p+ = p + dt v)
+        nb[0] = fmaf(dt, co * ra[0] - sn * ra[1], rb[0]);
+        nb[1] = fmaf(dt, sn * ra[0] + co * ra[1], rb[1]);
+#pragma unroll
+        for (int j = 2; j < 6; j++) nb[j] = fmaf(dt, ra[j], rb[j]);
+#pragma unroll
+        for (int j = 0; j < 6; j++) na[j] = ra[j];
+#pragma unroll
+        for (int r = 0; r < 6; r++) {
+            // Kh row r as pairs (Kh[r][j], Kh[r][6+j]);  Kn = -Kh
+            const float4 v0 = __ldg(kp + 3 * r), v1 = __ldg(kp + 3 * r + 1), v2 = __ldg(kp + 3 * r + 2);
+            const float m = -rb[r];
+            na[0] = fmaf(m, v0.x, na[0]); nb[0] = fmaf(m, v0.y, nb[0]); na[1] = fmaf(m, v0.z, na[1]); nb[1] = fmaf(m, v0.w, nb[1]);
+            na[2] = fmaf(m, v1.x, na[2]); nb[2] = fmaf(m, v1.y, nb[2]); na[3] = fmaf(m, v1.z, na[3]); nb[3] = fmaf(m, v1.w, nb[3]);
+            na[4] = fmaf(m, v2.x, na[4]); nb[4] = fmaf(m, v2.y, nb[4]); na[5] = fmaf(m, v2.z, na[5]); nb[5] = fmaf(m, v2.w, nb[5]);
+        }
+#pragma unroll
+        for (int j = 0; j < 6; j++) { ra[j] = na[j]; rb[j] = nb[j]; }
+    }
+    float *o = Psi + t * 12;
+#pragma unroll
+    for (int j = 0; j < 6; j++) { o[j] = ra[j]; o[6 + j] = rb[j]; }
+}
+
+// ---------------------------------------------------------------------------------------------
+// chain sweeps (one thread = one chunk of one env).  A sweep is software-pipelined over half stages: while
+// the 36 gains of one half (three rows of Kn) are consumed, the other half is in flight from tensor memory
+// (tcgen05.wait::ld waits for everything outstanding, so exactly one batch is outstanding at a time).
+// ---------------------------------------------------------------------------------------------
+struct Chain {
+    uint32_t tk;          // TMEM address of the chunk's gains (stage j at + 72 j)
+    uint32_t sA, sCS;     // shared-memory byte addresses: RA record / (cos, sin) of the chunk's stage 0 (this chain's slot)
+    uint32_t jstride;     // bytes from stage j to stage j + 1 of the chunk (slots are stage-major: all chains' stage j together)
+    uint32_t xoff;        // extra bytes for the chunk's last stage when it is the one extra stage (compacted slots)
+    uint32_t wstride;     // bytes between consecutive float4 groups of a record
+    int len;              // stages in the chunk (<= TM_LMAX)
+    int nsteps;           // steps of a sweep (warp-uniform): the longest chunk of the CTA
+    int base;             // stages every chunk has
+};
+__device__ __forceinline__ uint32_t chain_joff(const Chain &ch, int j) { return (uint32_t)j * ch.jstride + (j >= ch.base ? ch.xoff : 0u); }
+
+__device__ __forceinline__ float2 lds_f2(uint32_t a)
+{
+    float2 v;
+    asm volatile("ld.shared.v2.f32 {%0,%1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ float4 lds_f4(uint32_t a)
+{
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a));
+    return v;
+}
+
+// all 72 gains of stage j of the chunk, row-major Kn[r][0..11]
+__device__ __forceinline__ void chain_ld_stage(uint32_t tk, int j, float *k)
+{
+    const uint32_t a = tk + 72 * j;
+#pragma unroll
+    for (int q = 0; q < 9; q++) tm_ld8(a + 8 * q, k + 8 * q);
+}
+
+// A chunk shorter than the sweep (nsteps) has zero gains, zero exchange vectors and dt, g dt switched off in its unused
+// steps, which makes those steps the identity.  Within a step the 72 gains are requested at once and consumed row
+// by row as they arrive (the hardware scoreboard tracks every tcgen05.ld destination).
+
+// Backward sweep over the chunk, stages nsteps-1 .. 0:  hh = sigma0 + pv ;  p <- Phi^T p + Kn^T sigma0.
+// OUT: kappa = Mh^-1 hh - kg replaces sigma0 in the exchange vector of every stage (computed while the gains stream in;
+// an unused step keeps its zero).
+template <bool OUT, int RBW>
+__device__ __forceinline__ void chain_bwd_sweep(const Chain &ch, float dt, float *pq, float *pv)
+{
+    for (int j = ch.nsteps - 1; j >= 0; j--) {
+        float k[72], s0[6];
+        tm_ld6(ch.tk + TM_XOFF + 6 * j, s0);
+        chain_ld_stage(ch.tk, j, k);
+        const bool act = j < ch.len;
+        const float dte = act ? dt : 0.0f;
+        const float2 cs = lds_f2(ch.sCS + chain_joff(ch, j));
+        float Mi[28];
+        if (OUT) {
+            const uint32_t a = ch.sA + chain_joff(ch, j);
+#pragma unroll
+            for (int c = 0; c < 7; c++) {
+                const float4 q = lds_f4(a + c * ch.wstride);
+                Mi[4 * c] = q.x; Mi[4 * c + 1] = q.y; Mi[4 * c + 2] = q.z; Mi[4 * c + 3] = q.w;
+            }
+        }
+        tm_wait_ld();
+        float hh[6];
+#pragma unroll
+        for (int r = 0; r < 6; r++) hh[r] = s0[r] + pv[r];
+        if (OUT) {
+            float kp[6];
+            symv6(Mi, hh, kp);
+#pragma unroll
+            for (int r = 0; r < 6; r++) kp[r] = act ? kp[r] - Mi[21 + r] : 0.0f;
+            tm_st6(ch.tk + TM_XOFF + 6 * j, kp);
+        }
+        // (A^T p)_v = pv + dt Rot^T pq  (old pq)
+        {
+            const float t0 = cs.x * pq[0] - cs.y * pq[1], t1 = cs.x * pq[1] + cs.y * pq[0];
+            pv[0] = fmaf(dte, t0, pv[0]); pv[1] = fmaf(dte, t1, pv[1]);
+#pragma unroll
+            for (int i = 2; i < 6; i++) pv[i] = fmaf(dte, pq[i], pv[i]);
+        }
+#pragma unroll
+        for (int r = 0; r < 6; r++)
+#pragma unroll
+            for (int i = 0; i < 6; i++) {
+                pq[i] = fmaf(k[12 * r + i], hh[r], pq[i]);
+                pv[i] = fmaf(k[12 * r + 6 + i], hh[r], pv[i]);
+            }
+    }
+}
+
+// kappa = Mh^-1 hh - kg for every stage of the chunk (hh -> kappa in the exchange vectors; unused steps stay zero)
+__device__ __forceinline__ void chain_kappa(const Chain &ch)
+{
+    tm_wait_st();
+    for (int j = 0; j < ch.nsteps; j++) {
+        float hh[6], Mi[28], kp[6];
+        tm_ld6(ch.tk + TM_XOFF + 6 * j, hh);
+        const uint32_t a = ch.sA + chain_joff(ch, j);
+#pragma unroll
+        for (int c = 0; c < 7; c++) {
+            const float4 q = lds_f4(a + c * ch.wstride);
+            Mi[4 * c] = q.x; Mi[4 * c + 1] = q.y; Mi[4 * c + 2] = q.z; Mi[4 * c + 3] = q.w;
+        }
+        tm_wait_ld();
+        symv6(Mi, hh, kp);
+        const bool act = j < ch.len;
+#pragma unroll
+        for (int r = 0; r < 6; r++) kp[r] = act ? kp[r] - Mi[21 + r] : 0.0f;
+        tm_st6(ch.tk + TM_XOFF + 6 * j, kp);
+    }
+    tm_wait_st();
+}
+
+// Forward sweep over the chunk, stages 0 .. nsteps-1:  w = kappa + Kn x ;  x+ = A x + E (w + c).
+// OUT: w replaces kappa in the exchange vector; EMIT (with OUT): x+ -> ox (x_{k+1} of the output).
+template <bool OUT, bool EMIT, int RBW>
+__device__ __forceinline__ void chain_fwd_sweep(const Chain &ch, float dt, float gdt, float x12, int has_ext, float *xa, float *xb, bool wr, float *ox)
+{
+    for (int j = 0; j < ch.nsteps; j++) {
+        float k[72], w[6], cv[6];
+#pragma unroll
+        for (int i = 0; i < 6; i++) cv[i] = 0.0f;
+        tm_ld6(ch.tk + TM_XOFF + 6 * j, w);
+        if (has_ext) tm_ld6(ch.tk + TM_COFF + 6 * j, cv);
+        chain_ld_stage(ch.tk, j, k);
+        const bool act = j < ch.len;
+        const float dte = act ? dt : 0.0f, gdte = act ? gdt : 0.0f;
+        const float2 cs = lds_f2(ch.sCS + chain_joff(ch, j));
+        tm_wait_ld();
+#pragma unroll
+        for (int r = 0; r < 6; r++) {
+            float a = w[r], b = 0.0f;
+#pragma unroll
+            for (int i = 0; i < 6; i++) { a = fmaf(k[12 * r + i], xa[i], a); b = fmaf(k[12 * r + 6 + i], xb[i], b); }
+            w[r] = a + b;
+        }
+        if (OUT) tm_st6(ch.tk + TM_XOFF + 6 * j, w);
+        // x_a+ = x_a + dt Rot x_b (old x_b);  x_b+ = x_b + w + c
+        {
+            const float t0 = fmaf(cs.x, xb[0], cs.y * xb[1]), t1 = fmaf(cs.x, xb[1], -cs.y * xb[0]);
+            xa[0] = fmaf(dte, t0, xa[0]); xa[1] = fmaf(dte, t1, xa[1]);
+#pragma unroll
+            for (int i = 2; i < 6; i++) xa[i] = fmaf(dte, xb[i], xa[i]);
+        }
+#pragma unroll
+        for (int i = 0; i < 6; i++) xb[i] += w[i] + cv[i];
+        xb[5] += gdte;
+        if (OUT && EMIT && wr && act) {
+            float *o = ox + j * NX;
+#pragma unroll
+            for (int i = 0; i < 6; i++) { o[i] = xa[i]; o[6 + i] = xb[i]; }
+            o[12] = x12;
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// stage work of a worker thread (one stage at a time).  Stage records live in shared memory as float4 groups,
+// group-major over SLOTS (rec[group][slot], slot = the stage's position in lane order), so that the 32 lanes of a
+// warp read consecutive float4s (conflict-free LDS.128).  RB record (words): T^-1 (6) | I_w (6) | r (3 nc) |
+// R ubar' (nu) | cos sin.  The groups are (re)loaded phase by phase, so that next to z, y of the owned stages only a
+// few dozen registers are live.
+// ---------------------------------------------------------------------------------------------
+template <int NU> struct TmState { float z[NU], y[NU]; };
+
+#define TM_PHASE() asm volatile("" ::: "memory")
+
+// float4 groups [G0, G1) of a record -> v (v[0] = word 4 G0)
+template <int G0, int G1>
+__device__ __forceinline__ void tm_ld_groups(const float4 *rec, int nsl, float *v)
+{
+#pragma unroll
+    for (int g = G0; g < G1; g++) {
+        const float4 q = rec[g * nsl];
+        v[4 * (g - G0)] = q.x; v[4 * (g - G0) + 1] = q.y; v[4 * (g - G0) + 2] = q.z; v[4 * (g - G0) + 3] = q.w;
+    }
+}
+
+// G = Gh u0,  u0 = Rt^-1 (R ubar + rho (z - y));  v = the record from word 12 on (r | R ubar')
+template <int NU>
+__device__ __forceinline__ void tm_gh_u0(const SolveParams &P, const float *v, const float *z, const float *y, float *G)
+{
+    constexpr int NC = NW + (NU - 12) / 3;
+    const float *rr = v, *ru = v + 3 * NC;
+#pragma unroll
+    for (int a = 0; a < 6; a++) G[a] = 0.0f;
+#pragma unroll
+    for (int i = 0; i < NC; i++) {
+        const int fc = fcol(i);
+        const float rx = rr[3 * i], ry = rr[3 * i + 1], rz = rr[3 * i + 2];
+        float f[3];
+#pragma unroll
+        for (int a = 0; a < 3; a++) f[a] = fmaf(P.rtR[fc + a], z[fc + a] - y[fc + a], ru[fc + a]);
+        G[0] = fmaf(ry, f[2], fmaf(-rz, f[1], G[0]));
+        G[1] = fmaf(rz, f[0], fmaf(-rx, f[2], G[1]));
+        G[2] = fmaf(rx, f[1], fmaf(-ry, f[0], G[2]));
+        G[3] += f[0]; G[4] += f[1]; G[5] += f[2];
+        if (i < NW) {
+            const int mc = mcol(i);
+#pragma unroll
+            for (int a = 0; a < 3; a++) G[a] += fmaf(P.rtR[mc + a], z[mc + a] - y[mc + a], ru[mc + a]);
+        }
+    }
+}
+
+// sigma0 = D^-1 Lam^-1 G;  geo = the record's words 0 .. 12 + 3 nc (T^-1 | I_w | r)
+template <int NU>
+__device__ __forceinline__ void tm_sigma0(const SolveParams &P, const float *geo, const float *G, float idt, float m_dt, float *s0)
+{
+    float l0[6];
+    lam_inv_apply<NU>(P, geo, geo + 12, G, l0);
+    dinv_apply(geo + 6, idt, m_dt, l0, s0);
+}
+
+// u from w, projection (S4), dual update (S5), residuals (S6); then sigma0 of the next iteration.
+// wv: in w of this stage, out sigma0 of the next iteration.  res = running maxima (r_prim, |dz|, |u|, |z|, |y|).
+template <int NU, bool EMIT>
+__device__ __forceinline__ void tm_stage_update(const SolveParams &P, const float4 *rb, int nsl, int bits, float *z, float *y, float idt, float m_dt,
+                                                float *wv, bool update, float *ou, float *res, bool two_feet)
+{
+    constexpr int NC = NW + (NU - 12) / 3, RBW = tm_rbw(NU);
+    constexpr int GEO4 = (12 + 3 * NC + 3) / 4;                 // groups holding T^-1, I_w, r
+    float G0[6];
+    {
+        float v[RBW - 12];
+        tm_ld_groups<3, RBW / 4>(rb, nsl, v);
+        tm_gh_u0<NU>(P, v, z, y, G0);
+    }
+    TM_PHASE();
+    if (update) {
+        float lam[6];
+        {
+            float geo[4 * GEO4], dl[6];
+            tm_ld_groups<0, GEO4>(rb, nsl, geo);
+            dinv_apply(geo + 6, idt, m_dt, wv, dl);
+#pragma unroll
+            for (int a = 0; a < 6; a++) dl[a] -= G0[a];
+            lam_inv_apply<NU>(P, geo, geo + 12, dl, lam);
+        }
+        TM_PHASE();
+        // u = u0 + Rt^-1 Gh^T lam, contact by contact;  y <- y + u  (= the argument v of the projection)
+        float uk[EMIT ? NU : 1];
+        {
+            float v[RBW - 12];
+            tm_ld_groups<3, RBW / 4>(rb, nsl, v);
+            const float *rr = v, *ru = v + 3 * NC;
+#pragma unroll
+            for (int i = 0; i < NC; i++) {
+                const float rx = rr[3 * i], ry = rr[3 * i + 1], rz = rr[3 * i + 2];
+                const float gl[6] = { fmaf(lam[1], rz, fmaf(-lam[2], ry, lam[3])), fmaf(lam[2], rx, fmaf(-lam[0], rz, lam[4])),
+                                      fmaf(lam[0], ry, fmaf(-lam[1], rx, lam[5])), lam[0], lam[1], lam[2] };
+#pragma unroll
+                for (int a = 0; a < (i < NW ? 6 : 3); a++) {
+                    const int c = a < 3 ? fcol(i) + a : mcol(i) + a - 3;
+                    const float u = fmaf(P.tR[c], gl[a], fmaf(P.rtR[c], z[c] - y[c], ru[c]));
+                    if (EMIT) { uk[c] = u; ou[c] = u; res[2] = fmaxf(res[2], fabsf(u)); }
+                    y[c] += u;
+                }
+            }
+        }
+        TM_PHASE();
+        // the feet: ONE exact projection when no thread of the warp has both feet in stance (a swing foot projects to
+        // 0): the argument of the stance foot is selected, projected and scattered; else a second one of foot 0
+        float zf[NW][6];
+        {
+            const bool on0 = bits & 1, on1 = (bits >> 1) & 1;
+            float vs[6], zs[6];
+#pragma unroll
+            for (int a = 0; a < 6; a++) {
+                const int c0 = a < 3 ? fcol(0) + a : mcol(0) + a - 3, c1 = a < 3 ? fcol(1) + a : mcol(1) + a - 3;
+                vs[a] = on1 ? y[c1] : y[c0];
+            }
+            project_wrench(P, vs[0], vs[1], vs[2], vs[3], vs[4], vs[5], zs[0], zs[1], zs[2], zs[3], zs[4], zs[5]);
+#pragma unroll
+            for (int a = 0; a < 6; a++) { zf[1][a] = on1 ? zs[a] : 0.0f; zf[0][a] = (on0 && !on1) ? zs[a] : 0.0f; }
+            if (two_feet) {
+                float z0p[6];
+                project_wrench(P, y[fcol(0)], y[fcol(0) + 1], y[fcol(0) + 2], y[mcol(0)], y[mcol(0) + 1], y[mcol(0) + 2], z0p[0], z0p[1], z0p[2],
+                               z0p[3], z0p[4], z0p[5]);
+#pragma unroll
+                for (int a = 0; a < 6; a++) zf[0][a] = on0 ? z0p[a] : 0.0f;
+            }
+        }
+        // z <- projection, y <- v - z
+#pragma unroll
+        for (int i = 0; i < NC; i++) {
+            const bool on = (bits >> i) & 1;
+#pragma unroll
+            for (int a = 0; a < (i < NW ? 6 : 3); a++) {
+                const int c = a < 3 ? fcol(i) + a : mcol(i) + a - 3;
+                const float zn = i < NW ? zf[i < NW ? i : 0][a] : (on ? fminf(fmaxf(y[c], -P.hand_fmax), P.hand_fmax) : 0.0f);
+                const float yn = y[c] - zn;
+                if (EMIT) {
+                    res[0] = fmaxf(res[0], fabsf(uk[c] - zn));
+                    res[1] = fmaxf(res[1], fabsf(zn - z[c]));
+                    res[3] = fmaxf(res[3], fabsf(zn)); res[4] = fmaxf(res[4], fabsf(yn));
+                }
+                z[c] = zn; y[c] = yn;
+            }
+        }
+        TM_PHASE();
+        {
+            float v[RBW - 12];
+            tm_ld_groups<3, RBW / 4>(rb, nsl, v);
+            tm_gh_u0<NU>(P, v, z, y, G0);                       // Gh u0 of the next iteration
+        }
+        TM_PHASE();
+    }
+    {
+        float geo[4 * GEO4];
+        tm_ld_groups<0, GEO4>(rb, nsl, geo);
+        tm_sigma0<NU>(P, geo, G0, idt, m_dt, wv);               // frozen envs keep a well-defined (constant) sigma0
+    }
+}
+
+#ifdef PINMPC_TM_TIMING
+#define TM_TICK(i) { int dmy_ = *(volatile int *)ndone; asm volatile("" :: "r"(dmy_) : "memory"); tn = clock64(); tacc[i] += tn - tt; tt = tn; }
+#else
+#define TM_TICK(i)
+#endif
+
+// ---------------------------------------------------------------------------------------------
+// The iteration loop of a chain warp.  NOT inlined on purpose: the chain loop then gets its own register
+// allocation (operand buffers of a whole stage), independent of the stage-update code of the worker warps in the
+// kernel body; a value spilled in a sweep loop would cost an L2 round trip per step (the 227 KB of shared memory
+// leave no L1 for local memory).
+// ---------------------------------------------------------------------------------------------
+struct ChainArgs {
+    Chain ch;
+    float dt, gdt, x12;
+    int has_ext, iters, check_every, tol_mode, C, cc, cvalid, Gv;
+    float *slot_lo, *oxe;
+    int *done_e, *ndone;
+};
+
+template <int RBW>
+__device__ __noinline__ void tm_chain_main(ChainArgs A)
+{
+    const Chain ch = A.ch;
+    const float dt = A.dt, gdt = A.gdt, x12 = A.x12;
+    const int has_ext = A.has_ext, C = A.C, cc = A.cc;
+    const bool cvalid = A.cvalid != 0;
+    float *slot_lo = A.slot_lo, *slot_hi = A.slot_lo + 12, *oxe = A.oxe;
+    int *ndone = A.ndone;
+#ifdef PINMPC_TM_TIMING
+    long long tacc[8] = { 0, 0, 0, 0, 0, 0, 0, 0 }, tt = clock64(), tn;
+#endif
+    for (int it = 0; it < A.iters; it++) {
+        const bool is_check = A.tol_mode && ((it + 1) % A.check_every == 0);
+        const bool emit = (it == A.iters - 1) || is_check;
+        tm_sync();                                          // (1) sigma0 of every stage is in the exchange vectors
+        TM_TICK(0)
+        // ---- backward sweep A: zero terminal costate -> b_c (the last chunk: its true costate)
+        float pq[6], pv[6];
+        if (C > 1) {
+#pragma unroll
+            for (int i = 0; i < 6; i++) { pq[i] = 0.0f; pv[i] = 0.0f; }
+            if (TM_ABL != 3 && TM_ABL != 4) chain_bwd_sweep<false, RBW>(ch, dt, pq, pv);
+            if (cvalid && cc >= 1) {
+#pragma unroll
+                for (int i = 0; i < 6; i++) { slot_lo[i] = pq[i]; slot_lo[6 + i] = pv[i]; }
+            }
+        }
+        TM_TICK(1)
+        __syncthreads();                                    // (2) boundary recursion (workers)
+        __syncthreads();                                    // (3) true terminal costates in the slots
+        TM_TICK(2)
+        // ---- backward sweep B: true terminal costate; hh -> exchange, then kappa
+#pragma unroll
+        for (int i = 0; i < 6; i++) { pq[i] = slot_hi[i]; pv[i] = slot_hi[6 + i]; }
+        if (TM_ABL != 4) chain_bwd_sweep<true, RBW>(ch, dt, pq, pv);
+        tm_wait_st();
+        TM_TICK(3)
+        // ---- forward sweep A: zero start state (chunk 0: x_0) -> d_c (chunk 0: its true end state)
+        float xa[6], xb[6];
+        if (C > 1) {
+#pragma unroll
+            for (int i = 0; i < 6; i++) { xa[i] = cc == 0 ? slot_lo[i] : 0.0f; xb[i] = cc == 0 ? slot_lo[6 + i] : 0.0f; }
+            if (TM_ABL != 3 && TM_ABL != 4) chain_fwd_sweep<false, false, RBW>(ch, dt, gdt, x12, has_ext, xa, xb, false, oxe);
+            if (cvalid && cc <= C - 2) {
+#pragma unroll
+                for (int i = 0; i < 6; i++) { slot_hi[i] = xa[i]; slot_hi[6 + i] = xb[i]; }
+            }
+        }
+        TM_TICK(4)
+        __syncthreads();                                    // (4) boundary recursion (workers)
+        __syncthreads();                                    // (5) true start states in the slots
+        TM_TICK(5)
+        // ---- forward sweep B: true start state; w -> exchange, x -> output
+#pragma unroll
+        for (int i = 0; i < 6; i++) { xa[i] = slot_lo[i]; xb[i] = slot_lo[6 + i]; }
+        if (TM_ABL == 4) {}
+        else if (emit) chain_fwd_sweep<true, true, RBW>(ch, dt, gdt, x12, has_ext, xa, xb, cvalid && !*A.done_e, oxe);
+        else chain_fwd_sweep<true, false, RBW>(ch, dt, gdt, x12, has_ext, xa, xb, false, oxe);
+        TM_TICK(6)
+        tm_sync();                                          // (6) w of every stage is in the exchange vectors
+        if (emit) {
+            __syncthreads();                                // residuals reduced
+            __syncthreads();                                // done flags updated
+            if (is_check && *ndone == A.Gv) break;
+        }
+    }
+#ifdef PINMPC_TM_TIMING
+    if (blockIdx.x == 0 && threadIdx.x == 0)
+        printf("chain cycles/iter: wait-update %lld | bwdA %lld | bnd %lld | bwdB %lld | fwdA %lld | bnd %lld | fwdB %lld\n", tacc[0] / A.iters,
+               tacc[1] / A.iters, tacc[2] / A.iters, tacc[3] / A.iters, tacc[4] / A.iters, tacc[5] / A.iters, tacc[6] / A.iters);
+#endif
+}
+
+// ---------------------------------------------------------------------------------------------
+// S3-S6: all ADMM iterations of G envs per CTA.  12 warps: warps 0-3 are the CHAIN warps (lane t of warp q =
+// chain 32 q + t = TMEM lane), warps 4-7 and 8-11 the WORKER warps: worker (slot s = 0, 1; quarter q; lane t)
+// shares the TMEM lane of chain 32 q + t and owns stages 3 s .. 3 s + 2 of its chunk (z, y in registers).
+// 168 registers per thread: the chain threads hold two half-stage operand buffers, the workers three stages.
+// ---------------------------------------------------------------------------------------------
+template <int NU, bool WARM>
+__global__ void __launch_bounds__(TM_THREADS, 1) k_iterate_tm(SolveParams P, SrbWs W, const float *__restrict__ Psi, const float *__restrict__ x0g,
+                                                              const float *__restrict__ massg, OutPtrs o, int G, int C, int has_ext,
+                                                              const float *__restrict__ z0g, const float *__restrict__ y0g)
+{
+    constexpr int NC = NW + (NU - 12) / 3, RBW = tm_rbw(NU), GRBW = pinmpc_rb_width(NU);
+    extern __shared__ __align__(16) float smem[];
+    __shared__ uint32_t tmem_slot;
+    const int N = P.N, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const long st = (long)P.B * N;
+    const TmLay L = tm_layout(N, G, C, NU);
+    const int b0 = blockIdx.x * G;
+    const int Gv = min(G, P.B - b0);
+    float4 *recA4 = reinterpret_cast<float4 *>(smem + L.oA), *recB4 = reinterpret_cast<float4 *>(smem + L.oB);   // [group][slot]
+    float *psi = smem + L.oPsi, *bnd = smem + L.oBnd;
+    const int nsl = G * N, nch = G * C, cbase = N / C, crem = N - cbase * C;      // slots, chains, stages per chunk
+    // slot of stage j of chunk c of env e: stage-major over the chains; the one extra stage of the first crem chunks compacted
+    auto slot_of = [&](int e, int c, int j) { return j < cbase ? j * nch + e * C + c : cbase * nch + e * crem + c; };
+    int *ctl = reinterpret_cast<int *>(smem + L.oCtl);
+    int *done = ctl, *ndone = ctl + 32;
+    unsigned *red = reinterpret_cast<unsigned *>(ctl + 48);
+    const float dt = P.dt, idt = 1.0f / P.dt;
+    const int nst = Gv * N;
+
+    // ---- tensor memory: all 512 columns (one CTA per SM) -------------------------------------------------
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"((uint32_t)__cvta_generic_to_shared(&tmem_slot)));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    // ---- stage records, chunk operators, boundary slots -------------------------------------------------------
+    {
+        const float4 *RA4 = reinterpret_cast<const float4 *>(W.RA), *RB4 = reinterpret_cast<const float4 *>(W.RB);
+        const long s0 = (long)b0 * N;
+        const int big = crem * (cbase + 1);                      // stages covered by the longer chunks
+        for (int i = tid; i < nst * (7 + GRBW / 4); i += TM_THREADS) {
+            const int g = i / nst, sl = i - g * nst;
+            const int e = sl / N, k = sl - e * N;
+            int c, j;
+            if (k < big) { c = k / (cbase + 1); j = k - c * (cbase + 1); }
+            else { c = crem + (k - big) / cbase; j = (k - big) - (c - crem) * cbase; }
+            const int slot = slot_of(e, c, j);
+            if (g < 7) {
+                float4 v = __ldg(RA4 + (long)g * st + s0 + sl);
+                if (g == 6) v.w = __ldg(W.RB + pinmpc_rec_index(12 + 3 * NC + NU, st, s0 + sl));      // contact bits
+                recA4[g * nsl + slot] = v;
+            } else {
+                const int gb = g - 7;
+                float4 v = __ldg(RB4 + (long)gb * st + s0 + sl);
+                if (gb == GRBW / 4 - 1) { v.z = __ldg(W.cs + (s0 + sl) * 2); v.w = __ldg(W.cs + (s0 + sl) * 2 + 1); }
+                recB4[gb * nsl + slot] = v;
+            }
+        }
+        if (C > 2) {
+            const int per = (C - 2) * 144;
+            for (int i = tid; i < Gv * per; i += TM_THREADS) psi[i] = __ldg(Psi + (long)b0 * per + i);
+        }
+        for (int i = tid; i < Gv * (C + 1) * 12; i += TM_THREADS) {
+            const int e = i / ((C + 1) * 12), r = i - e * (C + 1) * 12;
+            bnd[i] = r < 12 ? x0g[(long)(b0 + e) * NX + r] : 0.0f;                      // slot 0 = x_0, slot C = 0
+        }
+        for (int i = tid; i < TM_CTL; i += TM_THREADS) ctl[i] = 0;
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t tbase = tmem_slot;
+    const int wq = warp & 3;
+    const uint32_t myt = tbase + ((uint32_t)(wq * 32) << 16);
+
+    // ---- the chain (env, chunk) of this TMEM lane -------------------------------------------------------------
+    const int q = wq * 32 + lane;
+    const int ce = q / C, cc = q - ce * C;
+    const bool cvalid = ce < Gv;
+    int k0 = 0, clen = 0;
+    tm_chunk(N, C, cc, k0, clen);
+    if (!cvalid) clen = 0;
+    const int eb = cvalid ? ce : 0;
+    const int sl0 = eb * N + (cvalid ? k0 : 0);                 // first stage of the chunk, CTA-local
+    const int nsteps = N / C + (N % C ? 1 : 0);                  // the longest chunk
+    const bool tol_mode = (P.eps_abs > 0.0f || P.eps_rel > 0.0f) && P.check_every > 0;
+#ifdef PINMPC_TM_TIMING
+    long long tacc[8] = { 0, 0, 0, 0, 0, 0, 0, 0 }, tt = clock64(), tn;
+#endif
+
+    if (warp < 4) {
+        // =========================== CHAIN WARPS =================================================================
+        // prologue: the chunk's gains -> this lane of tensor memory, row-major Kn[r][0..11] = -Kh[r][.]
+        for (int j = 0; j < TM_LMAX; j++) {
+            float kq[72];
+            if (j < clen) {
+                const float4 *src = reinterpret_cast<const float4 *>(W.Kh + ((long)b0 * N + sl0 + j) * 72);
+#pragma unroll
+                for (int r = 0; r < 6; r++) {
+                    const float4 v0 = __ldg(src + 3 * r), v1 = __ldg(src + 3 * r + 1), v2 = __ldg(src + 3 * r + 2);
+                    float *d = kq + 12 * r;
+                    d[0] = -v0.x; d[6] = -v0.y; d[1] = -v0.z; d[7] = -v0.w;
+                    d[2] = -v1.x; d[8] = -v1.y; d[3] = -v1.z; d[9] = -v1.w;
+                    d[4] = -v2.x; d[10] = -v2.y; d[5] = -v2.z; d[11] = -v2.w;
+                }
+            } else {
+#pragma unroll
+                for (int i = 0; i < 72; i++) kq[i] = 0.0f;
+            }
+#pragma unroll
+            for (int c = 0; c < 9; c++) tm_st8(myt + 72 * j + 8 * c, kq + 8 * c);
+            float cv[6] = { 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f };
+            if (has_ext && j < clen) {
+#pragma unroll
+                for (int i = 0; i < 6; i++) cv[i] = __ldg(W.c6 + ((long)b0 * N + sl0 + j) * 6 + i);
+            }
+            tm_st6(myt + TM_COFF + 6 * j, cv);
+        }
+        tm_wait_st();
+        ChainArgs A;
+        A.ch.tk = myt;
+        A.ch.sA = (uint32_t)__cvta_generic_to_shared(recA4 + eb * C + cc);
+        A.ch.sCS = (uint32_t)__cvta_generic_to_shared(recB4 + (RBW / 4 - 1) * nsl + eb * C + cc) + 8;
+        A.ch.jstride = (uint32_t)nch * 16u; A.ch.wstride = (uint32_t)nsl * 16u;
+        A.ch.xoff = (uint32_t)(-(eb * (C - crem)) * 16);
+        A.ch.len = clen; A.ch.nsteps = nsteps; A.ch.base = cbase;
+        A.x12 = x0g[(long)(b0 + eb) * NX + 12];
+        A.dt = dt; A.gdt = dt * A.x12;
+        A.has_ext = has_ext; A.iters = P.iters; A.check_every = P.check_every; A.tol_mode = tol_mode; A.C = C; A.cc = cc; A.cvalid = cvalid; A.Gv = Gv;
+        A.slot_lo = bnd + (eb * (C + 1) + cc) * 12;             // forward: start state; backward: own offset / true costate
+        A.oxe = o.x + ((long)b0 * N + sl0) * NX;
+        A.done_e = done + eb; A.ndone = ndone;
+        tm_chain_main<RBW>(A);
+    } else {
+        // =========================== WORKER WARPS ==================================================================
+        constexpr int WS = TM_LMAX / 2;                          // stages per worker
+        const int ws = (warp - 4) >> 2;
+        bool act[WS];
+        int sl[WS], bits[WS];
+        const float4 *rb[WS];
+        bool two_feet[WS];
+#pragma unroll
+        for (int a = 0; a < WS; a++) {
+            const int j = WS * ws + a;
+            act[a] = j < clen;
+            sl[a] = sl0 + (act[a] ? j : 0);                       // CTA-local stage index
+            const int slot = slot_of(eb, cc, act[a] ? j : 0);
+            rb[a] = recB4 + slot;
+            bits[a] = __float_as_int(recA4[6 * nsl + slot].w);
+            two_feet[a] = __any_sync(FULL, act[a] && (bits[a] & 3) == 3);   // then two projections per stage in this warp
+        }
+        const uint32_t tx = myt + TM_XOFF + 6 * WS * ws;        // exchange vectors of the owned stages
+        const long tsb = (long)b0 * N;
+        const float m_dt = massg[b0 + eb] / dt;
+        // boundary-recursion role: 12 lanes per env, two envs per warp
+        const int bw = warp - 4, bsub = lane / 12, bi = lane - 12 * bsub;
+        const int bsrc = 12 * (bsub < 2 ? bsub : 0);
+
+        TmState<NU> S[WS];
+#pragma unroll
+        for (int a = 0; a < WS; a++) {
+            float sv[6] = { 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f };
+            const long ts = tsb + sl[a];
+#pragma unroll
+            for (int j = 0; j < NU; j++) {
+                S[a].z[j] = (WARM && act[a]) ? __ldg(z0g + ts * NU + j) : 0.0f;
+                S[a].y[j] = (WARM && act[a]) ? __ldg(y0g + ts * NU + j) : 0.0f;
+            }
+            if (act[a]) {
+                float G0[6], v[RBW];
+                tm_ld_groups<0, RBW / 4>(rb[a], nsl, v);
+                tm_gh_u0<NU>(P, v + 12, S[a].z, S[a].y, G0);
+                tm_sigma0<NU>(P, v, G0, idt, m_dt, sv);
+            }
+            tm_st6(tx + 6 * a, sv);
+        }
+        bool frozen = false;
+
+        for (int it = 0; it < P.iters; it++) {
+            const bool is_check = tol_mode && ((it + 1) % P.check_every == 0);
+            const bool emit = (it == P.iters - 1) || is_check;
+            if (emit)
+                for (int i = tid - 128; i < 5 * TM_GMAX; i += TM_THREADS - 128) red[i] = 0u;
+            TM_TICK(0)
+            tm_sync();                                          // (1)
+            __syncthreads();                                    // (2) b_c of every chunk is in the slots
+            TM_TICK(1)
+            // ---- backward boundary recursion: slot[c] <- Psi_c^T slot[c+1] + slot[c],  c = C-2 .. 1
+            if (TM_ABL != 2 && C > 2 && bsub < 2) {
+                for (int ep = 2 * bw; ep < Gv; ep += 16) {        // two envs per warp (an env past the end rides along)
+                    const int e = ep + bsub, ee = e < Gv ? e : 0;
+                    float *sb = bnd + ee * (C + 1) * 12;
+                    const float *ps = psi + ee * (C - 2) * 144;
+                    float p = sb[(C - 1) * 12 + bi];
+                    for (int c = C - 2; c >= 1; c--) {
+                        const float *m = ps + (c - 1) * 144 + bi;               // column bi of Psi_c
+                        float a0 = sb[c * 12 + bi], a1 = 0.0f, a2 = 0.0f;
+#pragma unroll
+                        for (int j = 0; j < 12; j += 3) {
+                            a0 = fmaf(m[12 * j], __shfl_sync(BMASK, p, bsrc + j), a0);
+                            a1 = fmaf(m[12 * (j + 1)], __shfl_sync(BMASK, p, bsrc + j + 1), a1);
+                            a2 = fmaf(m[12 * (j + 2)], __shfl_sync(BMASK, p, bsrc + j + 2), a2);
+                        }
+                        p = a0 + (a1 + a2);
+                        if (e < Gv) sb[c * 12 + bi] = p;
+                    }
+                }
+            }
+            TM_TICK(2)
+            __syncthreads();                                    // (3)
+            __syncthreads();                                    // (4) d_c of every chunk is in the slots
+            TM_TICK(3)
+            // ---- forward boundary recursion: slot[c+1] <- Psi_c slot[c] + slot[c+1],  c = 1 .. C-2
+            if (TM_ABL != 2 && C > 2 && bsub < 2) {
+                for (int ep = 2 * bw; ep < Gv; ep += 16) {
+                    const int e = ep + bsub, ee = e < Gv ? e : 0;
+                    float *sb = bnd + ee * (C + 1) * 12;
+                    const float *ps = psi + ee * (C - 2) * 144;
+                    float x = sb[12 + bi];
+                    for (int c = 1; c <= C - 2; c++) {
+                        const float4 *m = reinterpret_cast<const float4 *>(ps + (c - 1) * 144 + 12 * bi);   // row bi of Psi_c
+                        const float4 m0 = m[0], m1 = m[1], m2 = m[2];
+                        float a0 = sb[(c + 1) * 12 + bi], a1, a2;
+                        a0 = fmaf(m0.x, __shfl_sync(BMASK, x, bsrc + 0), a0); a1 = m0.y * __shfl_sync(BMASK, x, bsrc + 1);
+                        a2 = m0.z * __shfl_sync(BMASK, x, bsrc + 2); a0 = fmaf(m0.w, __shfl_sync(BMASK, x, bsrc + 3), a0);
+                        a1 = fmaf(m1.x, __shfl_sync(BMASK, x, bsrc + 4), a1); a2 = fmaf(m1.y, __shfl_sync(BMASK, x, bsrc + 5), a2);
+                        a0 = fmaf(m1.z, __shfl_sync(BMASK, x, bsrc + 6), a0); a1 = fmaf(m1.w, __shfl_sync(BMASK, x, bsrc + 7), a1);
+                        a2 = fmaf(m2.x, __shfl_sync(BMASK, x, bsrc + 8), a2); a0 = fmaf(m2.y, __shfl_sync(BMASK, x, bsrc + 9), a0);
+                        a1 = fmaf(m2.z, __shfl_sync(BMASK, x, bsrc + 10), a1); a2 = fmaf(m2.w, __shfl_sync(BMASK, x, bsrc + 11), a2);
+                        x = a0 + (a1 + a2);
+                        if (e < Gv) sb[(c + 1) * 12 + bi] = x;
+                    }
+                }
+            }
+            TM_TICK(4)
+            __syncthreads();                                    // (5)
+            tm_sync();                                          // (6) w of every stage is in the exchange vectors
+            TM_TICK(5)
+            // ---- stage update: u from w, projection, dual update, residuals, next sigma0 (one stage after the other)
+            {
+                float res[5] = { 0.0f, 0.0f, 0.0f, 0.0f, 0.0f };
+#pragma unroll
+                for (int a = 0; a < WS; a++) {
+                    float wv[6];
+                    tm_ld6(tx + 6 * a, wv);
+                    tm_wait_ld();
+                    if (act[a] && TM_ABL != 1) {
+                        if (emit) tm_stage_update<NU, true>(P, rb[a], nsl, bits[a], S[a].z, S[a].y, idt, m_dt, wv, !frozen, o.u + (tsb + sl[a]) * NU, res, two_feet[a]);
+                        else tm_stage_update<NU, false>(P, rb[a], nsl, bits[a], S[a].z, S[a].y, idt, m_dt, wv, !frozen, o.u + (tsb + sl[a]) * NU, res, two_feet[a]);
+                    } else { wv[0] = wv[1] = wv[2] = wv[3] = wv[4] = wv[5] = 0.0f; }   // unused exchange vectors stay zero
+                    tm_st6(tx + 6 * a, wv);
+                    asm volatile("" ::: "memory");
+                }
+                if (emit && act[0] && !frozen) {
+                    atomicMax(&red[eb * 5 + 0], __float_as_uint(res[0])); atomicMax(&red[eb * 5 + 1], __float_as_uint(res[1]));
+                    atomicMax(&red[eb * 5 + 2], __float_as_uint(res[2])); atomicMax(&red[eb * 5 + 3], __float_as_uint(res[3]));
+                    atomicMax(&red[eb * 5 + 4], __float_as_uint(res[4]));
+                }
+            }
+            if (emit) {
+                __syncthreads();
+                const int ld = tid - 128;
+                if (ld < Gv && !done[ld]) {                    // one leader per env
+                    const int e = ld;
+                    const float rp = __uint_as_float(red[e * 5 + 0]), rd = P.rho * __uint_as_float(red[e * 5 + 1]);
+                    o.r_prim[b0 + e] = rp; o.r_dual[b0 + e] = rd; o.iters_done[b0 + e] = it + 1;
+                    if (is_check) {
+                        const float sc = fmaxf(__uint_as_float(red[e * 5 + 2]), __uint_as_float(red[e * 5 + 3]));
+                        const float ys = __uint_as_float(red[e * 5 + 4]);
+                        if (rp <= P.eps_abs + P.eps_rel * sc && rd <= P.eps_abs + P.eps_rel * P.rho * ys) {
+                            done[e] = 1;
+                            atomicAdd(ndone, 1);
+                        }
+                    }
+                }
+                __syncthreads();
+                if (is_check) {
+                    if (*ndone == Gv) break;
+                    frozen = done[eb] != 0;
+                }
+            }
+        }
+#ifdef PINMPC_TM_TIMING
+        if (blockIdx.x == 0 && tid == 128)
+            printf("worker cycles/iter: update %lld | wait bwdA %lld | bnd-bwd %lld | wait bwdB+fwdA %lld | bnd-fwd %lld | wait fwdB %lld\n", tacc[0] / P.iters,
+                   tacc[1] / P.iters, tacc[2] / P.iters, tacc[3] / P.iters, tacc[4] / P.iters, tacc[5] / P.iters);
+#endif
+#pragma unroll
+        for (int a = 0; a < WS; a++)
+            if (act[a]) {
+                float *oz = o.z + (tsb + sl[a]) * NU, *oy = o.y + (tsb + sl[a]) * NU;
+#pragma unroll
+                for (int j = 0; j < NU; j++) { oz[j] = S[a].z[j]; oy[j] = S[a].y[j]; }
+            }
+    }
+    // ---- release tensor memory ---------------------------------------------------------------------------------
+    tm_sync();
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tbase));
+}
+
+int tm_fail(pinmpc_ctx *h, const char *what, cudaError_t e)
+{
+    h->sticky = e;
+    snprintf(h->err, sizeof h->err, "%s: %s", what, cudaGetErrorString(e));
+    return -1;
+}
+
+}  // namespace
+
+size_t pinmpc_tm_smem_bytes(int N, int G, int C, int nu) { return (size_t)tm_layout(N, G, C, nu).total * sizeof(float); }
+
+// Chunk count and envs per CTA of the chunked kernel for this handle (0, 0 when the shape does not fit):
+// C = ceil(N / 6) unless forced; G = as many envs as chains (G C <= 128), shared memory and the batch allow,
+// fewest rounds of the batch over the device first, then the smallest such G (shorter boundary/update phases).
+bool pinmpc_tm_config(const pinmpc_ctx *h, int *Gout, int *Cout)
+{
+    const int N = h->N;
+    int C = h->chunks > 1 ? h->chunks : (N + TM_LMAX - 1) / TM_LMAX;
+    if (C < 1 || (N + C - 1) / C > TM_LMAX || C > N || C > TM_CHAINS || C - 2 > h->psi_cap) return false;
+    int best = 0;
+    long best_rounds = 0;
+    for (int G = 1; G <= TM_GMAX; G++) {
+        if (G * C > TM_CHAINS) break;
+        if (pinmpc_tm_smem_bytes(N, G, C, h->nu) + 256 > (size_t)h->smem_optin) break;
+        const long per_round = (long)G * h->sm_count;
+        const long rounds = (h->B + per_round - 1) / per_round;
+        if (best == 0 || rounds < best_rounds) { best = G; best_rounds = rounds; }
+    }
+    if (h->envs_per_cta > 0 && h->envs_per_cta <= TM_GMAX && h->envs_per_cta * C <= TM_CHAINS &&
+        pinmpc_tm_smem_bytes(N, h->envs_per_cta, C, h->nu) + 256 <= (size_t)h->smem_optin)
+        best = h->envs_per_cta;
+    if (best == 0) return false;
+    *Gout = best; *Cout = C;
+    return true;
+}
+
+template <int NU>
+static int tm_launch_t(pinmpc_ctx *h, const SolveParams &P, const ProblemPtrs &q, int G, int C, cudaStream_t st)
+{
+    const int ext = q.ext != nullptr;
+    int n = 0;
+    if (C > 2) {
+        const long rows = (long)h->B * (C - 2) * 12;
+        k_chunk_ops<<<(unsigned)((rows + 191) / 192), 192, 0, st>>>(h->B, h->N, C, h->dt, h->srb.Kh, h->srb.cs, h->psi);
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return tm_fail(h, "k_chunk_ops launch", e);
+        n++;
+    }
+    auto kern = q.z0 ? k_iterate_tm<NU, true> : k_iterate_tm<NU, false>;
+    const size_t smem = pinmpc_tm_smem_bytes(h->N, G, C, h->nu);
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem_optin - 256);
+    if (e != cudaSuccess) return tm_fail(h, "k_iterate_tm smem attribute", e);
+    kern<<<(unsigned)((h->B + G - 1) / G), TM_THREADS, smem, st>>>(P, h->srb, h->psi, q.x0, q.mass, h->out, G, C, ext, q.z0, q.y0);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return tm_fail(h, "k_iterate_tm launch", e);
+    return n + 1;
+}
+
+// Launch the chunk-operator kernel and the chunked iteration kernel (after assembly and factorisation).
+// Returns the number of kernels enqueued, or -1.
+int pinmpc_launch_iterate_tm(pinmpc_ctx *h, int G, int C, cudaStream_t st)
+{
+    SolveParams P = make_params(h);
+    ProblemPtrs q = make_problem_ptrs(h);
+    return h->nu == 12 ? tm_launch_t<12>(h, P, q, G, C, st) : tm_launch_t<18>(h, P, q, G, C, st);
+}
