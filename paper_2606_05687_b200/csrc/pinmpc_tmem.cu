@@ -43,7 +43,7 @@ constexpr int TM_THREADS = 384;                    // 4 chain warps + 8 worker w
 constexpr int TM_GMAX = 32;                        // envs per CTA
 constexpr int TM_RAW = 28;                         // Mh^-1 (21) | kg (6) | contact bits
 constexpr int TM_CTL = 48 + 5 * TM_GMAX;           // done[32] | ndone | pad[15] | red[32][5]
-constexpr unsigned BMASK = 0x00ffffffu;            // the 24 boundary lanes of a worker warp
+constexpr unsigned BMASK = 0x00ffffffu;            // the 24 boundary lanes of a worker warp (2 envs x 12 lanes)
 
 __host__ __device__ constexpr int tm_rbw(int nu) { return 12 + 3 * (2 + (nu - 12) / 3) + nu + 2; }   // T^-1 | I_w | r | R ubar' | cos sin
 
@@ -190,15 +190,20 @@ __device__ __forceinline__ void chain_ld_stage(uint32_t tk, int j, float *k)
 }
 
 // A chunk shorter than the sweep (nsteps) has zero gains, zero exchange vectors and dt, g dt switched off in its unused
-// steps, which makes those steps the identity.  Within a step the 72 gains are requested at once and consumed row
-// by row as they arrive (the hardware scoreboard tracks every tcgen05.ld destination).
+// steps, which makes those steps the identity.  Within a step the 72 gains are requested at once and consumed row by
+// row as they arrive (the hardware scoreboard tracks every tcgen05.ld destination).
 
 // Backward sweep over the chunk, stages nsteps-1 .. 0:  hh = sigma0 + pv ;  p <- Phi^T p + Kn^T sigma0.
-// OUT: kappa = Mh^-1 hh - kg replaces sigma0 in the exchange vector of every stage (computed while the gains stream in;
-// an unused step keeps its zero).
-template <bool OUT, int RBW>
-__device__ __forceinline__ void chain_bwd_sweep(const Chain &ch, float dt, float *pq, float *pv)
+// OUT: kappa = Mh^-1 hh - kg replaces sigma0 in the exchange vector of every stage (an unused step keeps its zero).
+// init: the terminal costate (12 floats in shared memory; nullptr = 0); fin: where the costate at the chunk start goes
+// (nullptr = nowhere).
+template <bool OUT>
+__device__ __forceinline__ void chain_bwd_sweep(const Chain &ch, float dt, const float *init, float *fin)
 {
+    float q[6], v[6];
+#pragma unroll
+    for (int i = 0; i < 6; i++) { q[i] = init ? init[i] : 0.0f; v[i] = init ? init[6 + i] : 0.0f; }
+#pragma unroll 1
     for (int j = ch.nsteps - 1; j >= 0; j--) {
         float k[72], s0[6];
         tm_ld6(ch.tk + TM_XOFF + 6 * j, s0);
@@ -206,21 +211,18 @@ __device__ __forceinline__ void chain_bwd_sweep(const Chain &ch, float dt, float
         const bool act = j < ch.len;
         const float dte = act ? dt : 0.0f;
         const float2 cs = lds_f2(ch.sCS + chain_joff(ch, j));
-        float Mi[28];
-        if (OUT) {
-            const uint32_t a = ch.sA + chain_joff(ch, j);
-#pragma unroll
-            for (int c = 0; c < 7; c++) {
-                const float4 q = lds_f4(a + c * ch.wstride);
-                Mi[4 * c] = q.x; Mi[4 * c + 1] = q.y; Mi[4 * c + 2] = q.z; Mi[4 * c + 3] = q.w;
-            }
-        }
         tm_wait_ld();
         float hh[6];
 #pragma unroll
-        for (int r = 0; r < 6; r++) hh[r] = s0[r] + pv[r];
+        for (int r = 0; r < 6; r++) hh[r] = s0[r] + v[r];
         if (OUT) {
-            float kp[6];
+            float Mi[28], kp[6];
+            const uint32_t a = ch.sA + chain_joff(ch, j);
+#pragma unroll
+            for (int c = 0; c < 7; c++) {
+                const float4 t = lds_f4(a + c * ch.wstride);
+                Mi[4 * c] = t.x; Mi[4 * c + 1] = t.y; Mi[4 * c + 2] = t.z; Mi[4 * c + 3] = t.w;
+            }
             symv6(Mi, hh, kp);
 #pragma unroll
             for (int r = 0; r < 6; r++) kp[r] = act ? kp[r] - Mi[21 + r] : 0.0f;
@@ -228,18 +230,23 @@ __device__ __forceinline__ void chain_bwd_sweep(const Chain &ch, float dt, float
         }
         // (A^T p)_v = pv + dt Rot^T pq  (old pq)
         {
-            const float t0 = cs.x * pq[0] - cs.y * pq[1], t1 = cs.x * pq[1] + cs.y * pq[0];
-            pv[0] = fmaf(dte, t0, pv[0]); pv[1] = fmaf(dte, t1, pv[1]);
+            const float t0 = cs.x * q[0] - cs.y * q[1], t1 = cs.x * q[1] + cs.y * q[0];
+            v[0] = fmaf(dte, t0, v[0]); v[1] = fmaf(dte, t1, v[1]);
 #pragma unroll
-            for (int i = 2; i < 6; i++) pv[i] = fmaf(dte, pq[i], pv[i]);
+            for (int i = 2; i < 6; i++) v[i] = fmaf(dte, q[i], v[i]);
         }
 #pragma unroll
         for (int r = 0; r < 6; r++)
 #pragma unroll
             for (int i = 0; i < 6; i++) {
-                pq[i] = fmaf(k[12 * r + i], hh[r], pq[i]);
-                pv[i] = fmaf(k[12 * r + 6 + i], hh[r], pv[i]);
+                q[i] = fmaf(k[12 * r + i], hh[r], q[i]);
+                v[i] = fmaf(k[12 * r + 6 + i], hh[r], v[i]);
             }
+    }
+    if (OUT) tm_wait_st();
+    if (fin) {
+#pragma unroll
+        for (int i = 0; i < 6; i++) { fin[i] = q[i]; fin[6 + i] = v[i]; }
     }
 }
 
@@ -267,10 +274,15 @@ __device__ __forceinline__ void chain_kappa(const Chain &ch)
 }
 
 // Forward sweep over the chunk, stages 0 .. nsteps-1:  w = kappa + Kn x ;  x+ = A x + E (w + c).
-// OUT: w replaces kappa in the exchange vector; EMIT (with OUT): x+ -> ox (x_{k+1} of the output).
-template <bool OUT, bool EMIT, int RBW>
-__device__ __forceinline__ void chain_fwd_sweep(const Chain &ch, float dt, float gdt, float x12, int has_ext, float *xa, float *xb, bool wr, float *ox)
+// OUT: w replaces kappa in the exchange vector; ox != nullptr (with OUT): x+ -> ox (x_{k+1} of the output).
+// init: the start state (12 floats in shared memory; nullptr = 0); fin: where the end state goes (nullptr = nowhere).
+template <bool OUT>
+__device__ __forceinline__ void chain_fwd_sweep(const Chain &ch, float dt, float gdt, float x12, int has_ext, const float *init, float *fin, float *ox)
 {
+    float xa[6], xb[6];
+#pragma unroll
+    for (int i = 0; i < 6; i++) { xa[i] = init ? init[i] : 0.0f; xb[i] = init ? init[6 + i] : 0.0f; }
+#pragma unroll 1
     for (int j = 0; j < ch.nsteps; j++) {
         float k[72], w[6], cv[6];
 #pragma unroll
@@ -300,12 +312,16 @@ __device__ __forceinline__ void chain_fwd_sweep(const Chain &ch, float dt, float
 #pragma unroll
         for (int i = 0; i < 6; i++) xb[i] += w[i] + cv[i];
         xb[5] += gdte;
-        if (OUT && EMIT && wr && act) {
+        if (ox != nullptr && act) {
             float *o = ox + j * NX;
 #pragma unroll
             for (int i = 0; i < 6; i++) { o[i] = xa[i]; o[6 + i] = xb[i]; }
             o[12] = x12;
         }
+    }
+    if (fin) {
+#pragma unroll
+        for (int i = 0; i < 6; i++) { fin[i] = xa[i]; fin[6 + i] = xb[i]; }
     }
 }
 
@@ -469,7 +485,10 @@ __device__ __forceinline__ void tm_stage_update(const SolveParams &P, const floa
 }
 
 #ifdef PINMPC_TM_TIMING
-#define TM_TICK(i) { int dmy_ = *(volatile int *)ndone; asm volatile("" :: "r"(dmy_) : "memory"); tn = clock64(); tacc[i] += tn - tt; tt = tn; }
+// timestamps of one iteration (chain: thread 0 -> pad[0..6], worker: thread 128 -> pad[7..13]); read after a barrier-protected load
+#define TM_TICK(i) { if (it == TM_TICK_IT && (threadIdx.x == 0 || threadIdx.x == 128)) { int dmy_ = *(volatile int *)ndone; asm volatile("" :: "r"(dmy_) : "memory"); \
+                     ((volatile int *)ndone)[1 + (threadIdx.x == 0 ? 0 : 7) + (i)] = (int)clock(); } }
+#define TM_TICK_IT 50
 #else
 #define TM_TICK(i)
 #endif
@@ -497,56 +516,29 @@ __device__ __noinline__ void tm_chain_main(ChainArgs A)
     const bool cvalid = A.cvalid != 0;
     float *slot_lo = A.slot_lo, *slot_hi = A.slot_lo + 12, *oxe = A.oxe;
     int *ndone = A.ndone;
-#ifdef PINMPC_TM_TIMING
-    long long tacc[8] = { 0, 0, 0, 0, 0, 0, 0, 0 }, tt = clock64(), tn;
-#endif
     for (int it = 0; it < A.iters; it++) {
         const bool is_check = A.tol_mode && ((it + 1) % A.check_every == 0);
         const bool emit = (it == A.iters - 1) || is_check;
         tm_sync();                                          // (1) sigma0 of every stage is in the exchange vectors
         TM_TICK(0)
         // ---- backward sweep A: zero terminal costate -> b_c (the last chunk: its true costate)
-        float pq[6], pv[6];
-        if (C > 1) {
-#pragma unroll
-            for (int i = 0; i < 6; i++) { pq[i] = 0.0f; pv[i] = 0.0f; }
-            if (TM_ABL != 3 && TM_ABL != 4) chain_bwd_sweep<false, RBW>(ch, dt, pq, pv);
-            if (cvalid && cc >= 1) {
-#pragma unroll
-                for (int i = 0; i < 6; i++) { slot_lo[i] = pq[i]; slot_lo[6 + i] = pv[i]; }
-            }
-        }
+        if (C > 1 && TM_ABL != 3 && TM_ABL != 4) chain_bwd_sweep<false>(ch, dt, nullptr, (cvalid && cc >= 1) ? slot_lo : nullptr);
         TM_TICK(1)
         __syncthreads();                                    // (2) boundary recursion (workers)
         __syncthreads();                                    // (3) true terminal costates in the slots
         TM_TICK(2)
-        // ---- backward sweep B: true terminal costate; hh -> exchange, then kappa
-#pragma unroll
-        for (int i = 0; i < 6; i++) { pq[i] = slot_hi[i]; pv[i] = slot_hi[6 + i]; }
-        if (TM_ABL != 4) chain_bwd_sweep<true, RBW>(ch, dt, pq, pv);
-        tm_wait_st();
+        // ---- backward sweep B: true terminal costate; kappa -> exchange
+        if (TM_ABL != 4) chain_bwd_sweep<true>(ch, dt, slot_hi, nullptr);
         TM_TICK(3)
         // ---- forward sweep A: zero start state (chunk 0: x_0) -> d_c (chunk 0: its true end state)
-        float xa[6], xb[6];
-        if (C > 1) {
-#pragma unroll
-            for (int i = 0; i < 6; i++) { xa[i] = cc == 0 ? slot_lo[i] : 0.0f; xb[i] = cc == 0 ? slot_lo[6 + i] : 0.0f; }
-            if (TM_ABL != 3 && TM_ABL != 4) chain_fwd_sweep<false, false, RBW>(ch, dt, gdt, x12, has_ext, xa, xb, false, oxe);
-            if (cvalid && cc <= C - 2) {
-#pragma unroll
-                for (int i = 0; i < 6; i++) { slot_hi[i] = xa[i]; slot_hi[6 + i] = xb[i]; }
-            }
-        }
+        if (C > 1 && TM_ABL != 3 && TM_ABL != 4)
+            chain_fwd_sweep<false>(ch, dt, gdt, x12, has_ext, cc == 0 ? slot_lo : nullptr, (cvalid && cc <= C - 2) ? slot_hi : nullptr, nullptr);
         TM_TICK(4)
         __syncthreads();                                    // (4) boundary recursion (workers)
         __syncthreads();                                    // (5) true start states in the slots
         TM_TICK(5)
         // ---- forward sweep B: true start state; w -> exchange, x -> output
-#pragma unroll
-        for (int i = 0; i < 6; i++) { xa[i] = slot_lo[i]; xb[i] = slot_lo[6 + i]; }
-        if (TM_ABL == 4) {}
-        else if (emit) chain_fwd_sweep<true, true, RBW>(ch, dt, gdt, x12, has_ext, xa, xb, cvalid && !*A.done_e, oxe);
-        else chain_fwd_sweep<true, false, RBW>(ch, dt, gdt, x12, has_ext, xa, xb, false, oxe);
+        if (TM_ABL != 4) chain_fwd_sweep<true>(ch, dt, gdt, x12, has_ext, slot_lo, nullptr, (emit && cvalid && !*A.done_e) ? oxe : nullptr);
         TM_TICK(6)
         tm_sync();                                          // (6) w of every stage is in the exchange vectors
         if (emit) {
@@ -555,11 +547,6 @@ __device__ __noinline__ void tm_chain_main(ChainArgs A)
             if (is_check && *ndone == A.Gv) break;
         }
     }
-#ifdef PINMPC_TM_TIMING
-    if (blockIdx.x == 0 && threadIdx.x == 0)
-        printf("chain cycles/iter: wait-update %lld | bwdA %lld | bnd %lld | bwdB %lld | fwdA %lld | bnd %lld | fwdB %lld\n", tacc[0] / A.iters,
-               tacc[1] / A.iters, tacc[2] / A.iters, tacc[3] / A.iters, tacc[4] / A.iters, tacc[5] / A.iters, tacc[6] / A.iters);
-#endif
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -648,10 +635,6 @@ __global__ void __launch_bounds__(TM_THREADS, 1) k_iterate_tm(SolveParams P, Srb
     const int sl0 = eb * N + (cvalid ? k0 : 0);                 // first stage of the chunk, CTA-local
     const int nsteps = N / C + (N % C ? 1 : 0);                  // the longest chunk
     const bool tol_mode = (P.eps_abs > 0.0f || P.eps_rel > 0.0f) && P.check_every > 0;
-#ifdef PINMPC_TM_TIMING
-    long long tacc[8] = { 0, 0, 0, 0, 0, 0, 0, 0 }, tt = clock64(), tn;
-#endif
-
     if (warp < 4) {
         // =========================== CHAIN WARPS =================================================================
         // prologue: the chunk's gains -> this lane of tensor memory, row-major Kn[r][0..11] = -Kh[r][.]
@@ -699,40 +682,37 @@ __global__ void __launch_bounds__(TM_THREADS, 1) k_iterate_tm(SolveParams P, Srb
         // =========================== WORKER WARPS ==================================================================
         constexpr int WS = TM_LMAX / 2;                          // stages per worker
         const int ws = (warp - 4) >> 2;
-        bool act[WS];
-        int sl[WS], bits[WS];
-        const float4 *rb[WS];
-        bool two_feet[WS];
+        // Few values stay live across an iteration next to z, y of the three owned stages: everything per stage (slot,
+        // contact bits, activity) is recomputed where it is used (a spilled value costs an L2 round trip here).
+        const int jw = WS * ws;                                   // first owned stage of the chunk
+        const int slot_x = cbase * nch + eb * crem + cc;          // slot of the chunk's extra stage (if it has one)
+        const int slot_0 = eb * C + cc;                           // slot of the chunk's stage 0
+        auto slot_w = [&](int a) { const int j = jw + a; return j >= clen ? slot_0 : (j < cbase ? slot_0 + j * nch : slot_x); };
+        int flags = 0;                                            // bit a: stage a owned; bit 4 + a: two projections in this warp
 #pragma unroll
         for (int a = 0; a < WS; a++) {
-            const int j = WS * ws + a;
-            act[a] = j < clen;
-            sl[a] = sl0 + (act[a] ? j : 0);                       // CTA-local stage index
-            const int slot = slot_of(eb, cc, act[a] ? j : 0);
-            rb[a] = recB4 + slot;
-            bits[a] = __float_as_int(recA4[6 * nsl + slot].w);
-            two_feet[a] = __any_sync(FULL, act[a] && (bits[a] & 3) == 3);   // then two projections per stage in this warp
+            const bool ac = jw + a < clen;
+            const int bits = __float_as_int(recA4[6 * nsl + slot_w(a)].w);
+            flags |= (ac ? 1 : 0) << a;
+            flags |= (__any_sync(FULL, ac && (bits & 3) == 3) ? 1 : 0) << (4 + a);
         }
-        const uint32_t tx = myt + TM_XOFF + 6 * WS * ws;        // exchange vectors of the owned stages
-        const long tsb = (long)b0 * N;
+        const uint32_t tx = myt + TM_XOFF + 6 * jw;              // exchange vectors of the owned stages
         const float m_dt = massg[b0 + eb] / dt;
-        // boundary-recursion role: 12 lanes per env, two envs per warp
-        const int bw = warp - 4, bsub = lane / 12, bi = lane - 12 * bsub;
-        const int bsrc = 12 * (bsub < 2 ? bsub : 0);
 
         TmState<NU> S[WS];
 #pragma unroll
         for (int a = 0; a < WS; a++) {
             float sv[6] = { 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f };
-            const long ts = tsb + sl[a];
+            const bool ac = (flags >> a) & 1;
+            const long ts = (long)b0 * N + sl0 + (ac ? jw + a : 0);
 #pragma unroll
             for (int j = 0; j < NU; j++) {
-                S[a].z[j] = (WARM && act[a]) ? __ldg(z0g + ts * NU + j) : 0.0f;
-                S[a].y[j] = (WARM && act[a]) ? __ldg(y0g + ts * NU + j) : 0.0f;
+                S[a].z[j] = (WARM && ac) ? __ldg(z0g + ts * NU + j) : 0.0f;
+                S[a].y[j] = (WARM && ac) ? __ldg(y0g + ts * NU + j) : 0.0f;
             }
-            if (act[a]) {
+            if (ac) {
                 float G0[6], v[RBW];
-                tm_ld_groups<0, RBW / 4>(rb[a], nsl, v);
+                tm_ld_groups<0, RBW / 4>(recB4 + slot_w(a), nsl, v);
                 tm_gh_u0<NU>(P, v + 12, S[a].z, S[a].y, G0);
                 tm_sigma0<NU>(P, v, G0, idt, m_dt, sv);
             }
@@ -746,27 +726,38 @@ __global__ void __launch_bounds__(TM_THREADS, 1) k_iterate_tm(SolveParams P, Srb
             if (emit)
                 for (int i = tid - 128; i < 5 * TM_GMAX; i += TM_THREADS - 128) red[i] = 0u;
             TM_TICK(0)
+#ifdef PINMPC_TM_TIMING
+            if (it == TM_TICK_IT + 1 && tid == 128) ((volatile int *)ndone)[14] = (int)clock();
+#endif
             tm_sync();                                          // (1)
             __syncthreads();                                    // (2) b_c of every chunk is in the slots
             TM_TICK(1)
             // ---- backward boundary recursion: slot[c] <- Psi_c^T slot[c+1] + slot[c],  c = C-2 .. 1
-            if (TM_ABL != 2 && C > 2 && bsub < 2) {
-                for (int ep = 2 * bw; ep < Gv; ep += 16) {        // two envs per warp (an env past the end rides along)
+            // Lane bi owns component bi.  The twelve components of the previous step are gathered from the slot itself
+            // (three broadcast LDS.128 after a warp sync), column bi of Psi_c is fetched one step ahead.
+            if (TM_ABL != 2 && C > 2 && lane < 24) {
+                const int bsub = lane / 12, bi = lane - 12 * bsub;                       // 12 lanes per env, two envs per warp
+                for (int ep = 2 * (warp - 4); ep < Gv; ep += 16) {                     // (an env past the end rides along)
                     const int e = ep + bsub, ee = e < Gv ? e : 0;
                     float *sb = bnd + ee * (C + 1) * 12;
-                    const float *ps = psi + ee * (C - 2) * 144;
-                    float p = sb[(C - 1) * 12 + bi];
-                    for (int c = C - 2; c >= 1; c--) {
-                        const float *m = ps + (c - 1) * 144 + bi;               // column bi of Psi_c
-                        float a0 = sb[c * 12 + bi], a1 = 0.0f, a2 = 0.0f;
+                    const float *ps = psi + ee * (C - 2) * 144 + bi;
+                    float m[12];
 #pragma unroll
-                        for (int j = 0; j < 12; j += 3) {
-                            a0 = fmaf(m[12 * j], __shfl_sync(BMASK, p, bsrc + j), a0);
-                            a1 = fmaf(m[12 * (j + 1)], __shfl_sync(BMASK, p, bsrc + j + 1), a1);
-                            a2 = fmaf(m[12 * (j + 2)], __shfl_sync(BMASK, p, bsrc + j + 2), a2);
+                    for (int j = 0; j < 12; j++) m[j] = ps[(C - 3) * 144 + 12 * j];
+                    for (int c = C - 2; c >= 1; c--) {
+                        const float4 *pv4 = reinterpret_cast<const float4 *>(sb + (c + 1) * 12);
+                        const float4 p0 = pv4[0], p1 = pv4[1], p2 = pv4[2];
+                        float a0 = sb[c * 12 + bi];
+                        float a1 = m[1] * p0.y, a2 = m[2] * p0.z;
+                        a0 = fmaf(m[0], p0.x, a0); a0 = fmaf(m[3], p0.w, a0);
+                        a1 = fmaf(m[4], p1.x, a1); a2 = fmaf(m[5], p1.y, a2); a0 = fmaf(m[6], p1.z, a0); a1 = fmaf(m[7], p1.w, a1);
+                        a2 = fmaf(m[8], p2.x, a2); a0 = fmaf(m[9], p2.y, a0); a1 = fmaf(m[10], p2.z, a1); a2 = fmaf(m[11], p2.w, a2);
+                        if (c > 1) {
+#pragma unroll
+                            for (int j = 0; j < 12; j++) m[j] = ps[(c - 2) * 144 + 12 * j];
                         }
-                        p = a0 + (a1 + a2);
-                        if (e < Gv) sb[c * 12 + bi] = p;
+                        if (e < Gv) sb[c * 12 + bi] = a0 + (a1 + a2);
+                        __syncwarp(BMASK);
                     }
                 }
             }
@@ -775,24 +766,24 @@ __global__ void __launch_bounds__(TM_THREADS, 1) k_iterate_tm(SolveParams P, Srb
             __syncthreads();                                    // (4) d_c of every chunk is in the slots
             TM_TICK(3)
             // ---- forward boundary recursion: slot[c+1] <- Psi_c slot[c] + slot[c+1],  c = 1 .. C-2
-            if (TM_ABL != 2 && C > 2 && bsub < 2) {
-                for (int ep = 2 * bw; ep < Gv; ep += 16) {
+            if (TM_ABL != 2 && C > 2 && lane < 24) {
+                const int bsub = lane / 12, bi = lane - 12 * bsub;
+                for (int ep = 2 * (warp - 4); ep < Gv; ep += 16) {
                     const int e = ep + bsub, ee = e < Gv ? e : 0;
                     float *sb = bnd + ee * (C + 1) * 12;
-                    const float *ps = psi + ee * (C - 2) * 144;
-                    float x = sb[12 + bi];
+                    const float4 *ps = reinterpret_cast<const float4 *>(psi + ee * (C - 2) * 144 + 12 * bi);   // row bi
+                    float4 m0 = ps[0], m1 = ps[1], m2 = ps[2];
                     for (int c = 1; c <= C - 2; c++) {
-                        const float4 *m = reinterpret_cast<const float4 *>(ps + (c - 1) * 144 + 12 * bi);   // row bi of Psi_c
-                        const float4 m0 = m[0], m1 = m[1], m2 = m[2];
-                        float a0 = sb[(c + 1) * 12 + bi], a1, a2;
-                        a0 = fmaf(m0.x, __shfl_sync(BMASK, x, bsrc + 0), a0); a1 = m0.y * __shfl_sync(BMASK, x, bsrc + 1);
-                        a2 = m0.z * __shfl_sync(BMASK, x, bsrc + 2); a0 = fmaf(m0.w, __shfl_sync(BMASK, x, bsrc + 3), a0);
-                        a1 = fmaf(m1.x, __shfl_sync(BMASK, x, bsrc + 4), a1); a2 = fmaf(m1.y, __shfl_sync(BMASK, x, bsrc + 5), a2);
-                        a0 = fmaf(m1.z, __shfl_sync(BMASK, x, bsrc + 6), a0); a1 = fmaf(m1.w, __shfl_sync(BMASK, x, bsrc + 7), a1);
-                        a2 = fmaf(m2.x, __shfl_sync(BMASK, x, bsrc + 8), a2); a0 = fmaf(m2.y, __shfl_sync(BMASK, x, bsrc + 9), a0);
-                        a1 = fmaf(m2.z, __shfl_sync(BMASK, x, bsrc + 10), a1); a2 = fmaf(m2.w, __shfl_sync(BMASK, x, bsrc + 11), a2);
-                        x = a0 + (a1 + a2);
-                        if (e < Gv) sb[(c + 1) * 12 + bi] = x;
+                        const float4 *xv4 = reinterpret_cast<const float4 *>(sb + c * 12);
+                        const float4 x0 = xv4[0], x1 = xv4[1], x2 = xv4[2];
+                        float a0 = sb[(c + 1) * 12 + bi];
+                        float a1 = m0.y * x0.y, a2 = m0.z * x0.z;
+                        a0 = fmaf(m0.x, x0.x, a0); a0 = fmaf(m0.w, x0.w, a0);
+                        a1 = fmaf(m1.x, x1.x, a1); a2 = fmaf(m1.y, x1.y, a2); a0 = fmaf(m1.z, x1.z, a0); a1 = fmaf(m1.w, x1.w, a1);
+                        a2 = fmaf(m2.x, x2.x, a2); a0 = fmaf(m2.y, x2.y, a0); a1 = fmaf(m2.z, x2.z, a1); a2 = fmaf(m2.w, x2.w, a2);
+                        if (c < C - 2) { m0 = ps[c * 36]; m1 = ps[c * 36 + 1]; m2 = ps[c * 36 + 2]; }
+                        if (e < Gv) sb[(c + 1) * 12 + bi] = a0 + (a1 + a2);
+                        __syncwarp(BMASK);
                     }
                 }
             }
@@ -808,14 +799,19 @@ __global__ void __launch_bounds__(TM_THREADS, 1) k_iterate_tm(SolveParams P, Srb
                     float wv[6];
                     tm_ld6(tx + 6 * a, wv);
                     tm_wait_ld();
-                    if (act[a] && TM_ABL != 1) {
-                        if (emit) tm_stage_update<NU, true>(P, rb[a], nsl, bits[a], S[a].z, S[a].y, idt, m_dt, wv, !frozen, o.u + (tsb + sl[a]) * NU, res, two_feet[a]);
-                        else tm_stage_update<NU, false>(P, rb[a], nsl, bits[a], S[a].z, S[a].y, idt, m_dt, wv, !frozen, o.u + (tsb + sl[a]) * NU, res, two_feet[a]);
+                    if (((flags >> a) & 1) && TM_ABL != 1) {
+                        int slot = slot_w(a);
+                        asm volatile("" : "+r"(slot));             // opaque: no address of the stage record is hoisted out of the iteration loop
+                        const int bits = __float_as_int(recA4[6 * nsl + slot].w);
+                        const bool two = (flags >> (4 + a)) & 1;
+                        if (emit) tm_stage_update<NU, true>(P, recB4 + slot, nsl, bits, S[a].z, S[a].y, idt, m_dt, wv, !frozen,
+                                                            o.u + ((long)b0 * N + sl0 + jw + a) * NU, res, two);
+                        else tm_stage_update<NU, false>(P, recB4 + slot, nsl, bits, S[a].z, S[a].y, idt, m_dt, wv, !frozen, nullptr, res, two);
                     } else { wv[0] = wv[1] = wv[2] = wv[3] = wv[4] = wv[5] = 0.0f; }   // unused exchange vectors stay zero
                     tm_st6(tx + 6 * a, wv);
                     asm volatile("" ::: "memory");
                 }
-                if (emit && act[0] && !frozen) {
+                if (emit && (flags & 1) && !frozen) {
                     atomicMax(&red[eb * 5 + 0], __float_as_uint(res[0])); atomicMax(&red[eb * 5 + 1], __float_as_uint(res[1]));
                     atomicMax(&red[eb * 5 + 2], __float_as_uint(res[2])); atomicMax(&red[eb * 5 + 3], __float_as_uint(res[3]));
                     atomicMax(&red[eb * 5 + 4], __float_as_uint(res[4]));
@@ -844,21 +840,26 @@ __global__ void __launch_bounds__(TM_THREADS, 1) k_iterate_tm(SolveParams P, Srb
                 }
             }
         }
-#ifdef PINMPC_TM_TIMING
-        if (blockIdx.x == 0 && tid == 128)
-            printf("worker cycles/iter: update %lld | wait bwdA %lld | bnd-bwd %lld | wait bwdB+fwdA %lld | bnd-fwd %lld | wait fwdB %lld\n", tacc[0] / P.iters,
-                   tacc[1] / P.iters, tacc[2] / P.iters, tacc[3] / P.iters, tacc[4] / P.iters, tacc[5] / P.iters);
-#endif
 #pragma unroll
         for (int a = 0; a < WS; a++)
-            if (act[a]) {
-                float *oz = o.z + (tsb + sl[a]) * NU, *oy = o.y + (tsb + sl[a]) * NU;
+            if ((flags >> a) & 1) {
+                const long ts = (long)b0 * N + sl0 + jw + a;
+                float *oz = o.z + ts * NU, *oy = o.y + ts * NU;
 #pragma unroll
                 for (int j = 0; j < NU; j++) { oz[j] = S[a].z[j]; oy[j] = S[a].y[j]; }
             }
     }
     // ---- release tensor memory ---------------------------------------------------------------------------------
     tm_sync();
+#ifdef PINMPC_TM_TIMING
+    if (blockIdx.x == 0 && tid == 0) {
+        const int *t = ndone + 1;
+        printf("chain : (1)->bwdA start %d | bwdA %d | bnd %d | bwdB %d | fwdA %d | bnd %d | fwdB %d   total %d\n", 0, t[1] - t[0], t[2] - t[1], t[3] - t[2],
+               t[4] - t[3], t[5] - t[4], t[6] - t[5], t[6] - t[0]);
+        printf("worker: wait bwdA %d | bnd-bwd %d | wait bwdB+fwdA %d | bnd-fwd %d | wait fwdB %d | update %d   total %d\n", t[8] - t[7], t[9] - t[8],
+               t[10] - t[9], t[11] - t[10], t[12] - t[11], t[13] - t[12], t[13] - t[7]);
+    }
+#endif
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tbase));
 }
 
