@@ -29,16 +29,56 @@ if ROOT not in sys.path:
 
 METRIC = "batched ADMM-MPC solves/s at B=4096,N=50 (fixed iters); % of roofline"
 
-# Algorithmic FLOPs of the formulation shipped (structured 6-D-input LQR):
-FLOP_PER_STAGE_ITER = {12: 930.0, 18: 1150.0}     # one stage of one ADMM iteration
+# Algorithmic FLOPs of the formulation shipped (structured 6-D-input LQR): one stage of one ADMM
+# iteration without the wrench projections, plus 95 per foot in stance (the exact projection of one 6-D wrench; a swing
+# foot projects to 0 for free), counted from the workload's own contact flags
+FLOP_PER_STAGE_ITER_BASE = {12: 740.0, 18: 960.0}
+FLOP_PER_PROJECTION = 95.0
 FLOP_PER_STAGE_ONCE = {12: 3900.0, 18: 4700.0}    # assembly + factorisation, once per solve
 # dense-generic count of SURVEY.md 8(d), used when --method dense is timed
 FLOP_DENSE_ITER = {12: 2700.0, 18: 3700.0}
 FLOP_DENSE_ONCE = {12: 33000.0, 18: 60000.0}
 FMA_LANES_PER_SM = 128
-# DRAM bytes (read + write) of one k_iterate_srb launch at config 2 from the `ncu --set full` capture
-# summarised in profiles/r1_final_iterate_ncu.md (dram__bytes_read.sum + dram__bytes_write.sum)
-NCU_DRAM_BYTES_ITERATE = {"c2_long_horizon": 110317568 + 13498368}
+# DRAM bytes (read + write) of one launch of the dominant kernel from an `ncu --set full` capture: written by
+# `bench.py --write-traffic <ncu raw csv>` together with a hash of the kernel sources it was measured on; reported only
+# while that hash still matches the sources (else null)
+TRAFFIC_JSON = os.path.join(ROOT, "profiles", "r2_traffic.json")
+
+
+def source_hash():
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2606_05687_b200", "csrc")
+    for f in sorted(os.listdir(d)):
+        if f.endswith((".cu", ".cuh")):
+            h.update(open(os.path.join(d, f), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def measured_traffic(workload):
+    try:
+        t = json.load(open(TRAFFIC_JSON))
+    except (OSError, ValueError):
+        return None
+    return t.get("dram_bytes") if t.get("workload") == workload and t.get("source_hash") == source_hash() else None
+
+
+def write_traffic(csv_path, workload):
+    """Parse `ncu -i x.ncu-rep --page raw --csv` of the dominant kernel and record its DRAM traffic per launch."""
+    import csv
+    rows = list(csv.reader(open(csv_path)))
+    hdr, units, vals = rows[0], rows[1], rows[2]
+    col = {n: i for i, n in enumerate(hdr)}
+    mult = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+
+    def get(name):
+        return float(vals[col[name]].replace(",", "")) * mult[units[col[name]]]
+    out = {"workload": workload, "kernel": vals[col["Kernel Name"]], "source_hash": source_hash(),
+           "dram_bytes": get("dram__bytes_read.sum") + get("dram__bytes_write.sum"),
+           "dram_bytes_read": get("dram__bytes_read.sum"), "dram_bytes_write": get("dram__bytes_write.sum"),
+           "gpu_time_ms": float(vals[col["gpu__time_duration.sum"]].replace(",", "")) * {"ns": 1e-6, "us": 1e-3, "ms": 1.0}[units[col["gpu__time_duration.sum"]]]}
+    json.dump(out, open(TRAFFIC_JSON, "w"), indent=1)
+    print(json.dumps(out))
 
 
 def parse():
@@ -57,6 +97,9 @@ def parse():
                     help="time the paper's own stage-local ADMM (pinmpc_split_solve) on the config instead (one JSON line)")
     ap.add_argument("--split-sweep", action="store_true",
                     help="scalability table of the stage-local method like the paper's Fig. 3: envs x horizon up to N = 400")
+    ap.add_argument("--chunks", type=int, default=0, help="horizon chunks of the equality step (0 = auto, 1 = sequential-pass kernel)")
+    ap.add_argument("--write-traffic", default=None, metavar="NCU_RAW_CSV",
+                    help="record the DRAM traffic of the dominant kernel from an ncu raw-page csv into profiles/r2_traffic.json and exit")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -104,6 +147,15 @@ class ClockSampler:
                 "samples": len(sm)}
 
 
+def probe_fma(blocks, iters, d_out, stream):
+    """Bench-only helper library (csrc/bench_probe.cu): enqueue `blocks` CTAs x 256 threads x 128*iters FMAs, return the FLOPs."""
+    import ctypes
+    lib = ctypes.CDLL(os.path.join(ROOT, "paper_2606_05687_b200", "libpinmpc_benchprobe.so"))
+    lib.bench_probe_fma.restype = ctypes.c_double
+    lib.bench_probe_fma.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p]
+    return float(lib.bench_probe_fma(int(blocks), int(iters), ctypes.c_void_p(d_out.data_ptr()), ctypes.c_void_p(stream)))
+
+
 def max_over_ranks(values, dist, device):
     """Replicas only: the one collective of a multi-GPU run is this MAX of the per-rank
     step times; `value` is then (envs of all ranks) / (the slowest rank's time)."""
@@ -120,11 +172,17 @@ def aggregate_value(envs_per_rank, world, ms):
     return envs_per_rank * world / (ms * 1e-3)
 
 
+def flop_per_stage_iter(w):
+    """Algorithmic FLOPs of one stage of one ADMM iteration for this workload (projections counted per stance foot)."""
+    feet = float(w.contact[..., :2].astype("float64").sum() / (w.B * w.N))
+    return FLOP_PER_STAGE_ITER_BASE[w.nu] + FLOP_PER_PROJECTION * feet
+
+
 def flops_per_solve(w, method):
     st = w.B * w.N
     if method == "dense":
         return st * (FLOP_DENSE_ONCE[w.nu] + w.iters * FLOP_DENSE_ITER[w.nu])
-    return st * (FLOP_PER_STAGE_ONCE[w.nu] + w.iters * FLOP_PER_STAGE_ITER[w.nu])
+    return st * (FLOP_PER_STAGE_ONCE[w.nu] + w.iters * flop_per_stage_iter(w))
 
 
 def time_oracle(w, n_envs, threads=0):
@@ -319,6 +377,9 @@ def run_sweep(args):
 
 def main():
     args = parse()
+    if args.write_traffic:
+        import gen
+        return write_traffic(args.write_traffic, gen.make_config(args.config, B=args.B, N=args.N).name)
     if args.impl == "reference":
         return run_reference(args)
     if args.split:
@@ -354,6 +415,8 @@ def main():
     s.set_workload(w)
     if args.envs_per_cta:
         s.set_tuning(args.envs_per_cta)
+    if args.chunks:
+        s.set_horizon_chunks(args.chunks)
     stream = torch.cuda.current_stream(dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
 
@@ -498,8 +561,9 @@ def main():
             # dominant kernel = the iteration kernel: its own algorithmic FLOPs over its own duration (CUDA events
             # recorded by pinmpc_solve on the launching stream around the kernel, averaged over K launches)
             k_ms = [float(np.mean([k[i] for k in kernel_ms])) for i in range(3)]
-            fl = w.B * w.N * w.iters * FLOP_PER_STAGE_ITER[w.nu]
+            fl = w.B * w.N * w.iters * flop_per_stage_iter(w)
             achieved = fl / (k_ms[2] * 1e-3) / 1e12
+            G_used, C_used = s.launch_shape()
         else:
             k_ms = None
             achieved = fl / (ms * 1e-3) / 1e12                 # TFLOP/s of the whole step (dense variant)
@@ -513,11 +577,11 @@ def main():
         peak = props.multi_processor_count * FMA_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
         # measured FMA-pipe peak on this device (register-resident loop), for context
         scratch = torch.zeros(1, device=dev)
-        binding.pinmpc_probe_fma(props.multi_processor_count * 8, 2000, scratch, stream.cuda_stream)
+        probe_fma(props.multi_processor_count * 8, 2000, scratch, stream.cuda_stream)
         torch.cuda.synchronize(dev)
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         a.record(stream)
-        pf = binding.pinmpc_probe_fma(props.multi_processor_count * 8, 20000, scratch, stream.cuda_stream)
+        pf = probe_fma(props.multi_processor_count * 8, 20000, scratch, stream.cuda_stream)
         b.record(stream); torch.cuda.synchronize(dev)
         fma_meas = pf / (a.elapsed_time(b) * 1e-3) / 1e12
 
@@ -528,15 +592,18 @@ def main():
             "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": w.name, "B": w.B, "N": w.N, "iters": w.iters, "nu": w.nu, "rho": w.rho,
-                       "method": mname, "l2": "flushed (256 MiB write) between timed steps; per-step CUDA events",
+                       "method": mname, "horizon_chunks": (s.launch_shape()[1] if mname == "srb" else None), "l2": "flushed (256 MiB write) between timed steps; per-step CUDA events",
                        "multi_gpu": "replicas only (no collective on the data path)"},
             "stage_iters_per_s": total_solves * w.N * w.iters / (ms * 1e-3),
             "ms_min": float(np.min(ms_steps)), "ms_median": float(np.median(ms_steps)),
             "gpu_launches": launches,
             "clocks": clocks,
             "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                         "traffic": NCU_DRAM_BYTES_ITERATE.get(w.name),
-                         "kernel": "k_iterate_srb (S3-S6, all iterations)" if k_ms else "whole step",
+                         "traffic": measured_traffic(w.name) if k_ms else None,
+                         "kernel": (("k_iterate_tm (S3-S6, all iterations; chunked two-sweep equality step, gains in tensor memory)"
+                                     if C_used > 1 else "k_iterate_srb (S3-S6, all iterations; sequential passes)")
+                                    + f", {G_used} envs per CTA, {C_used} horizon chunks") if k_ms else "whole step",
+                         "flop_per_stage_iter": flop_per_stage_iter(w) if k_ms else None,
                          "kernel_ms": {"assemble": k_ms[0], "factor": k_ms[1], "iterate": k_ms[2]} if k_ms else None,
                          "whole_step_tflops": flops_per_solve(w, mname) / (ms * 1e-3) / 1e12,
                          "peak_source": f"{props.multi_processor_count} SMs x {FMA_LANES_PER_SM} FP32 lanes x 2 x "

@@ -39,7 +39,7 @@ extern "C" {
 #endif
 
 #define PINMPC_NX 13
-#define PINMPC_N_MAX 256
+#define PINMPC_N_MAX 512
 #define PINMPC_SPLIT_N_MAX 1024     /* the stage-local method has no per-horizon on-chip state (N to 400) */
 
 typedef struct pinmpc_ctx *pinmpc_t;
@@ -117,10 +117,11 @@ pinmpc_status pinmpc_set_tuning(pinmpc_t h, int envs_per_cta);
 /* How the equality step (S3) is parallelised across the horizon (north_star (2); PAPER.md:L206-208 Remark 2,
  * L23): the N stages are cut into `chunks` chunks that are swept concurrently (chunked two-sweep over the
  * time-varying LQR recursion, gains resident in tensor memory).
- *   0 (default) = ceil(N / 6) chunks when the shape fits the chunked kernel, else sequential passes;
+ *   0 (default) = ceil(N / L) chunks, L = 6 (nu = 12) or 4 (nu = 18), when the shape fits the chunked kernel, else
+ *                 sequential passes;
  *   1           = the sequential-pass kernel (two N-step recursions per iteration);
- *   >= 2        = that many chunks; PINMPC_EUNSUPPORTED unless ceil(N / chunks) <= 6, chunks <= 128 and
- *                 chunks <= ceil(N / 4) (room for the chunk operators in the workspace).
+ *   >= 2        = that many chunks; PINMPC_EUNSUPPORTED unless ceil(N / chunks) <= L, chunks <= 128 and
+ *                 chunks <= ceil(N / (L - 1)) (room for the chunk operators in the workspace).
  * Results agree to rounding for every setting. */
 pinmpc_status pinmpc_set_horizon_chunks(pinmpc_t h, int chunks);
 
@@ -152,7 +153,8 @@ pinmpc_status pinmpc_set_problem(pinmpc_t h, const pinmpc_problem *p);
 pinmpc_status pinmpc_set_dynamics(pinmpc_t h, const float *A, const float *Bm, const float *c);
 
 /* One batched solve: assembly (S1) + factorisation (S2) + iters x (equality step S3, projection
- * S4, dual update S5, residuals / early exit S6), cold start z = y = 0.  Asynchronous on `stream`. */
+ * S4, dual update S5, residuals / early exit S6), from z = y = 0 or from the values given to pinmpc_set_warm_start.
+ * Asynchronous on `stream`. */
 pinmpc_status pinmpc_solve(pinmpc_t h, void *stream);
 
 /* Copy results of the last solve into caller DEVICE buffers (any may be NULL), asynchronously on
@@ -176,11 +178,14 @@ pinmpc_status pinmpc_shift_aux(pinmpc_t h, int shift, float *z0, float *y0, void
  * A [B,N,nx,nx], Bm [B,N,nx,nu], c [B,N,nx] (any may be NULL); runs the assembly kernel on `stream`. */
 pinmpc_status pinmpc_get_dynamics(pinmpc_t h, float *A, float *Bm, float *c, void *stream);
 
-/* Measurement aid, not part of the solve path: enqueue a register-resident FP32 FMA loop
- * (`blocks` CTAs x 256 threads x 128*iters FMAs) on `stream` and return the FLOPs it performs
- * (0 on a launch error).  bench.py times it with CUDA events to report the measured FMA-pipe peak
- * next to the roofline.  d_out: one float of device scratch. */
-double pinmpc_probe_fma(int blocks, int iters, float *d_out, void *stream);
+/* Test hook of the product's dynamics assembly (S1, the structured solver never forms A_k, B_k): runs the assembly
+ * kernel of the structured solver on the current problem and expands ITS per-stage records (cos/sin of the yaw,
+ * I_w, contact offsets, c_k rows, mass) back into dense A [B,N,nx,nx], Bm [B,N,nx,nu] (= E D_k Gh_k, SRB form of
+ * PAPER.md:L49-57 eq. (2)-(4)) and c [B,N,nx]; S [B,N,21] is the stored packed upper triangle of
+ * S_k = (Bh_k Rt^-1 Bh_k^T)^-1 (Bh_k = rows 6..11 of B_k, Rt = R + rho I) and Tinv [B,N,6] the packed inverse of
+ * the Schur complement T_k of the torque block of Gh_k Rt^-1 Gh_k^T.  DEVICE buffers, any may be NULL; asynchronous
+ * on `stream`; the workspace's factor arrays are overwritten (call before, not between, solve and get). */
+pinmpc_status pinmpc_get_srb_assembly(pinmpc_t h, float *A, float *Bm, float *c, float *S, float *Tinv, void *stream);
 
 /* Number of kernel launches the last pinmpc_solve enqueued (for bench.py's gpu_launches). */
 int pinmpc_last_launch_count(pinmpc_t h);

@@ -23,8 +23,8 @@ _STATUS = {0: "PINMPC_OK", 1: "PINMPC_EINVAL", 2: "PINMPC_EALLOC", 3: "PINMPC_EC
 
 EXPORTS = ("pinmpc_workspace_bytes", "pinmpc_workspace_bytes_method", "pinmpc_create", "pinmpc_set_weights",
            "pinmpc_set_tolerance", "pinmpc_set_method", "pinmpc_set_tuning", "pinmpc_set_horizon_chunks", "pinmpc_get_launch_shape", "pinmpc_set_problem", "pinmpc_set_dynamics", "pinmpc_solve",
-           "pinmpc_get", "pinmpc_get_aux", "pinmpc_get_dynamics", "pinmpc_last_launch_count", "pinmpc_last_error",
-           "pinmpc_destroy", "pinmpc_probe_fma", "pinmpc_set_profiling", "pinmpc_get_kernel_ms",
+           "pinmpc_get", "pinmpc_get_aux", "pinmpc_get_dynamics", "pinmpc_get_srb_assembly", "pinmpc_last_launch_count", "pinmpc_last_error",
+           "pinmpc_destroy", "pinmpc_set_profiling", "pinmpc_get_kernel_ms",
            "pinmpc_set_warm_start", "pinmpc_shift_aux", "pinmpc_landmark_ring_bytes", "pinmpc_landmark_reset", "pinmpc_landmark_push",
            "pinmpc_landmark_push_solver", "pinmpc_landmark_reward", "pinmpc_split_workspace_bytes", "pinmpc_split_solve")
 MAX_LANDMARKS = 8
@@ -98,12 +98,12 @@ def load():
     lib.pinmpc_get_aux.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p]
     lib.pinmpc_get_dynamics.restype = c_int
     lib.pinmpc_get_dynamics.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]
+    lib.pinmpc_get_srb_assembly.restype = c_int
+    lib.pinmpc_get_srb_assembly.argtypes = [c_void_p] + [c_void_p] * 6
     lib.pinmpc_last_launch_count.restype = c_int
     lib.pinmpc_last_launch_count.argtypes = [c_void_p]
     lib.pinmpc_last_error.restype = c_char_p
     lib.pinmpc_last_error.argtypes = [c_void_p]
-    lib.pinmpc_probe_fma.restype = ctypes.c_double
-    lib.pinmpc_probe_fma.argtypes = [c_int, c_int, c_void_p, c_void_p]
     lib.pinmpc_set_warm_start.restype = c_int
     lib.pinmpc_set_warm_start.argtypes = [c_void_p, c_void_p, c_void_p]
     lib.pinmpc_set_profiling.restype = c_int
@@ -239,8 +239,8 @@ def pinmpc_get_kernel_ms(h):
     return [float(v) for v in ms]
 
 
-def pinmpc_probe_fma(blocks, iters, d_out, stream=0) -> float:
-    return float(load().pinmpc_probe_fma(int(blocks), int(iters), _ptr(d_out), c_void_p(stream)))
+def pinmpc_get_srb_assembly(h, A, Bm, c, S, Tinv, stream=0):
+    _check(load().pinmpc_get_srb_assembly(h, _ptr(A), _ptr(Bm), _ptr(c), _ptr(S), _ptr(Tinv), c_void_p(stream)), h)
 
 
 def pinmpc_destroy(h):
@@ -388,6 +388,15 @@ class Solver:
         c = t.empty((B, N, NX), dtype=t.float32, device=self.device)
         pinmpc_get_dynamics(self.h, A, Bm, c, self._stream(stream))
         return A, Bm, c
+
+    def get_srb_assembly(self, stream=None):
+        """A, Bm, c expanded from the structured solver's own assembly records, plus its S [B,N,21] and Tinv [B,N,6]."""
+        t = self.torch
+        B, N, nu = self.B, self.N, self.nu
+        mk = lambda *shape: t.empty(shape, dtype=t.float32, device=self.device)
+        A, Bm, c, S, Ti = mk(B, N, NX, NX), mk(B, N, NX, nu), mk(B, N, NX), mk(B, N, 21), mk(B, N, 6)
+        pinmpc_get_srb_assembly(self.h, A, Bm, c, S, Ti, self._stream(stream))
+        return A, Bm, c, S, Ti
 
     def close(self):
         if getattr(self, "h", None) is not None:

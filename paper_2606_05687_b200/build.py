@@ -8,7 +8,10 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpinmpc.so")
-SOURCES = ["pinmpc_api.cu", "pinmpc_dense.cu", "pinmpc_srb.cu", "pinmpc_tmem.cu", "pinmpc_probe.cu", "pinmpc_landmarks.cu", "pinmpc_split.cu"]
+SOURCES = ["pinmpc_api.cu", "pinmpc_dense.cu", "pinmpc_srb.cu", "pinmpc_tmem.cu", "pinmpc_landmarks.cu", "pinmpc_split.cu"]
+# bench-only helper (a register-resident FMA loop that measures the FP32 peak): its own library, not part of the product ABI
+PROBE_SRC = "bench_probe.cu"
+PROBE_LIB = os.path.join(HERE, "libpinmpc_benchprobe.so")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"] + os.environ.get("PINMPC_NVCC_EXTRA", "").split()
 
@@ -42,9 +45,12 @@ def build(force: bool = False, verbose: bool = False) -> str:
     tmp = LIB + f".tmp{os.getpid()}"
     subprocess.check_call([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", tmp] + objs + ["-lcudart"])
     os.replace(tmp, LIB)
-    with open(os.path.join(CSRC, "ptxas_v.log"), "w") as f:
-        # without ptxas' wall-clock lines, so that the committed log changes only when the code does
-        f.write("\n".join(l for l in "\n".join(log).splitlines() if "Compile time" not in l) + "\n")
+    tmp = PROBE_LIB + f".tmp{os.getpid()}"
+    subprocess.check_call([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-shared", "-Xcompiler", "-fPIC", "-o", tmp,
+                           os.path.join(CSRC, PROBE_SRC), "-lcudart"])
+    os.replace(tmp, PROBE_LIB)
+    with open(LIB.replace(".so", ".ptxas.log"), "w") as f:      # register / spill report of the build (git-ignored)
+        f.write("\n".join(log) + "\n")
     if verbose:
         print("\n".join(log))
     return LIB

@@ -1,6 +1,6 @@
-// pinmpc_probe.cu — a register-resident FP32 FMA loop used by bench.py to MEASURE the FMA-pipe
+// bench_probe.cu — a register-resident FP32 FMA loop used by bench.py to MEASURE the FMA-pipe
 // peak of the device the solver runs on (the denominator context for the "alu" roofline; SURVEY.md
-// 8(d)).  Not part of the solve path.
+// 8(d)).  Built as its own helper library (libpinmpc_benchprobe.so); not part of libpinmpc.so or its ABI.
 #include <cuda_runtime.h>
 
 __global__ void __launch_bounds__(256) k_probe_fma(int iters, float a, float b, float *out)
@@ -21,7 +21,7 @@ __global__ void __launch_bounds__(256) k_probe_fma(int iters, float a, float b, 
 
 // Enqueue the probe: `blocks` CTAs of 256 threads, each thread 128 * iters FMAs.
 // Returns the number of FLOPs the launch performs (2 per FMA), or 0 on a launch error.
-extern "C" double pinmpc_probe_fma(int blocks, int iters, float *d_out, void *stream)
+extern "C" double bench_probe_fma(int blocks, int iters, float *d_out, void *stream)
 {
     k_probe_fma<<<blocks, 256, 0, (cudaStream_t)stream>>>(iters, 0.999f, 0.001f, d_out);
     if (cudaGetLastError() != cudaSuccess) return 0.0;

@@ -23,7 +23,7 @@ static void srb_sizes(int nu, int N, int B, size_t *f)
     size_t st = (size_t)B * N;
     f[0] = st * 72; f[1] = (size_t)B * (N + 1) * 12; f[2] = st * 6; f[3] = st * 2; f[4] = st * 21;
     f[5] = st * PINMPC_RA_W; f[6] = st * (size_t)pinmpc_rb_width(nu);
-    f[7] = (size_t)B * pinmpc_psi_cap(N) * 144;
+    f[7] = (size_t)B * pinmpc_psi_cap(N, nu) * 144;
 }
 
 size_t pinmpc_ws_srb_bytes(int nu, int N, int B)
@@ -82,7 +82,7 @@ extern "C" pinmpc_status pinmpc_create(pinmpc_t *out, int nx, int nu, int N, int
     *out = nullptr;
     pinmpc_status why = PINMPC_OK;
     if (!sizes_ok(nx, nu, N, B, layout, &why))
-        return set_err(nullptr, why, "pinmpc_create: unsupported or invalid sizes (nx=13, nu in {12,18}, 1<=N<=256, B>=1)");
+        return set_err(nullptr, why, "pinmpc_create: unsupported or invalid sizes (nx=13, nu in {12,18}, 1<=N<=512, B>=1)");
     if (!(rho > 0.0f) || iters < 1) return set_err(nullptr, PINMPC_EINVAL, "pinmpc_create: rho must be > 0 and iters >= 1");
     if (!(layout->mu > 0.0f) || !(layout->fz_max > 0.0f) || !(layout->mx_coef > 0.0f) || !(layout->my_coef > 0.0f) ||
         !(layout->mz_coef > 0.0f) || (layout->n_force > 0 && !(layout->hand_fmax >= 0.0f)))
@@ -129,7 +129,7 @@ extern "C" pinmpc_status pinmpc_create(pinmpc_t *out, int nx, int nu, int N, int
         h->srb.Kh = (float *)take(f[0] * 4); h->srb.qv = (float *)take(f[1] * 4); h->srb.c6 = (float *)take(f[2] * 4);
         h->srb.cs = (float *)take(f[3] * 4); h->srb.MI = (float *)take(f[4] * 4);
         h->srb.RA = (float *)take(f[5] * 4); h->srb.RB = (float *)take(f[6] * 4);
-        h->psi = (float *)take(f[7] * 4); h->psi_cap = pinmpc_psi_cap(N);
+        h->psi = (float *)take(f[7] * 4); h->psi_cap = pinmpc_psi_cap(N, nu);
     }
     if (workspace_bytes >= pinmpc_ws_dense_bytes(nu, N, B)) {
         h->dA = (float *)take(st * NX * NX * 4);
@@ -199,7 +199,7 @@ extern "C" pinmpc_status pinmpc_set_horizon_chunks(pinmpc_t h, int chunks)
         t.chunks = chunks; t.envs_per_cta = 0;
         int G, C;
         if (!pinmpc_tm_config(&t, &G, &C))
-            return set_err(h, PINMPC_EUNSUPPORTED, "pinmpc_set_horizon_chunks: needs ceil(N / chunks) <= 6, chunks <= 128 and chunks - 2 <= ceil(N / 4) - 2");
+            return set_err(h, PINMPC_EUNSUPPORTED, "pinmpc_set_horizon_chunks: needs ceil(N / chunks) <= 6 (4 at nu = 18), chunks <= 128 and chunks <= ceil(N / 5) (ceil(N / 3) at nu = 18)");
     }
     h->chunks = chunks;
     return PINMPC_OK;
@@ -344,6 +344,15 @@ extern "C" pinmpc_status pinmpc_get_dynamics(pinmpc_t h, float *A, float *Bm, fl
     if (!h->have_problem || !raw_inputs_present(h)) return set_err(h, PINMPC_ESTATE, "pinmpc_get_dynamics: set_problem with raw inputs first");
     if (!A && !Bm && !c) return PINMPC_OK;
     int n = pinmpc_launch_assemble_dense(h, A, Bm, c, (cudaStream_t)stream);
+    return n < 0 ? PINMPC_ECUDA : PINMPC_OK;
+}
+
+extern "C" pinmpc_status pinmpc_get_srb_assembly(pinmpc_t h, float *A, float *Bm, float *c, float *S, float *Tinv, void *stream)
+{
+    if (!h) return PINMPC_EINVAL;
+    if (h->sticky != cudaSuccess) return PINMPC_ECUDA;
+    if (!h->have_problem || !raw_inputs_present(h)) return set_err(h, PINMPC_ESTATE, "pinmpc_get_srb_assembly: set_problem with raw inputs first");
+    int n = pinmpc_launch_srb_assembly_debug(h, A, Bm, c, S, Tinv, (cudaStream_t)stream);
     return n < 0 ? PINMPC_ECUDA : PINMPC_OK;
 }
 

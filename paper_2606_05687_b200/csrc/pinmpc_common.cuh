@@ -103,11 +103,13 @@ size_t pinmpc_ws_dense_bytes(int nu, int N, int B);
 int pinmpc_launch_assemble_dense(pinmpc_ctx *h, float *A, float *Bm, float *c, cudaStream_t st);
 int pinmpc_launch_solve_dense(pinmpc_ctx *h, cudaStream_t st);
 int pinmpc_launch_solve_srb(pinmpc_ctx *h, cudaStream_t st);
+int pinmpc_launch_srb_assembly_debug(pinmpc_ctx *h, float *A, float *Bm, float *c, float *S, float *Tinv, cudaStream_t st);
 size_t pinmpc_ws_srb_bytes(int nu, int N, int B);
 // chunked, TMEM-resident iteration kernel (pinmpc_tmem.cu)
 bool pinmpc_tm_config(const pinmpc_ctx *h, int *G, int *C);
 int pinmpc_launch_iterate_tm(pinmpc_ctx *h, int G, int C, cudaStream_t st);
-inline int pinmpc_psi_cap(int N) { int c = (N + 3) / 4 - 2; return c > 0 ? c : 0; }
+// chunk operators of up to ceil(N / 5) chunks (nu = 12: 5 or 6 stages per chunk), ceil(N / 3) chunks (nu = 18: 3 or 4)
+inline int pinmpc_psi_cap(int N, int nu) { int c = (nu == 12 ? (N + 4) / 5 : (N + 2) / 3) - 2; return c > 0 ? c : 0; }
 
 static inline SolveParams make_params(const pinmpc_ctx *h)
 {

@@ -19,11 +19,12 @@
 // Three kernels per solve:
 //   k_assemble_srb  S1   one thread per (env, stage): geometry, Lam^-1, S, R ubar, Q xbar, ch
 //   k_factor_srb    S2   one warp per env: the 13-state Riccati recursion in the 6-D input
-//   k_iterate_srb   S3-6 one CTA per G envs, all ADMM iterations with every factor on chip:
-//                        Kh and the exchange vectors in shared memory, the per-stage symmetric blocks,
-//                        z and y in the registers of the thread that owns the stage (lane = stage);
-//                        the two sequential passes run in warp 0, 8 lanes per env.
-#include "pinmpc_common.cuh"
+//   k_iterate_srb   S3-6 the SEQUENTIAL-PASS iteration kernel (pinmpc_set_horizon_chunks(h, 1), and the fallback for
+//                        shapes the chunked kernel of pinmpc_tmem.cu cannot hold): one CTA per G envs, all ADMM
+//                        iterations with Kh and the exchange vectors in shared memory; PW pass warps run the two
+//                        N-step recursions (six lanes per env, five envs per warp), the stage threads own two
+//                        stages each with z, y in registers and stream the stage records from L2.
+#include <mutex>
 
 #include "pinmpc_srb_math.cuh"
 
@@ -1055,9 +1056,16 @@ int launch_t(pinmpc_ctx *h, cudaStream_t st)
         }
         const int threads = iterate_threads(h->N, G), PW = (G + PASS_ENVS - 1) / PASS_ENVS;
         const size_t smem = iterate_smem_bytes(h->N, G, ext, h->nu);
-        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
-        if (e != cudaSuccess) return fail(h, "k_iterate_srb smem attribute", e);
+        // the attributes are process-global per kernel: set once to the device maximum (never per solve, so that handles
+        // used from different host threads cannot race between setting and launching)
+        static std::once_flag once[2];
+        static cudaError_t once_err[2];
+        const int wi = q.z0 ? 1 : 0;
+        std::call_once(once[wi], [&] {
+            once_err[wi] = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem_optin);
+            if (once_err[wi] == cudaSuccess) once_err[wi] = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+        });
+        if (once_err[wi] != cudaSuccess) return fail(h, "k_iterate_srb smem attribute", once_err[wi]);
         kern<<<(unsigned)((h->B + G - 1) / G), threads, smem, st>>>(P, h->srb, q.x0, q.mass, h->out, G, PW, ext, q.z0, q.y0);
         e = cudaGetLastError();
         if (e != cudaSuccess) return fail(h, "k_iterate_srb launch", e);
@@ -1069,6 +1077,84 @@ int launch_t(pinmpc_ctx *h, cudaStream_t st)
 }
 
 }  // namespace
+
+// ---------------------------------------------------------------------------------------------
+// Test hook of S1 (pinmpc_get_srb_assembly): run the product's assembly kernel and expand ITS records
+// (cos sin, I_w, r, ch, mass) back into dense A_k, B_k = E D_k Gh_k, c_k, next to S_k and T_k^-1 as stored.
+// ---------------------------------------------------------------------------------------------
+namespace {
+template <int NU>
+__global__ void __launch_bounds__(128) k_srb_expand(SolveParams P, SrbWs W, const float *__restrict__ massg, int has_ext, float *A, float *Bm,
+                                                    float *c, float *S, float *Tinv)
+{
+    constexpr int NC = NW + (NU - 12) / 3;
+    const long st = (long)P.B * P.N;
+    const long s = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= st) return;
+    const int b = (int)(s / P.N);
+    const float dt = P.dt, dtm = dt / massg[b];
+    float rec[pinmpc_rb_width(NU)];
+    for (int w = 0; w < pinmpc_rb_width(NU); w++) rec[w] = W.RB[pinmpc_rec_index(w, st, s)];
+    const float Iw[9] = { rec[6], rec[7], rec[8], rec[7], rec[9], rec[10], rec[8], rec[10], rec[11] };
+    float Wi[9];
+    inv3f(Iw, Wi);
+    if (A) {
+        float *a = A + s * NX * NX;
+        for (int i = 0; i < NX * NX; i++) a[i] = 0.0f;
+        for (int i = 0; i < NX; i++) a[i * NX + i] = 1.0f;
+        const float cs = W.cs[s * 2], sn = W.cs[s * 2 + 1];
+        a[0 * NX + 6] = dt * cs; a[0 * NX + 7] = dt * sn; a[1 * NX + 6] = -dt * sn; a[1 * NX + 7] = dt * cs; a[2 * NX + 8] = dt;   // dt R_z^T
+        for (int i = 0; i < 3; i++) a[(3 + i) * NX + 9 + i] = dt;
+        a[11 * NX + 12] = dt;
+    }
+    if (Bm) {
+        float *bm = Bm + s * NX * NU;
+        for (int i = 0; i < NX * NU; i++) bm[i] = 0.0f;
+        for (int i = 0; i < NC; i++) {
+            const float rx = rec[12 + 3 * i], ry = rec[13 + 3 * i], rz = rec[14 + 3 * i];
+            const float X[9] = { 0.0f, -rz, ry, rz, 0.0f, -rx, -ry, rx, 0.0f };                 // [r]x
+            const int fc = fcol(i);
+            for (int x = 0; x < 3; x++)
+                for (int y = 0; y < 3; y++) {
+                    float acc = 0.0f;
+                    for (int l = 0; l < 3; l++) acc = fmaf(Wi[x * 3 + l], X[l * 3 + y], acc);
+                    bm[(6 + x) * NU + fc + y] = dt * acc;
+                    if (i < NW) bm[(6 + x) * NU + mcol(i) + y] = dt * Wi[x * 3 + y];
+                }
+            for (int x = 0; x < 3; x++) bm[(9 + x) * NU + fc + x] = dtm;
+        }
+    }
+    if (c) {
+        float *cc = c + s * NX;
+        for (int i = 0; i < NX; i++) cc[i] = 0.0f;
+        if (has_ext)
+            for (int i = 0; i < 6; i++) cc[6 + i] = W.c6[s * 6 + i];
+    }
+    if (S)
+        for (int i = 0; i < 21; i++) S[s * 21 + i] = W.MI[(long)i * st + s];
+    if (Tinv)
+        for (int i = 0; i < 6; i++) Tinv[s * 6 + i] = rec[i];
+}
+}  // namespace
+
+int pinmpc_launch_srb_assembly_debug(pinmpc_ctx *h, float *A, float *Bm, float *c, float *S, float *Tinv, cudaStream_t st)
+{
+    SolveParams P = make_params(h);
+    ProblemPtrs q = make_problem_ptrs(h);
+    const long stages = (long)h->B * h->N;
+    const unsigned blocks = (unsigned)((stages + 127) / 128);
+    const int ext = q.ext != nullptr;
+    if (h->nu == 12) {
+        k_assemble_srb<12><<<blocks, 128, 0, st>>>(P, q, h->srb);
+        k_srb_expand<12><<<blocks, 128, 0, st>>>(P, h->srb, q.mass, ext, A, Bm, c, S, Tinv);
+    } else {
+        k_assemble_srb<18><<<blocks, 128, 0, st>>>(P, q, h->srb);
+        k_srb_expand<18><<<blocks, 128, 0, st>>>(P, h->srb, q.mass, ext, A, Bm, c, S, Tinv);
+    }
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(h, "k_srb_expand launch", e);
+    return 2;
+}
 
 int pinmpc_launch_solve_srb(pinmpc_ctx *h, cudaStream_t st)
 {

@@ -27,6 +27,8 @@
 // each: u from w, the exact projection (S4), the dual update (S5), residuals (S6) and sigma0 of the next
 // iteration, with the stage constants (Mh^-1, kg, T^-1, I_w, r, R ubar) in shared memory — nothing streams from
 // L2 after the prologue.
+#include <mutex>
+
 #include "pinmpc_srb_math.cuh"
 
 namespace {
@@ -35,7 +37,10 @@ namespace {
 #define TM_ABL 0
 #endif
 
-constexpr int TM_LMAX = 6;                         // stages per chunk
+constexpr int TM_LMAX = 6;                         // stages per chunk (tensor-memory columns: 6 x 72 gains + exchange + ch)
+// stages per chunk actually used: a worker owns half of them with z, y in registers (2 x nu floats per stage), which at
+// nu = 18 leaves room for two stages per worker only
+__host__ __device__ constexpr int tm_lmax(int nu) { return nu == 12 ? 6 : 4; }
 constexpr int TM_XOFF = TM_LMAX * 72;              // exchange vectors   [LMAX][6]   columns 432..467
 constexpr int TM_COFF = TM_XOFF + TM_LMAX * 6;     // ch (ext only)      [LMAX][6]   columns 468..503
 constexpr int TM_CHAINS = 128;                     // chain threads = TMEM lanes
@@ -680,7 +685,7 @@ __global__ void __launch_bounds__(TM_THREADS, 1) k_iterate_tm(SolveParams P, Srb
         tm_chain_main<RBW>(A);
     } else {
         // =========================== WORKER WARPS ==================================================================
-        constexpr int WS = TM_LMAX / 2;                          // stages per worker
+        constexpr int WS = tm_lmax(NU) / 2;                      // stages per worker
         const int ws = (warp - 4) >> 2;
         // Few values stay live across an iteration next to z, y of the three owned stages: everything per stage (slot,
         // contact bits, activity) is recomputed where it is used (a spilled value costs an L2 round trip here).
@@ -880,8 +885,9 @@ size_t pinmpc_tm_smem_bytes(int N, int G, int C, int nu) { return (size_t)tm_lay
 bool pinmpc_tm_config(const pinmpc_ctx *h, int *Gout, int *Cout)
 {
     const int N = h->N;
-    int C = h->chunks > 1 ? h->chunks : (N + TM_LMAX - 1) / TM_LMAX;
-    if (C < 1 || (N + C - 1) / C > TM_LMAX || C > N || C > TM_CHAINS || C - 2 > h->psi_cap) return false;
+    const int lmax = tm_lmax(h->nu);
+    int C = h->chunks > 1 ? h->chunks : (N + lmax - 1) / lmax;
+    if (C < 1 || (N + C - 1) / C > lmax || C > N || C > TM_CHAINS || C - 2 > h->psi_cap) return false;
     int best = 0;
     long best_rounds = 0;
     for (int G = 1; G <= TM_GMAX; G++) {
@@ -913,8 +919,12 @@ static int tm_launch_t(pinmpc_ctx *h, const SolveParams &P, const ProblemPtrs &q
     }
     auto kern = q.z0 ? k_iterate_tm<NU, true> : k_iterate_tm<NU, false>;
     const size_t smem = pinmpc_tm_smem_bytes(h->N, G, C, h->nu);
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem_optin - 256);
-    if (e != cudaSuccess) return tm_fail(h, "k_iterate_tm smem attribute", e);
+    static std::once_flag once[2];                             // process-global attribute: set once, not per solve
+    static cudaError_t once_err[2];
+    const int wi = q.z0 ? 1 : 0;
+    std::call_once(once[wi], [&] { once_err[wi] = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem_optin - 256); });
+    if (once_err[wi] != cudaSuccess) return tm_fail(h, "k_iterate_tm smem attribute", once_err[wi]);
+    cudaError_t e;
     kern<<<(unsigned)((h->B + G - 1) / G), TM_THREADS, smem, st>>>(P, h->srb, h->psi, q.x0, q.mass, h->out, G, C, ext, q.z0, q.y0);
     e = cudaGetLastError();
     if (e != cudaSuccess) return tm_fail(h, "k_iterate_tm launch", e);

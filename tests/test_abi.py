@@ -38,14 +38,15 @@ def test_host_only_entry_points_without_a_gpu(lib):
     base = binding.pinmpc_workspace_bytes(13, 12, 50, 4096, lay)
     dense = binding.pinmpc_workspace_bytes(13, 12, 50, 4096, lay, binding.METHOD_DENSE)
     st = 4096 * 50
-    # outputs x,u,z,y (13 + 36 floats per stage) + the structured solver's factors (175 per stage + q_0)
+    # outputs x,u,z,y (13 + 36 floats per stage) + the structured solver's factors (175 per stage + q_0) + the chunk
+    # operators of the chunked iteration kernel (ceil(N / 5) - 2 = 8 matrices of 144 floats per env)
     per_stage = (13 + 36) + (72 + 12 + 6 + 2 + 21 + 28 + 32)
-    lo = (st * per_stage + 4096 * 12) * 4
+    lo = (st * per_stage + 4096 * 12 + 4096 * 8 * 144) * 4
     assert base >= lo and base < lo + 20 * 256 + 3 * 4096 * 4
     assert dense > base + st * (169 + 156 + 156 + 144) * 4
     assert binding.pinmpc_workspace_bytes(12, 12, 50, 64, lay) == 0          # nx must be 13
     assert binding.pinmpc_workspace_bytes(13, 14, 50, 64, lay) == 0          # nu must match the layout
-    assert binding.pinmpc_workspace_bytes(13, 12, 257, 64, lay) == 0         # N_MAX
+    assert binding.pinmpc_workspace_bytes(13, 12, 513, 64, lay) == 0         # N_MAX
     assert binding.pinmpc_workspace_bytes(13, 12, 10, 0, lay) == 0           # empty batch
     assert binding.pinmpc_workspace_bytes(13, 12, 0, 4, lay) == 0            # empty horizon
     assert binding.pinmpc_workspace_bytes(13, 18, 30, 64, binding.make_layout(2, 2)) > 0

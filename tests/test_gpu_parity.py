@@ -42,13 +42,21 @@ def run_gpu(w, method="srb", iters=None, rho=None, tol=None, dynamics=None):
     return res
 
 
+# Absolute floor of the residual comparison per unit of (1 + |u|_inf) (reading D15): r_prim = max|u - z| is a
+# difference of O(|u|) float32 numbers, so its absolute error is a few ulp of |u| whatever its own size.
+RES_FLOOR = 5e-5
+WORST_RES = {"r_prim": -1.0, "r_dual": -1.0}
+
+
 def check_parity(w, got, ref, envs=None):
     """got: GPU outputs for all envs of w (or for `envs`); ref: oracle outputs for `envs`."""
     sel = slice(None) if envs is None else envs
     u = got["u"][sel].astype(np.float64); x = got["x"][sel].astype(np.float64)
     ax = tuple(range(1, u.ndim))
     du = np.abs(u - ref["u"]).max(axis=ax); dx = np.abs(x - ref["x"]).max(axis=ax)
-    un = np.minimum(np.abs(ref["u"]).max(axis=ax), np.abs(w.u_ref[sel]).max(axis=ax))
+    un = np.abs(ref["u"]).max(axis=ax)
+    if w.u_ref is not None:                         # (u_ref = NULL: there is no tracking reference to take the norm of)
+        un = np.minimum(un, np.abs(w.u_ref[sel]).max(axis=ax))
     xn = np.minimum(np.abs(ref["x"]).max(axis=ax), np.abs(w.x_ref[sel]).max(axis=ax))
     tol_u = 1e-3 * (1 + un); tol_x = 1e-4 * (1 + xn)
     worst_u = np.max(du / tol_u); worst_x = np.max(dx / tol_x)
@@ -57,10 +65,13 @@ def check_parity(w, got, ref, envs=None):
     # residuals: 1e-3 relative (north_star) plus an absolute floor (reading D15).  r_prim = max|u - z|
     # is a difference of O(|u|) fp32 numbers, so it inherits the ABSOLUTE error of u and z, which
     # north_star itself allows to be 1e-3 (1 + |u|); the floor is 1/20 of that allowance.
-    floor = 0.05 * 1e-3 * (1 + np.abs(ref["u"]).max(axis=ax))
+    floor = RES_FLOOR * (1 + np.abs(ref["u"]).max(axis=ax))
     for name in ("r_prim", "r_dual"):
         r = got[name][sel].astype(np.float64)
-        assert np.all(np.abs(r - ref[name]) <= 1e-3 * ref[name] + floor), name
+        err = np.abs(r - ref[name])
+        # measured excess over the relative bar, in units of (1 + |u|_inf): what the floor has to cover
+        WORST_RES[name] = max(WORST_RES[name], float(np.max((err - 1e-3 * ref[name]) / (1 + np.abs(ref["u"]).max(axis=ax)))))
+        assert np.all(err <= 1e-3 * ref[name] + floor), (name, float(np.max(err / (1e-3 * ref[name] + floor))))
     assert np.array_equal(got["iters_done"][sel], ref["iters_done"])
     # z and y are not part of north_star's bar.  Both live in the units of u (y accumulates u - z every
     # iteration, so it inherits u's absolute rounding error), hence both get u's allowance.
