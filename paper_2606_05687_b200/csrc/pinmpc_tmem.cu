@@ -554,6 +554,94 @@ __device__ __noinline__ void tm_chain_main(ChainArgs A)
     }
 }
 
+// Prologue of a chain thread: the gains of its chunk -> its lane of tensor memory, row-major Kn[r][0..11] = -Kh[r][.]
+// (Kh arrives as the pairs (Kh[r][j], Kh[r][6+j])), and the chunk's ch rows.  Its own function: the 36 loads in flight
+// per trip must not count against the register allocation of the kernel body.
+__device__ __noinline__ void tm_chain_load(const float *__restrict__ Kh, const float *__restrict__ c6, int clen, uint32_t myt)
+{
+    for (int j0 = 0; j0 < TM_LMAX; j0 += 2) {                      // two stages per trip
+        float4 v[2][18];
+#pragma unroll
+        for (int t = 0; t < 2; t++) {
+            const int j = j0 + t;
+            const float4 *src = reinterpret_cast<const float4 *>(Kh + (long)(j < clen ? j : 0) * 72);
+#pragma unroll
+            for (int i = 0; i < 18; i++) v[t][i] = __ldg(src + i);
+        }
+#pragma unroll
+        for (int t = 0; t < 2; t++) {
+            const int j = j0 + t;
+            const float m = j < clen ? -1.0f : 0.0f;            // Kn = -Kh; zero gains in the unused steps of a short chunk
+            float kq[72];
+#pragma unroll
+            for (int r = 0; r < 6; r++) {
+                const float4 v0 = v[t][3 * r], v1 = v[t][3 * r + 1], v2 = v[t][3 * r + 2];
+                float *d = kq + 12 * r;
+                d[0] = m * v0.x; d[6] = m * v0.y; d[1] = m * v0.z; d[7] = m * v0.w;
+                d[2] = m * v1.x; d[8] = m * v1.y; d[3] = m * v1.z; d[9] = m * v1.w;
+                d[4] = m * v2.x; d[10] = m * v2.y; d[5] = m * v2.z; d[11] = m * v2.w;
+            }
+#pragma unroll
+            for (int c = 0; c < 9; c++) tm_st8(myt + 72 * j + 8 * c, kq + 8 * c);
+            float cv[6] = { 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f };
+            if (c6 != nullptr && j < clen) {
+#pragma unroll
+                for (int i = 0; i < 6; i++) cv[i] = __ldg(c6 + j * 6 + i);
+            }
+            tm_st6(myt + TM_COFF + 6 * j, cv);
+        }
+    }
+    tm_wait_st();
+}
+
+// Prologue of the CTA: stage records of its envs -> shared memory (float4 groups, slot-major), chunk operators,
+// boundary slots, control words.  Its own function for the same reason as tm_chain_load.
+template <int NU>
+__device__ __noinline__ void tm_cta_load(SrbWs W, const float *__restrict__ Psi, const float *__restrict__ x0g, long st, int b0, int Gv, int N, int G,
+                                          int C, float *smem)
+{
+    constexpr int GRBW = pinmpc_rb_width(NU);
+    const int tid = threadIdx.x;
+    const TmLay L = tm_layout(N, G, C, NU);
+    float4 *recA4 = reinterpret_cast<float4 *>(smem + L.oA), *recB4 = reinterpret_cast<float4 *>(smem + L.oB);
+    float *psi = smem + L.oPsi, *bnd = smem + L.oBnd;
+    int *ctl = reinterpret_cast<int *>(smem + L.oCtl);
+    const int nsl = G * N, nch = G * C, cbase = N / C, crem = N - cbase * C, nst = Gv * N;
+    const float4 *RA4 = reinterpret_cast<const float4 *>(W.RA), *RB4 = reinterpret_cast<const float4 *>(W.RB);
+    const long s0 = (long)b0 * N;
+    const int big = crem * (cbase + 1);                          // stages covered by the longer chunks
+    for (int sl = tid; sl < nst; sl += TM_THREADS) {              // one stage per thread and trip, all its groups in flight
+        const int e = sl / N, k = sl - e * N;
+        int c, j;
+        if (k < big) { c = k / (cbase + 1); j = k - c * (cbase + 1); }
+        else { c = crem + (k - big) / cbase; j = (k - big) - (c - crem) * cbase; }
+        const int slot = j < cbase ? j * nch + e * C + c : cbase * nch + e * crem + c;
+        float4 va[7], vb[GRBW / 4];
+#pragma unroll
+        for (int g = 0; g < 7; g++) va[g] = __ldg(RA4 + (long)g * st + s0 + sl);
+#pragma unroll
+        for (int g = 0; g < GRBW / 4; g++) vb[g] = __ldg(RB4 + (long)g * st + s0 + sl);
+        const float2 csv = __ldg(reinterpret_cast<const float2 *>(W.cs) + s0 + sl);
+        va[6].w = vb[GRBW / 4 - 1].z;                            // contact bits (word 12 + 3 nc + nu of the RB record)
+        vb[GRBW / 4 - 1].z = csv.x; vb[GRBW / 4 - 1].w = csv.y;
+#pragma unroll
+        for (int g = 0; g < 7; g++) recA4[g * nsl + slot] = va[g];
+#pragma unroll
+        for (int g = 0; g < GRBW / 4; g++) recB4[g * nsl + slot] = vb[g];
+    }
+    if (C > 2) {
+        const int per = (C - 2) * 144;
+        const float4 *src = reinterpret_cast<const float4 *>(Psi + (long)b0 * per);
+        float4 *dst = reinterpret_cast<float4 *>(psi);
+        for (int i = tid; i < Gv * per / 4; i += TM_THREADS) dst[i] = __ldg(src + i);
+    }
+    for (int i = tid; i < Gv * (C + 1) * 12; i += TM_THREADS) {
+        const int e = i / ((C + 1) * 12), r = i - e * (C + 1) * 12;
+        bnd[i] = r < 12 ? x0g[(long)(b0 + e) * NX + r] : 0.0f;                          // slot 0 = x_0, slot C = 0
+    }
+    for (int i = tid; i < TM_CTL; i += TM_THREADS) ctl[i] = 0;
+}
+
 // ---------------------------------------------------------------------------------------------
 // S3-S6: all ADMM iterations of G envs per CTA.  12 warps: warps 0-3 are the CHAIN warps (lane t of warp q =
 // chain 32 q + t = TMEM lane), warps 4-7 and 8-11 the WORKER warps: worker (slot s = 0, 1; quarter q; lane t)
@@ -590,38 +678,7 @@ __global__ void __launch_bounds__(TM_THREADS, 1) k_iterate_tm(SolveParams P, Srb
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
     }
     // ---- stage records, chunk operators, boundary slots -------------------------------------------------------
-    {
-        const float4 *RA4 = reinterpret_cast<const float4 *>(W.RA), *RB4 = reinterpret_cast<const float4 *>(W.RB);
-        const long s0 = (long)b0 * N;
-        const int big = crem * (cbase + 1);                      // stages covered by the longer chunks
-        for (int i = tid; i < nst * (7 + GRBW / 4); i += TM_THREADS) {
-            const int g = i / nst, sl = i - g * nst;
-            const int e = sl / N, k = sl - e * N;
-            int c, j;
-            if (k < big) { c = k / (cbase + 1); j = k - c * (cbase + 1); }
-            else { c = crem + (k - big) / cbase; j = (k - big) - (c - crem) * cbase; }
-            const int slot = slot_of(e, c, j);
-            if (g < 7) {
-                float4 v = __ldg(RA4 + (long)g * st + s0 + sl);
-                if (g == 6) v.w = __ldg(W.RB + pinmpc_rec_index(12 + 3 * NC + NU, st, s0 + sl));      // contact bits
-                recA4[g * nsl + slot] = v;
-            } else {
-                const int gb = g - 7;
-                float4 v = __ldg(RB4 + (long)gb * st + s0 + sl);
-                if (gb == GRBW / 4 - 1) { v.z = __ldg(W.cs + (s0 + sl) * 2); v.w = __ldg(W.cs + (s0 + sl) * 2 + 1); }
-                recB4[gb * nsl + slot] = v;
-            }
-        }
-        if (C > 2) {
-            const int per = (C - 2) * 144;
-            for (int i = tid; i < Gv * per; i += TM_THREADS) psi[i] = __ldg(Psi + (long)b0 * per + i);
-        }
-        for (int i = tid; i < Gv * (C + 1) * 12; i += TM_THREADS) {
-            const int e = i / ((C + 1) * 12), r = i - e * (C + 1) * 12;
-            bnd[i] = r < 12 ? x0g[(long)(b0 + e) * NX + r] : 0.0f;                      // slot 0 = x_0, slot C = 0
-        }
-        for (int i = tid; i < TM_CTL; i += TM_THREADS) ctl[i] = 0;
-    }
+    tm_cta_load<NU>(W, Psi, x0g, st, b0, Gv, N, G, C, smem);
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
@@ -642,32 +699,7 @@ __global__ void __launch_bounds__(TM_THREADS, 1) k_iterate_tm(SolveParams P, Srb
     const bool tol_mode = (P.eps_abs > 0.0f || P.eps_rel > 0.0f) && P.check_every > 0;
     if (warp < 4) {
         // =========================== CHAIN WARPS =================================================================
-        // prologue: the chunk's gains -> this lane of tensor memory, row-major Kn[r][0..11] = -Kh[r][.]
-        for (int j = 0; j < TM_LMAX; j++) {
-            float kq[72];
-            if (j < clen) {
-                const float4 *src = reinterpret_cast<const float4 *>(W.Kh + ((long)b0 * N + sl0 + j) * 72);
-#pragma unroll
-                for (int r = 0; r < 6; r++) {
-                    const float4 v0 = __ldg(src + 3 * r), v1 = __ldg(src + 3 * r + 1), v2 = __ldg(src + 3 * r + 2);
-                    float *d = kq + 12 * r;
-                    d[0] = -v0.x; d[6] = -v0.y; d[1] = -v0.z; d[7] = -v0.w;
-                    d[2] = -v1.x; d[8] = -v1.y; d[3] = -v1.z; d[9] = -v1.w;
-                    d[4] = -v2.x; d[10] = -v2.y; d[5] = -v2.z; d[11] = -v2.w;
-                }
-            } else {
-#pragma unroll
-                for (int i = 0; i < 72; i++) kq[i] = 0.0f;
-            }
-#pragma unroll
-            for (int c = 0; c < 9; c++) tm_st8(myt + 72 * j + 8 * c, kq + 8 * c);
-            float cv[6] = { 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f };
-            if (has_ext && j < clen) {
-#pragma unroll
-                for (int i = 0; i < 6; i++) cv[i] = __ldg(W.c6 + ((long)b0 * N + sl0 + j) * 6 + i);
-            }
-            tm_st6(myt + TM_COFF + 6 * j, cv);
-        }
+        tm_chain_load(W.Kh + ((long)b0 * N + sl0) * 72, has_ext ? W.c6 + ((long)b0 * N + sl0) * 6 : nullptr, clen, myt);
         tm_wait_st();
         ChainArgs A;
         A.ch.tk = myt;
@@ -849,9 +881,22 @@ __global__ void __launch_bounds__(TM_THREADS, 1) k_iterate_tm(SolveParams P, Srb
         for (int a = 0; a < WS; a++)
             if ((flags >> a) & 1) {
                 const long ts = (long)b0 * N + sl0 + jw + a;
-                float *oz = o.z + ts * NU, *oy = o.y + ts * NU;
+                constexpr int VW = NU % 4 == 0 ? 4 : 2;              // a stage's z, y start on a 48 B (nu = 12) or 72 B (nu = 18) boundary
+                if (VW == 4) {
+                    float4 *oz = reinterpret_cast<float4 *>(o.z + ts * NU), *oy = reinterpret_cast<float4 *>(o.y + ts * NU);
 #pragma unroll
-                for (int j = 0; j < NU; j++) { oz[j] = S[a].z[j]; oy[j] = S[a].y[j]; }
+                    for (int j = 0; j < NU / 4; j++) {
+                        oz[j] = make_float4(S[a].z[4 * j], S[a].z[4 * j + 1], S[a].z[4 * j + 2], S[a].z[4 * j + 3]);
+                        oy[j] = make_float4(S[a].y[4 * j], S[a].y[4 * j + 1], S[a].y[4 * j + 2], S[a].y[4 * j + 3]);
+                    }
+                } else {
+                    float2 *oz = reinterpret_cast<float2 *>(o.z + ts * NU), *oy = reinterpret_cast<float2 *>(o.y + ts * NU);
+#pragma unroll
+                    for (int j = 0; j < NU / 2; j++) {
+                        oz[j] = make_float2(S[a].z[2 * j], S[a].z[2 * j + 1]);
+                        oy[j] = make_float2(S[a].y[2 * j], S[a].y[2 * j + 1]);
+                    }
+                }
             }
     }
     // ---- release tensor memory ---------------------------------------------------------------------------------
