@@ -352,6 +352,8 @@ def run_sweep(args):
             s = Solver(w.nu, w.N, w.B, layout=lay, rho=w.rho, iters=w.iters, Qdiag=w.Qdiag, Rdiag=w.Rdiag, dt=w.dt,
                        method=METHOD_SRB, device=dev)
             s.set_workload(w)
+            if args.chunks:
+                s.set_horizon_chunks(args.chunks)
             for _ in range(3):
                 s.solve()
             torch.cuda.synchronize(dev)
@@ -365,7 +367,8 @@ def run_sweep(args):
             ms = float(np.median(ts))
             inputs = sum(getattr(w, n).nbytes for n in gen.Workload.ARRAYS if getattr(w, n) is not None)
             io_bytes = inputs + w.B * w.N * (13 + 3 * w.nu) * 4 + w.B * 12
-            print(json.dumps({"sweep": w.name, "B": B, "N": N, "iters": w.iters, "ms_per_solve": ms,
+            G_used, C_used = s.launch_shape()
+            print(json.dumps({"sweep": w.name, "B": B, "N": N, "iters": w.iters, "envs_per_cta": G_used, "horizon_chunks": C_used, "ms_per_solve": ms,
                               "solves_per_s": B / (ms * 1e-3), "stage_iters_per_s": B * N * w.iters / (ms * 1e-3),
                               "tflops": flops_per_solve(w, "srb") / (ms * 1e-3) / 1e12,
                               "hbm_gbs_algorithmic": io_bytes / (ms * 1e-3) / 1e9,

@@ -117,8 +117,8 @@ pinmpc_status pinmpc_set_tuning(pinmpc_t h, int envs_per_cta);
 /* How the equality step (S3) is parallelised across the horizon (north_star (2); PAPER.md:L206-208 Remark 2,
  * L23): the N stages are cut into `chunks` chunks that are swept concurrently (chunked two-sweep over the
  * time-varying LQR recursion, gains resident in tensor memory).
- *   0 (default) = ceil(N / L) chunks, L = 6 (nu = 12) or 4 (nu = 18), when the shape fits the chunked kernel, else
- *                 sequential passes;
+ *   0 (default) = ceil(N / L) chunks, L = 6 (nu = 12) or 4 (nu = 18), for N >= 16 when the shape fits the chunked
+ *                 kernel, else sequential passes (the measured crossover, profiles/r2_sweep_config4.md);
  *   1           = the sequential-pass kernel (two N-step recursions per iteration);
  *   >= 2        = that many chunks; PINMPC_EUNSUPPORTED unless ceil(N / chunks) <= L, chunks <= 128 and
  *                 chunks <= ceil(N / (L - 1)) (room for the chunk operators in the workspace).

@@ -106,6 +106,7 @@ int pinmpc_launch_solve_srb(pinmpc_ctx *h, cudaStream_t st);
 int pinmpc_launch_srb_assembly_debug(pinmpc_ctx *h, float *A, float *Bm, float *c, float *S, float *Tinv, cudaStream_t st);
 size_t pinmpc_ws_srb_bytes(int nu, int N, int B);
 // chunked, TMEM-resident iteration kernel (pinmpc_tmem.cu)
+#define PINMPC_CHUNKED_MIN_N 16     // horizons from which pinmpc_set_horizon_chunks(h, 0) picks the chunked kernel
 bool pinmpc_tm_config(const pinmpc_ctx *h, int *G, int *C);
 int pinmpc_launch_iterate_tm(pinmpc_ctx *h, int G, int C, cudaStream_t st);
 // chunk operators of up to ceil(N / 5) chunks (nu = 12: 5 or 6 stages per chunk), ceil(N / 3) chunks (nu = 18: 3 or 4)

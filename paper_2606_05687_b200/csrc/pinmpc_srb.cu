@@ -1032,10 +1032,12 @@ int launch_t(pinmpc_ctx *h, cudaStream_t st)
     if (prof) cudaEventRecord(h->ev[2], st);
 
     // S3-S6: the chunked, TMEM-resident kernel (parallel in the horizon) when the shape fits, else the
-    // sequential-pass kernel (also: pinmpc_set_horizon_chunks(h, 1))
+    // sequential-pass kernel (also: pinmpc_set_horizon_chunks(h, 1)).  Chosen by measurement (profiles/r2_sweep_config4.md):
+    // the chunked kernel wins from N = 20 on (1.05x at N = 20, 1.2x at N = 50, 1.35x at N = 100) and loses below (0.7-0.9x
+    // at N = 10, where two chunks of five stages leave nothing to run in parallel).
     int nk = 2;
     int tmG = 0, tmC = 0;
-    if (h->chunks != 1 && pinmpc_tm_config(h, &tmG, &tmC)) {
+    if (h->chunks != 1 && (h->chunks > 1 || h->N >= PINMPC_CHUNKED_MIN_N) && pinmpc_tm_config(h, &tmG, &tmC)) {
         const int n = pinmpc_launch_iterate_tm(h, tmG, tmC, st);
         if (n < 0) return -1;
         nk += n;
