@@ -44,7 +44,10 @@ __host__ __device__ constexpr int tm_lmax(int nu) { return nu == 12 ? 6 : 4; }
 constexpr int TM_XOFF = TM_LMAX * 72;              // exchange vectors   [LMAX][6]   columns 432..467
 constexpr int TM_COFF = TM_XOFF + TM_LMAX * 6;     // ch (ext only)      [LMAX][6]   columns 468..503
 constexpr int TM_CHAINS = 128;                     // chain threads = TMEM lanes
-constexpr int TM_THREADS = 384;                    // 4 chain warps + 8 worker warps (168 registers per thread)
+// worker threads per chain (they share its TMEM lane and split its stages): three at nu = 12 (two stages each, 512 threads
+// at 128 registers), two at nu = 18 (384 threads at 168 registers)
+__host__ __device__ constexpr int tm_nwpc(int nu) { return nu == 12 ? 3 : 2; }
+__host__ __device__ constexpr int tm_threads(int nu) { return 128 * (1 + tm_nwpc(nu)); }
 constexpr int TM_GMAX = 32;                        // envs per CTA
 constexpr int TM_RAW = 28;                         // Mh^-1 (21) | kg (6) | contact bits
 constexpr int TM_CTL = 48 + 5 * TM_GMAX;           // done[32] | ndone | pad[15] | red[32][5]
@@ -343,11 +346,11 @@ template <int NU> struct TmState { float z[NU], y[NU]; };
 
 // float4 groups [G0, G1) of a record -> v (v[0] = word 4 G0)
 template <int G0, int G1>
-__device__ __forceinline__ void tm_ld_groups(const float4 *rec, int nsl, float *v)
+__device__ __forceinline__ void tm_ld_groups(uint32_t rec, uint32_t gstride, float *v)      // rec: shared-memory byte address of group 0
 {
 #pragma unroll
     for (int g = G0; g < G1; g++) {
-        const float4 q = rec[g * nsl];
+        const float4 q = lds_f4(rec + g * gstride);
         v[4 * (g - G0)] = q.x; v[4 * (g - G0) + 1] = q.y; v[4 * (g - G0) + 2] = q.z; v[4 * (g - G0) + 3] = q.w;
     }
 }
@@ -391,7 +394,7 @@ __device__ __forceinline__ void tm_sigma0(const SolveParams &P, const float *geo
 // u from w, projection (S4), dual update (S5), residuals (S6); then sigma0 of the next iteration.
 // wv: in w of this stage, out sigma0 of the next iteration.  res = running maxima (r_prim, |dz|, |u|, |z|, |y|).
 template <int NU, bool EMIT>
-__device__ __forceinline__ void tm_stage_update(const SolveParams &P, const float4 *rb, int nsl, int bits, float *z, float *y, float idt, float m_dt,
+__device__ __forceinline__ void tm_stage_update(const SolveParams &P, uint32_t rb, uint32_t nsl, int bits, float *z, float *y, float idt, float m_dt,
                                                 float *wv, bool update, float *ou, float *res, bool two_feet)
 {
     constexpr int NC = NW + (NU - 12) / 3, RBW = tm_rbw(NU);
@@ -559,17 +562,17 @@ __device__ __noinline__ void tm_chain_main(ChainArgs A)
 // per trip must not count against the register allocation of the kernel body.
 __device__ __noinline__ void tm_chain_load(const float *__restrict__ Kh, const float *__restrict__ c6, int clen, uint32_t myt)
 {
-    for (int j0 = 0; j0 < TM_LMAX; j0 += 2) {                      // two stages per trip
-        float4 v[2][18];
+    for (int j0 = 0; j0 < TM_LMAX; j0 += 1) {                      // one stage per trip: 18 loads in flight
+        float4 v[1][18];
 #pragma unroll
-        for (int t = 0; t < 2; t++) {
+        for (int t = 0; t < 1; t++) {
             const int j = j0 + t;
             const float4 *src = reinterpret_cast<const float4 *>(Kh + (long)(j < clen ? j : 0) * 72);
 #pragma unroll
             for (int i = 0; i < 18; i++) v[t][i] = __ldg(src + i);
         }
 #pragma unroll
-        for (int t = 0; t < 2; t++) {
+        for (int t = 0; t < 1; t++) {
             const int j = j0 + t;
             const float m = j < clen ? -1.0f : 0.0f;            // Kn = -Kh; zero gains in the unused steps of a short chunk
             float kq[72];
@@ -610,6 +613,7 @@ __device__ __noinline__ void tm_cta_load(SrbWs W, const float *__restrict__ Psi,
     const float4 *RA4 = reinterpret_cast<const float4 *>(W.RA), *RB4 = reinterpret_cast<const float4 *>(W.RB);
     const long s0 = (long)b0 * N;
     const int big = crem * (cbase + 1);                          // stages covered by the longer chunks
+    constexpr int TM_THREADS = tm_threads(NU);
     for (int sl = tid; sl < nst; sl += TM_THREADS) {              // one stage per thread and trip, all its groups in flight
         const int e = sl / N, k = sl - e * N;
         int c, j;
@@ -649,11 +653,11 @@ __device__ __noinline__ void tm_cta_load(SrbWs W, const float *__restrict__ Psi,
 // 168 registers per thread: the chain threads hold two half-stage operand buffers, the workers three stages.
 // ---------------------------------------------------------------------------------------------
 template <int NU, bool WARM>
-__global__ void __launch_bounds__(TM_THREADS, 1) k_iterate_tm(SolveParams P, SrbWs W, const float *__restrict__ Psi, const float *__restrict__ x0g,
+__global__ void __launch_bounds__(tm_threads(NU), 1) k_iterate_tm(SolveParams P, SrbWs W, const float *__restrict__ Psi, const float *__restrict__ x0g,
                                                               const float *__restrict__ massg, OutPtrs o, int G, int C, int has_ext,
                                                               const float *__restrict__ z0g, const float *__restrict__ y0g)
 {
-    constexpr int NC = NW + (NU - 12) / 3, RBW = tm_rbw(NU), GRBW = pinmpc_rb_width(NU);
+    constexpr int NC = NW + (NU - 12) / 3, RBW = tm_rbw(NU), GRBW = pinmpc_rb_width(NU), TM_THREADS = tm_threads(NU);
     extern __shared__ __align__(16) float smem[];
     __shared__ uint32_t tmem_slot;
     const int N = P.N, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -717,7 +721,7 @@ __global__ void __launch_bounds__(TM_THREADS, 1) k_iterate_tm(SolveParams P, Srb
         tm_chain_main<RBW>(A);
     } else {
         // =========================== WORKER WARPS ==================================================================
-        constexpr int WS = tm_lmax(NU) / 2;                      // stages per worker
+        constexpr int WS = tm_lmax(NU) / tm_nwpc(NU);            // stages per worker
         const int ws = (warp - 4) >> 2;
         // Few values stay live across an iteration next to z, y of the three owned stages: everything per stage (slot,
         // contact bits, activity) is recomputed where it is used (a spilled value costs an L2 round trip here).
@@ -734,6 +738,7 @@ __global__ void __launch_bounds__(TM_THREADS, 1) k_iterate_tm(SolveParams P, Srb
             flags |= (__any_sync(FULL, ac && (bits & 3) == 3) ? 1 : 0) << (4 + a);
         }
         const uint32_t tx = myt + TM_XOFF + 6 * jw;              // exchange vectors of the owned stages
+        const uint32_t recB_u32 = (uint32_t)__cvta_generic_to_shared(recB4);
         const float m_dt = massg[b0 + eb] / dt;
 
         TmState<NU> S[WS];
@@ -749,7 +754,7 @@ __global__ void __launch_bounds__(TM_THREADS, 1) k_iterate_tm(SolveParams P, Srb
             }
             if (ac) {
                 float G0[6], v[RBW];
-                tm_ld_groups<0, RBW / 4>(recB4 + slot_w(a), nsl, v);
+                tm_ld_groups<0, RBW / 4>(recB_u32 + 16u * slot_w(a), 16u * nsl, v);
                 tm_gh_u0<NU>(P, v + 12, S[a].z, S[a].y, G0);
                 tm_sigma0<NU>(P, v, G0, idt, m_dt, sv);
             }
@@ -774,7 +779,7 @@ __global__ void __launch_bounds__(TM_THREADS, 1) k_iterate_tm(SolveParams P, Srb
             // (three broadcast LDS.128 after a warp sync), column bi of Psi_c is fetched one step ahead.
             if (TM_ABL != 2 && C > 2 && lane < 24) {
                 const int bsub = lane / 12, bi = lane - 12 * bsub;                       // 12 lanes per env, two envs per warp
-                for (int ep = 2 * (warp - 4); ep < Gv; ep += 16) {                     // (an env past the end rides along)
+                for (int ep = 2 * (warp - 4); ep < Gv; ep += 2 * (TM_THREADS / 32 - 4)) {                     // (an env past the end rides along)
                     const int e = ep + bsub, ee = e < Gv ? e : 0;
                     float *sb = bnd + ee * (C + 1) * 12;
                     const float *ps = psi + ee * (C - 2) * 144 + bi;
@@ -805,7 +810,7 @@ __global__ void __launch_bounds__(TM_THREADS, 1) k_iterate_tm(SolveParams P, Srb
             // ---- forward boundary recursion: slot[c+1] <- Psi_c slot[c] + slot[c+1],  c = 1 .. C-2
             if (TM_ABL != 2 && C > 2 && lane < 24) {
                 const int bsub = lane / 12, bi = lane - 12 * bsub;
-                for (int ep = 2 * (warp - 4); ep < Gv; ep += 16) {
+                for (int ep = 2 * (warp - 4); ep < Gv; ep += 2 * (TM_THREADS / 32 - 4)) {
                     const int e = ep + bsub, ee = e < Gv ? e : 0;
                     float *sb = bnd + ee * (C + 1) * 12;
                     const float4 *ps = reinterpret_cast<const float4 *>(psi + ee * (C - 2) * 144 + 12 * bi);   // row bi
@@ -841,9 +846,9 @@ __global__ void __launch_bounds__(TM_THREADS, 1) k_iterate_tm(SolveParams P, Srb
                         asm volatile("" : "+r"(slot));             // opaque: no address of the stage record is hoisted out of the iteration loop
                         const int bits = __float_as_int(recA4[6 * nsl + slot].w);
                         const bool two = (flags >> (4 + a)) & 1;
-                        if (emit) tm_stage_update<NU, true>(P, recB4 + slot, nsl, bits, S[a].z, S[a].y, idt, m_dt, wv, !frozen,
+                        if (emit) tm_stage_update<NU, true>(P, recB_u32 + 16u * slot, 16u * nsl, bits, S[a].z, S[a].y, idt, m_dt, wv, !frozen,
                                                             o.u + ((long)b0 * N + sl0 + jw + a) * NU, res, two);
-                        else tm_stage_update<NU, false>(P, recB4 + slot, nsl, bits, S[a].z, S[a].y, idt, m_dt, wv, !frozen, nullptr, res, two);
+                        else tm_stage_update<NU, false>(P, recB_u32 + 16u * slot, 16u * nsl, bits, S[a].z, S[a].y, idt, m_dt, wv, !frozen, nullptr, res, two);
                     } else { wv[0] = wv[1] = wv[2] = wv[3] = wv[4] = wv[5] = 0.0f; }   // unused exchange vectors stay zero
                     tm_st6(tx + 6 * a, wv);
                     asm volatile("" ::: "memory");
@@ -970,7 +975,7 @@ static int tm_launch_t(pinmpc_ctx *h, const SolveParams &P, const ProblemPtrs &q
     std::call_once(once[wi], [&] { once_err[wi] = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem_optin - 256); });
     if (once_err[wi] != cudaSuccess) return tm_fail(h, "k_iterate_tm smem attribute", once_err[wi]);
     cudaError_t e;
-    kern<<<(unsigned)((h->B + G - 1) / G), TM_THREADS, smem, st>>>(P, h->srb, h->psi, q.x0, q.mass, h->out, G, C, ext, q.z0, q.y0);
+    kern<<<(unsigned)((h->B + G - 1) / G), tm_threads(NU), smem, st>>>(P, h->srb, h->psi, q.x0, q.mass, h->out, G, C, ext, q.z0, q.y0);
     e = cudaGetLastError();
     if (e != cudaSuccess) return tm_fail(h, "k_iterate_tm launch", e);
     return n + 1;
