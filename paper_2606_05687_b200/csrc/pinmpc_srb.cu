@@ -194,8 +194,8 @@ __global__ void __launch_bounds__(128) k_assemble_srb(SolveParams P, ProblemPtrs
 // arithmetic in the loop); lanes 0..20 own one packed element of the symmetric 6x6 Mh each.
 // ---------------------------------------------------------------------------------------------
 constexpr int FAC_WARPS = 4;                        // warps (envs) per CTA
-constexpr int FAC_LD = 16;                          // padded row length
-constexpr int FAC_SMEM = 13 * 16 + 13 * 16 + 6 * 16 + 24;   // floats per warp: P, X, Kh, Mh^-1
+constexpr int FAC_LD = 20;                          // padded row length: rows 80 B apart, the float4 row accesses of eight lanes hit distinct banks
+constexpr int FAC_SMEM = 13 * FAC_LD + 13 * FAC_LD + 6 * FAC_LD + 24;   // floats per warp: P, X, Kh, Mh^-1
 
 __global__ void __launch_bounds__(FAC_WARPS * 32, 7) k_factor_srb(SolveParams P, const float *__restrict__ x0, SrbWs W, int has_ext)
 {
