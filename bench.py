@@ -337,7 +337,8 @@ def run_split_sweep(args):
 
 def run_sweep(args):
     """BASELINE.json config 4: B in {1024, 4096, 16384, 65536} x N in {10, 25, 50, 100}, 100 iterations, fp32:
-    solves/s, achieved FP32 and HBM rates and the device-memory footprint of every point."""
+    solves/s, achieved FP32 and HBM rates and the device-memory footprint of every point; then the long horizons
+    N in {200, 400} of PAPER.md Fig. 3 (L277-279, "even to N = 400" L314) at B in {1024, 4096, 16384}."""
     import numpy as np
     import torch
     import gen
@@ -345,8 +346,10 @@ def run_sweep(args):
     dev = torch.device("cuda", 0)
     stream = torch.cuda.current_stream(dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
-    for B in (1024, 4096, 16384, 65536):
-        for N in (10, 25, 50, 100):
+    grid = [(B, N) for B in (1024, 4096, 16384, 65536) for N in (10, 25, 50, 100)]
+    grid += [(B, N) for B in (1024, 4096, 16384) for N in (200, 400)]
+    for B, N in grid:
+        if True:
             w = gen.make_config(4, B=B, N=N)
             lay = make_layout(w.n_wrench, w.n_force, w.mu, w.fz_max, w.mx_coef, w.my_coef, w.mz_coef, w.hand_fmax)
             s = Solver(w.nu, w.N, w.B, layout=lay, rho=w.rho, iters=w.iters, Qdiag=w.Qdiag, Rdiag=w.Rdiag, dt=w.dt,

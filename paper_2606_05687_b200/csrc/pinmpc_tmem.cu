@@ -343,6 +343,14 @@ __device__ __forceinline__ void chain_fwd_sweep(const Chain &ch, float dt, float
 template <int NU> struct TmState { float z[NU], y[NU]; };
 
 #define TM_PHASE() asm volatile("" ::: "memory")
+#ifdef PINMPC_TM_TIMING
+__device__ int g_ut[16 * 32];
+#define TM_UT(i) { if (ut != nullptr) { asm volatile("" ::: "memory"); ut[i] = (int)clock(); asm volatile("" ::: "memory"); } }
+#define TM_UTARG , int *ut
+#else
+#define TM_UT(i)
+#define TM_UTARG
+#endif
 
 // float4 groups [G0, G1) of a record -> v (v[0] = word 4 G0)
 template <int G0, int G1>
@@ -395,8 +403,9 @@ __device__ __forceinline__ void tm_sigma0(const SolveParams &P, const float *geo
 // wv: in w of this stage, out sigma0 of the next iteration.  res = running maxima (r_prim, |dz|, |u|, |z|, |y|).
 template <int NU, bool EMIT>
 __device__ __forceinline__ void tm_stage_update(const SolveParams &P, uint32_t rb, uint32_t nsl, int bits, float *z, float *y, float idt, float m_dt,
-                                                float *wv, bool update, float *ou, float *res, bool two_feet)
+                                                float *wv, bool update, float *ou, float *res, bool two_feet TM_UTARG)
 {
+    TM_UT(0)
     constexpr int NC = NW + (NU - 12) / 3, RBW = tm_rbw(NU);
     constexpr int GEO4 = (12 + 3 * NC + 3) / 4;                 // groups holding T^-1, I_w, r
     float G0[6];
@@ -406,6 +415,7 @@ __device__ __forceinline__ void tm_stage_update(const SolveParams &P, uint32_t r
         tm_gh_u0<NU>(P, v, z, y, G0);
     }
     TM_PHASE();
+    TM_UT(1)
     if (update) {
         float lam[6];
         {
@@ -417,6 +427,7 @@ __device__ __forceinline__ void tm_stage_update(const SolveParams &P, uint32_t r
             lam_inv_apply<NU>(P, geo, geo + 12, dl, lam);
         }
         TM_PHASE();
+        TM_UT(2)
         // u = u0 + Rt^-1 Gh^T lam, contact by contact;  y <- y + u  (= the argument v of the projection)
         float uk[EMIT ? NU : 1];
         {
@@ -438,6 +449,7 @@ __device__ __forceinline__ void tm_stage_update(const SolveParams &P, uint32_t r
             }
         }
         TM_PHASE();
+        TM_UT(3)
         // the feet: ONE exact projection when no thread of the warp has both feet in stance (a swing foot projects to
         // 0): the argument of the stance foot is selected, projected and scattered; else a second one of foot 0
         float zf[NW][6];
@@ -460,6 +472,7 @@ __device__ __forceinline__ void tm_stage_update(const SolveParams &P, uint32_t r
                 for (int a = 0; a < 6; a++) zf[0][a] = on0 ? z0p[a] : 0.0f;
             }
         }
+        TM_UT(4)
         // z <- projection, y <- v - z
 #pragma unroll
         for (int i = 0; i < NC; i++) {
@@ -478,18 +491,21 @@ __device__ __forceinline__ void tm_stage_update(const SolveParams &P, uint32_t r
             }
         }
         TM_PHASE();
+        TM_UT(5)
         {
             float v[RBW - 12];
             tm_ld_groups<3, RBW / 4>(rb, nsl, v);
             tm_gh_u0<NU>(P, v, z, y, G0);                       // Gh u0 of the next iteration
         }
         TM_PHASE();
+        TM_UT(6)
     }
     {
         float geo[4 * GEO4];
         tm_ld_groups<0, GEO4>(rb, nsl, geo);
         tm_sigma0<NU>(P, geo, G0, idt, m_dt, wv);               // frozen envs keep a well-defined (constant) sigma0
     }
+    TM_UT(7)
 }
 
 #ifdef PINMPC_TM_TIMING
@@ -839,6 +855,13 @@ __global__ void __launch_bounds__(tm_threads(NU), 1) k_iterate_tm(SolveParams P,
 #pragma unroll
                 for (int a = 0; a < WS; a++) {
                     float wv[6];
+#ifdef PINMPC_TM_TIMING
+                    int *ut = (it == TM_TICK_IT && lane == 0 && blockIdx.x == 0) ? g_ut + (warp - 4) * 32 + a * 10 : nullptr;
+                    TM_UT(8)
+#define TM_UTPASS , ut
+#else
+#define TM_UTPASS
+#endif
                     tm_ld6(tx + 6 * a, wv);
                     tm_wait_ld();
                     if (((flags >> a) & 1) && TM_ABL != 1) {
@@ -847,11 +870,12 @@ __global__ void __launch_bounds__(tm_threads(NU), 1) k_iterate_tm(SolveParams P,
                         const int bits = __float_as_int(recA4[6 * nsl + slot].w);
                         const bool two = (flags >> (4 + a)) & 1;
                         if (emit) tm_stage_update<NU, true>(P, recB_u32 + 16u * slot, 16u * nsl, bits, S[a].z, S[a].y, idt, m_dt, wv, !frozen,
-                                                            o.u + ((long)b0 * N + sl0 + jw + a) * NU, res, two);
-                        else tm_stage_update<NU, false>(P, recB_u32 + 16u * slot, 16u * nsl, bits, S[a].z, S[a].y, idt, m_dt, wv, !frozen, nullptr, res, two);
+                                                            o.u + ((long)b0 * N + sl0 + jw + a) * NU, res, two TM_UTPASS);
+                        else tm_stage_update<NU, false>(P, recB_u32 + 16u * slot, 16u * nsl, bits, S[a].z, S[a].y, idt, m_dt, wv, !frozen, nullptr, res, two TM_UTPASS);
                     } else { wv[0] = wv[1] = wv[2] = wv[3] = wv[4] = wv[5] = 0.0f; }   // unused exchange vectors stay zero
                     tm_st6(tx + 6 * a, wv);
                     asm volatile("" ::: "memory");
+                    TM_UT(9)
                 }
                 if (emit && (flags & 1) && !frozen) {
                     atomicMax(&red[eb * 5 + 0], __float_as_uint(res[0])); atomicMax(&red[eb * 5 + 1], __float_as_uint(res[1]));
@@ -911,6 +935,16 @@ __global__ void __launch_bounds__(tm_threads(NU), 1) k_iterate_tm(SolveParams P,
         const int *t = ndone + 1;
         printf("chain : (1)->bwdA start %d | bwdA %d | bnd %d | bwdB %d | fwdA %d | bnd %d | fwdB %d   total %d\n", 0, t[1] - t[0], t[2] - t[1], t[3] - t[2],
                t[4] - t[3], t[5] - t[4], t[6] - t[5], t[6] - t[0]);
+        for (int w = 0; w < TM_THREADS / 32 - 4; w++) {
+            const int *u = g_ut + w * 32;
+            printf("upd warp %2d:", w);
+            for (int a = 0; a < 2; a++) {
+                const int *q = u + a * 10;
+                printf("  [ld %d G0 %d lam %d u %d proj %d zy %d G0n %d sig %d st %d | %d]", q[0] - q[8], q[1] - q[0], q[2] - q[1], q[3] - q[2], q[4] - q[3], q[5] - q[4],
+                       q[6] - q[5], q[7] - q[6], q[9] - q[7], q[9] - q[8]);
+            }
+            printf("  total %d\n", u[19] - u[8]);
+        }
         printf("worker: wait bwdA %d | bnd-bwd %d | wait bwdB+fwdA %d | bnd-fwd %d | wait fwdB %d | update %d   total %d\n", t[8] - t[7], t[9] - t[8],
                t[10] - t[9], t[11] - t[10], t[12] - t[11], t[13] - t[12], t[13] - t[7]);
     }
