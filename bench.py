@@ -471,6 +471,7 @@ def main():
     ms = float(np.mean(ms_steps))
 
     # ---- end to end through the public API with host buffers ----------------------------------------
+    shape = s.launch_shape() if mname == "srb" else (None, None)     # (envs per CTA, horizon chunks) of the timed launches
     e2e = None
     if not args.no_e2e:
         names = [n for n in gen.Workload.ARRAYS if getattr(w, n) is not None]
@@ -569,7 +570,7 @@ def main():
             k_ms = [float(np.mean([k[i] for k in kernel_ms])) for i in range(3)]
             fl = w.B * w.N * w.iters * flop_per_stage_iter(w)
             achieved = fl / (k_ms[2] * 1e-3) / 1e12
-            G_used, C_used = s.launch_shape()
+            G_used, C_used = shape
         else:
             k_ms = None
             achieved = fl / (ms * 1e-3) / 1e12                 # TFLOP/s of the whole step (dense variant)
@@ -598,7 +599,7 @@ def main():
             "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": w.name, "B": w.B, "N": w.N, "iters": w.iters, "nu": w.nu, "rho": w.rho,
-                       "method": mname, "horizon_chunks": (s.launch_shape()[1] if mname == "srb" else None), "l2": "flushed (256 MiB write) between timed steps; per-step CUDA events",
+                       "method": mname, "horizon_chunks": shape[1], "l2": "flushed (256 MiB write) between timed steps; per-step CUDA events",
                        "multi_gpu": "replicas only (no collective on the data path)"},
             "stage_iters_per_s": total_solves * w.N * w.iters / (ms * 1e-3),
             "ms_min": float(np.min(ms_steps)), "ms_median": float(np.median(ms_steps)),

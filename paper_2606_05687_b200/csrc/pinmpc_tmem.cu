@@ -343,7 +343,11 @@ __device__ __forceinline__ void chain_fwd_sweep(const Chain &ch, float dt, float
 template <int NU> struct TmState { float z[NU], y[NU]; };
 
 #define TM_PHASE() asm volatile("" ::: "memory")
-#ifdef PINMPC_TM_TIMING
+// -DPINMPC_TM_TIMING=2: lane 0 of every worker warp of CTA 0 also stores clock() between the phases of the stage update
+#if defined(PINMPC_TM_TIMING) && PINMPC_TM_TIMING >= 2
+#define PINMPC_TM_UTIMING
+#endif
+#ifdef PINMPC_TM_UTIMING
 __device__ int g_ut[16 * 32];
 #define TM_UT(i) { if (ut != nullptr) { asm volatile("" ::: "memory"); ut[i] = (int)clock(); asm volatile("" ::: "memory"); } }
 #define TM_UTARG , int *ut
@@ -855,7 +859,7 @@ __global__ void __launch_bounds__(tm_threads(NU), 1) k_iterate_tm(SolveParams P,
 #pragma unroll
                 for (int a = 0; a < WS; a++) {
                     float wv[6];
-#ifdef PINMPC_TM_TIMING
+#ifdef PINMPC_TM_UTIMING
                     int *ut = (it == TM_TICK_IT && lane == 0 && blockIdx.x == 0) ? g_ut + (warp - 4) * 32 + a * 10 : nullptr;
                     TM_UT(8)
 #define TM_UTPASS , ut
@@ -935,6 +939,7 @@ __global__ void __launch_bounds__(tm_threads(NU), 1) k_iterate_tm(SolveParams P,
         const int *t = ndone + 1;
         printf("chain : (1)->bwdA start %d | bwdA %d | bnd %d | bwdB %d | fwdA %d | bnd %d | fwdB %d   total %d\n", 0, t[1] - t[0], t[2] - t[1], t[3] - t[2],
                t[4] - t[3], t[5] - t[4], t[6] - t[5], t[6] - t[0]);
+#ifdef PINMPC_TM_UTIMING
         for (int w = 0; w < TM_THREADS / 32 - 4; w++) {
             const int *u = g_ut + w * 32;
             printf("upd warp %2d:", w);
@@ -945,6 +950,7 @@ __global__ void __launch_bounds__(tm_threads(NU), 1) k_iterate_tm(SolveParams P,
             }
             printf("  total %d\n", u[19] - u[8]);
         }
+#endif
         printf("worker: wait bwdA %d | bnd-bwd %d | wait bwdB+fwdA %d | bnd-fwd %d | wait fwdB %d | update %d   total %d\n", t[8] - t[7], t[9] - t[8],
                t[10] - t[9], t[11] - t[10], t[12] - t[11], t[13] - t[12], t[13] - t[7]);
     }
