@@ -95,6 +95,10 @@ def parse():
     ap.add_argument("--sweep", action="store_true", help="BASELINE.json config 4: B x N table (one JSON line per point)")
     ap.add_argument("--split", action="store_true",
                     help="time the paper's own stage-local ADMM (pinmpc_split_solve) on the config instead (one JSON line)")
+    ap.add_argument("--split-scaled", action="store_true", help="--split with the variable scaling Sx = Q^-1/2, su = 100 (DESIGN.md 7c)")
+    ap.add_argument("--split-accel", action="store_true", help="--split with Nesterov acceleration and restart")
+    ap.add_argument("--converge", action="store_true",
+                    help="iterations to tolerance x ms per iteration for the exact-dynamics path and the stage-local method (one JSON line per setting)")
     ap.add_argument("--split-sweep", action="store_true",
                     help="scalability table of the stage-local method like the paper's Fig. 3: envs x horizon up to N = 400")
     ap.add_argument("--chunks", type=int, default=0, help="horizon chunks of the equality step (0 = auto, 1 = sequential-pass kernel)")
@@ -240,7 +244,12 @@ def run_split(args):
     A, Bm, c = s.get_dynamics()
     d = lambda a, t=torch.float32: None if a is None else torch.from_numpy(np.ascontiguousarray(a)).to(dev, t)
     x0, x_ref, u_ref, contact = d(w.x0), d(w.x_ref), d(w.u_ref), d(w.contact, torch.uint8)
-    sp = SplitSolver(w.nu, w.N, w.B, lay, w.Qdiag, w.Rdiag, w.rho, w.iters, device=dev)
+    opts = {}
+    if args.split_scaled:
+        opts.update(scale_x=split_scale_x(w), scale_u=100.0)
+    if args.split_accel:
+        opts.update(accel=True)
+    sp = SplitSolver(w.nu, w.N, w.B, lay, w.Qdiag, w.Rdiag, w.rho, w.iters, device=dev, **opts)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
     run = lambda: sp.solve(A, Bm, c if w.ext_wrench is not None else None, x0, None, x_ref, u_ref, contact)
     for _ in range(max(args.warmup, 3)):
@@ -266,8 +275,9 @@ def run_split(args):
         peaks = {"hbm_gbs": 6540.0}                            # fallback of the profiling guide
     print(json.dumps({"metric": "stage-local ADMM (paper eq. 22) solves/s", "value": w.B / (ms * 1e-3), "unit": "solves/s",
                       "ms_per_step": ms, "steps": args.steps, "n_gpus": 1, "dtype": "f32", "data": "synthetic",
-                      "config": {"workload": w.name, "B": w.B, "N": w.N, "iters": w.iters, "nu": w.nu, "method": "split"},
-                      "stage_iters_per_s": st * w.iters / (ms * 1e-3), "gpu_launches": 2 + 2 * w.iters,
+                      "config": {"workload": w.name, "B": w.B, "N": w.N, "iters": w.iters, "nu": w.nu, "method": "split",
+                                 "scaled": bool(args.split_scaled), "accel": bool(args.split_accel)},
+                      "stage_iters_per_s": st * w.iters / (ms * 1e-3), "gpu_launches": sp.launch_count(),
                       "roofline": {"bound": "hbm", "achieved": gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                                    "frac": gbs / peaks["hbm_gbs"],
                                    # dram read + write of one k_split_a plus one k_split_b launch (one iteration),
@@ -276,6 +286,92 @@ def run_split(args):
                                    "traffic_unit": "bytes per iteration (both kernels)",
                                    "bytes_per_stage_iter": per_stage_iter, "scope": "whole solve (factorisation + all iterations)"},
                       "workspace_mb": sp.workspace_bytes / 1e6, "r_prim_max": float(sp.r_prim.max())}))
+
+
+def split_scale_x(w):
+    """Sx = Q^-1/2 (1 where Q = 0): the state scaling of the iterations-to-tolerance pin (tests/test_oracle_split.py)."""
+    return [1.0 / float(q) ** 0.5 if q > 0 else 1.0 for q in w.Qdiag]
+
+
+def run_converge(args):
+    """Iterations to tolerance x time per iteration, both methods, full-size workload.
+    Reference point: the exact-dynamics path run to convergence (rho = 1e-3, 20000 iterations); error of a run =
+    max(|u - u*|_inf / (1 + |u*|_inf), |x - x*|_inf / (1 + |x*|_inf)) per env; a setting has reached eps when the median
+    env has.  Iteration counts are scanned on a geometric grid (every run starts from zero), so "iters_to" is the
+    first grid point at or below eps."""
+    import numpy as np
+    import torch
+    import gen
+    from paper_2606_05687_b200 import Solver, SplitSolver, make_layout
+    dev = torch.device("cuda", 0)
+    stream = torch.cuda.current_stream(dev)
+    w = gen.make_config(args.config, B=args.B, N=args.N)
+    lay = make_layout(w.n_wrench, w.n_force, w.mu, w.fz_max, w.mx_coef, w.my_coef, w.mz_coef, w.hand_fmax)
+    grid = [25, 50, 100, 200, 400, 800, 1600, 3200, 6400]
+
+    def timed(fn):
+        fn(); torch.cuda.synchronize(dev)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream); fn(); b.record(stream)
+        torch.cuda.synchronize(dev)
+        return a.elapsed_time(b)
+
+    def exact(rho, iters):
+        s = Solver(w.nu, w.N, w.B, layout=lay, rho=rho, iters=iters, Qdiag=w.Qdiag, Rdiag=w.Rdiag, dt=w.dt, device=dev)
+        s.set_workload(w)
+        ms = timed(s.solve)
+        o = s.get()
+        x, u = o["x"].clone(), o["u"].clone()
+        s.close()
+        return x, u, ms
+
+    xs, us, _ = exact(1e-3, 20000)
+    nx_ = 1 + xs.abs().amax(dim=(1, 2)); nu_ = 1 + us.abs().amax(dim=(1, 2))
+
+    def err(x, u):
+        e = torch.maximum((x - xs).abs().amax(dim=(1, 2)) / nx_, (u - us).abs().amax(dim=(1, 2)) / nu_)
+        return float(e.median()), float(e.quantile(0.95))
+
+    def report(name, runs):
+        rec = {"converge": name, "workload": w.name, "B": w.B, "N": w.N, "grid": []}
+        for it, (x, u, ms) in runs:
+            med, p95 = err(x, u)
+            rec["grid"].append({"iters": it, "ms": ms, "err_median": med, "err_p95": p95})
+        for eps in (1e-2, 1e-3):
+            hit = next((g for g in rec["grid"] if g["err_median"] <= eps), None)
+            rec[f"iters_to_{eps:g}"] = hit["iters"] if hit else None
+            rec[f"ms_to_{eps:g}"] = hit["ms"] if hit else None
+        rec["ms_per_iter"] = rec["grid"][-1]["ms"] / rec["grid"][-1]["iters"]
+        print(json.dumps(rec), flush=True)
+
+    for rho in (1.0, 1e-1, 1e-2, 1e-3):
+        runs = []
+        for it in grid:
+            runs.append((it, exact(rho, it)))
+            if err(*runs[-1][1][:2])[0] <= 1e-3:
+                break
+        report(f"exact-dynamics ADMM (product path), rho = {rho:g}", runs)
+
+    s = Solver(w.nu, w.N, w.B, layout=lay, rho=w.rho, iters=1, Qdiag=w.Qdiag, Rdiag=w.Rdiag, dt=w.dt, device=dev)
+    s.set_workload(w)
+    A, Bm, c = s.get_dynamics()
+    d = lambda a, t=torch.float32: None if a is None else torch.from_numpy(np.ascontiguousarray(a)).to(dev, t)
+    x0, x_ref, u_ref, contact = d(w.x0), d(w.x_ref), d(w.u_ref), d(w.contact, torch.uint8)
+    u_prev = u_ref[:, 0].contiguous()
+    for name, opts in (("stage-local ADMM, unscaled, rho = 1", {}),
+                       ("stage-local ADMM, Sx = Q^-1/2, su = 100, rho = 1", dict(scale_x=split_scale_x(w), scale_u=100.0)),
+                       ("stage-local ADMM, scaled, accelerated with restart", dict(scale_x=split_scale_x(w), scale_u=100.0, accel=True))):
+        runs = []
+        for it in grid:
+            sp = SplitSolver(w.nu, w.N, w.B, lay, w.Qdiag, w.Rdiag, 1.0, it, device=dev, **opts)
+            fn = lambda: sp.solve(A, Bm, c if w.ext_wrench is not None else None, x0, u_prev, x_ref, u_ref, contact)
+            ms = timed(fn)
+            z = sp.z
+            runs.append((it, (z[:, :, :13].clone(), z[:, :, 13:].clone(), ms)))
+            del sp
+            if err(*runs[-1][1][:2])[0] <= 1e-3:
+                break
+        report(name, runs)
 
 
 def device_dynamics(w, lay, dev):
@@ -392,6 +488,8 @@ def main():
         return run_split(args)
     if args.split_sweep:
         return run_split_sweep(args)
+    if args.converge:
+        return run_converge(args)
     if args.sweep:
         return run_sweep(args)
 

@@ -264,6 +264,36 @@ pinmpc_status pinmpc_split_solve(int nu, int N, int B, const pinmpc_layout *layo
                                  float rho, int iters, const pinmpc_split_problem *p, void *d_workspace, size_t workspace_bytes,
                                  float *xi, float *z, float *r_prim, void *stream);
 
+/* Options of pinmpc_split_solve_ex.  NULL or all-zero = pinmpc_split_solve.
+ *  - Variable scaling x = Sx x~, u = su u~ (PAPER.md:L184 leaves rho and the units open): the iteration (22) runs on
+ *    the scaled problem A~ = Sx^-1 A Sx, B~ = su Sx^-1 B, c~ = Sx^-1 c, Q~ = Sx^2 Q, R~ = su^2 R, references and
+ *    xi_0 divided by the scales, U~_k = U_k / su (same cone, box bounds divided by su; ONE scalar for all inputs keeps
+ *    the projection Euclidean); xi and z are returned in the caller's units, r_prim in the scaled ones.  The limit is
+ *    the optimum of the same QP; the iterates differ.
+ *  - accel != 0: Nesterov acceleration with restart (PAPER.md:L210 Remark 3; reading: "fast ADMM with restart",
+ *    Goldstein et al. 2014) on w = (z, v, theta, beta, lambda): iteration m starts from w^_m and yields w_m;
+ *    c_m = rho (|theta_m - theta^_m|^2 + |beta_m - beta^_m|^2 + |lambda_m - lambda^_m|^2 + |dz|^2 + |dv|^2 + |dz - dv|^2)
+ *    summed over the env's stages; c_m < eta c_{m-1}: a_{m+1} = (1 + sqrt(1 + 4 a_m^2)) / 2, w^_{m+1} = w_m +
+ *    (a_m - 1) / a_{m+1} (w_m - w_{m-1}); else restart: a_{m+1} = 1, w^_{m+1} = w_{m-1}, c_m <- c_{m-1} / eta.
+ *    Every env decides for itself.  z is w_M of the last iteration. */
+typedef struct {
+    const float *h_scale_x;    /* HOST [13] positive, or NULL => 1                                    */
+    float scale_u;             /* > 0; 0 => 1                                                         */
+    int accel;                 /* 0 plain iteration, 1 accelerated with restart                       */
+    float eta;                 /* restart threshold in (0, 1]; 0 => 0.999                             */
+    int *d_restarts;           /* DEVICE [B] or NULL: restarts taken per env (accel only)             */
+} pinmpc_split_options;
+
+/* Workspace of pinmpc_split_solve_ex for these options (scaling adds the scaled problem, about 1.5 KB per stage at
+ * nu = 12; acceleration adds two more copies of the five iterate vectors, 1 KB per stage). */
+size_t pinmpc_split_workspace_bytes_ex(int nu, int N, int B, const pinmpc_split_options *opts);
+
+/* pinmpc_split_solve with options.  Extra errors: PINMPC_EINVAL for a non-positive or non-finite scale, eta outside
+ * (0, 1]. */
+pinmpc_status pinmpc_split_solve_ex(int nu, int N, int B, const pinmpc_layout *layout, const float *h_Qdiag, const float *h_Rdiag,
+                                    float rho, int iters, const pinmpc_split_problem *p, const pinmpc_split_options *opts,
+                                    void *d_workspace, size_t workspace_bytes, float *xi, float *z, float *r_prim, void *stream);
+
 /* Human-readable description of the last error on this handle (owned by the handle; "" if none).
  * With h = NULL: the last pinmpc_create failure in this thread. */
 const char *pinmpc_last_error(pinmpc_t h);

@@ -102,7 +102,7 @@ def solve_env(A, Bm, e, Qd, Rd, rho, iters, x0, u_prev, x_ref, u_ref, project_u,
     r_prim = 0.0
     names = ("z", "v", "theta", "beta", "lam")
     w_prev = dict(z=z.copy(), v=v.copy(), theta=theta.copy(), beta=beta.copy(), lam=lam.copy())      # w_{m-1}
-    alpha, c_prev, restarts, c_hist = 1.0, np.inf, 0, []
+    alpha, c_prev, restarts, c_hist, margin = 1.0, np.inf, 0, [], np.inf
     for _ in range(iters):
         hat = dict(z=z.copy(), v=v.copy(), theta=theta.copy(), beta=beta.copy(), lam=lam.copy())     # w^_m: (22) starts here
         # (21a): every k from the previous iterates
@@ -136,6 +136,8 @@ def solve_env(A, Bm, e, Qd, Rd, rho, iters, x0, u_prev, x_ref, u_ref, project_u,
             dz, dv = z - hat["z"], v - hat["v"]
             c_m = rho * sum(float(np.sum((w_m[k] - hat[k]) ** 2)) for k in ("theta", "beta", "lam")) \
                 + rho * float(np.sum(dz ** 2) + np.sum(dv ** 2) + np.sum((dz - dv) ** 2))
+            if np.isfinite(c_prev):
+                margin = min(margin, abs(c_m - eta * c_prev) / max(c_m, eta * c_prev, 1e-300))   # how close the decision was
             if c_m < eta * c_prev:
                 a_next = 0.5 * (1.0 + np.sqrt(1.0 + 4.0 * alpha * alpha))
                 mom = (alpha - 1.0) / a_next
@@ -151,5 +153,5 @@ def solve_env(A, Bm, e, Qd, Rd, rho, iters, x0, u_prev, x_ref, u_ref, project_u,
                 z, v, theta, beta, lam = (nxt[k] for k in names)
     out = dict(xi=xi * S, z=z * S, du=du * su, v=v * S, theta=theta * S, beta=beta * S, lam=lam * S, r_prim=r_prim)
     if accel:
-        out.update(restarts=restarts, c=np.array(c_hist))
+        out.update(restarts=restarts, c=np.array(c_hist), margin=margin)
     return out

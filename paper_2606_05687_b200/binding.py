@@ -26,7 +26,8 @@ EXPORTS = ("pinmpc_workspace_bytes", "pinmpc_workspace_bytes_method", "pinmpc_cr
            "pinmpc_get", "pinmpc_get_aux", "pinmpc_get_dynamics", "pinmpc_get_srb_assembly", "pinmpc_last_launch_count", "pinmpc_last_error",
            "pinmpc_destroy", "pinmpc_set_profiling", "pinmpc_get_kernel_ms",
            "pinmpc_set_warm_start", "pinmpc_shift_aux", "pinmpc_landmark_ring_bytes", "pinmpc_landmark_reset", "pinmpc_landmark_push",
-           "pinmpc_landmark_push_solver", "pinmpc_landmark_reward", "pinmpc_split_workspace_bytes", "pinmpc_split_solve")
+           "pinmpc_landmark_push_solver", "pinmpc_landmark_reward", "pinmpc_split_workspace_bytes", "pinmpc_split_solve",
+           "pinmpc_split_workspace_bytes_ex", "pinmpc_split_solve_ex")
 MAX_LANDMARKS = 8
 
 
@@ -48,6 +49,10 @@ class Problem(ctypes.Structure):
 
 class SplitProblem(ctypes.Structure):
     _fields_ = [(n, c_void_p) for n in ("A", "Bm", "c", "x0", "u_prev", "x_ref", "u_ref", "contact")]
+
+
+class SplitOptions(ctypes.Structure):
+    _fields_ = [("h_scale_x", POINTER(c_float)), ("scale_u", c_float), ("accel", c_int), ("eta", c_float), ("d_restarts", c_void_p)]
 
 
 class LandmarkCfg(ctypes.Structure):
@@ -127,6 +132,12 @@ def load():
     lib.pinmpc_split_solve.restype = c_int
     lib.pinmpc_split_solve.argtypes = [c_int, c_int, c_int, POINTER(Layout), POINTER(c_float), POINTER(c_float), c_float, c_int,
                                        POINTER(SplitProblem), c_void_p, c_size_t, c_void_p, c_void_p, c_void_p, c_void_p]
+    lib.pinmpc_split_workspace_bytes_ex.restype = c_size_t
+    lib.pinmpc_split_workspace_bytes_ex.argtypes = [c_int, c_int, c_int, POINTER(SplitOptions)]
+    lib.pinmpc_split_solve_ex.restype = c_int
+    lib.pinmpc_split_solve_ex.argtypes = [c_int, c_int, c_int, POINTER(Layout), POINTER(c_float), POINTER(c_float), c_float, c_int,
+                                          POINTER(SplitProblem), POINTER(SplitOptions), c_void_p, c_size_t, c_void_p, c_void_p, c_void_p,
+                                          c_void_p]
     lib.pinmpc_destroy.restype = None
     lib.pinmpc_destroy.argtypes = [c_void_p]
     _lib = lib
@@ -460,13 +471,18 @@ class Landmarks:
 
 # ---- the paper's own stage-local ADMM (include/pinmpc.h, eq. (18)-(22)) ---------------------------------
 class SplitSolver:
-    """Owns the workspace and the output tensors of pinmpc_split_solve; solve() is one asynchronous C-ABI call."""
+    """Owns the workspace and the output tensors of pinmpc_split_solve_ex; solve() is one asynchronous C-ABI call.
+    scale_x (13 positive numbers) / scale_u: variable scaling; accel: Nesterov acceleration with restart (include/pinmpc.h)."""
 
-    def __init__(self, nu, N, B, layout, Qdiag, Rdiag, rho, iters, device="cuda:0"):
+    def __init__(self, nu, N, B, layout, Qdiag, Rdiag, rho, iters, device="cuda:0", scale_x=None, scale_u=1.0, accel=False, eta=0.999):
         import torch
         self.torch, self.device = torch, torch.device(device)
         self.nu, self.N, self.B, self.layout, self.rho, self.iters = int(nu), int(N), int(B), layout, float(rho), int(iters)
-        self.workspace_bytes = load().pinmpc_split_workspace_bytes(self.nu, self.N, self.B)
+        self.restarts = torch.zeros(self.B, dtype=torch.int32, device=self.device) if accel else None
+        self._sx = None if scale_x is None else (c_float * NX)(*[float(v) for v in scale_x])
+        self.opts = SplitOptions(self._sx if self._sx is not None else ctypes.cast(None, POINTER(c_float)), float(scale_u), int(bool(accel)),
+                                 float(eta), None if self.restarts is None else self.restarts.data_ptr())
+        self.workspace_bytes = load().pinmpc_split_workspace_bytes_ex(self.nu, self.N, self.B, ctypes.byref(self.opts))
         if self.workspace_bytes == 0:
             raise PinmpcError(EUNSUPPORTED, "unsupported sizes")
         self.ws = torch.empty(self.workspace_bytes, dtype=torch.uint8, device=self.device)
@@ -475,21 +491,28 @@ class SplitSolver:
         self.r_prim = torch.empty(self.B, dtype=torch.float32, device=self.device)
         self.Qd = (c_float * NX)(*[float(v) for v in Qdiag]); self.Rd = (c_float * self.nu)(*[float(v) for v in Rdiag])
 
+    def launch_count(self):
+        """Kernel launches of one solve (factorisation + iterations + outputs)."""
+        scaled = self._sx is not None or self.opts.scale_u not in (0.0, 1.0)
+        per_it = 4 if self.opts.accel else 2
+        return 1 + per_it * self.iters - (2 if self.opts.accel else 0) + 1 + (3 if scaled else 0) + (1 if self.opts.accel else 0)
+
     def solve(self, A, Bm, c, x0, u_prev, x_ref, u_ref, contact, stream=None):
         prob = SplitProblem(*[None if t is None else t.data_ptr() for t in (A, Bm, c, x0, u_prev, x_ref, u_ref, contact)])
         st = c_void_p(self.torch.cuda.current_stream(self.device).cuda_stream if stream is None else stream.cuda_stream)
-        _check(load().pinmpc_split_solve(self.nu, self.N, self.B, ctypes.byref(self.layout), self.Qd, self.Rd, self.rho, self.iters,
-                                         ctypes.byref(prob), _ptr(self.ws), self.workspace_bytes, _ptr(self.xi), _ptr(self.z),
-                                         _ptr(self.r_prim), st))
+        _check(load().pinmpc_split_solve_ex(self.nu, self.N, self.B, ctypes.byref(self.layout), self.Qd, self.Rd, self.rho, self.iters,
+                                            ctypes.byref(prob), ctypes.byref(self.opts), _ptr(self.ws), self.workspace_bytes, _ptr(self.xi),
+                                            _ptr(self.z), _ptr(self.r_prim), st))
         return self.xi, self.z, self.r_prim
 
 
-def split_solve(A, Bm, c, x0, u_prev, x_ref, u_ref, contact, layout, Qdiag, Rdiag, rho, iters, stream=None):
-    """One pinmpc_split_solve call on torch CUDA tensors (float32, contiguous; c, u_prev, u_ref may be None).
-    Returns (xi [B,N,13+nu], z [B,N,13+nu], r_prim [B]); synchronises the stream."""
+def split_solve(A, Bm, c, x0, u_prev, x_ref, u_ref, contact, layout, Qdiag, Rdiag, rho, iters, stream=None, scale_x=None, scale_u=1.0,
+                accel=False, eta=0.999, return_restarts=False):
+    """One pinmpc_split_solve_ex call on torch CUDA tensors (float32, contiguous; c, u_prev, u_ref may be None).
+    Returns (xi [B,N,13+nu], z [B,N,13+nu], r_prim [B]) (+ restarts [B] int32 when asked for); synchronises the stream."""
     import torch
     B, N, _, nu = Bm.shape
-    s = SplitSolver(nu, N, B, layout, Qdiag, Rdiag, rho, iters, device=Bm.device)
+    s = SplitSolver(nu, N, B, layout, Qdiag, Rdiag, rho, iters, device=Bm.device, scale_x=scale_x, scale_u=scale_u, accel=accel, eta=eta)
     out = s.solve(A, Bm, c, x0, u_prev, x_ref, u_ref, contact, stream)
     torch.cuda.current_stream(Bm.device).synchronize()
-    return out
+    return out + (s.restarts,) if return_restarts else out

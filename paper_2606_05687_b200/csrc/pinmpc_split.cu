@@ -12,7 +12,17 @@
 //   k_split_b       (21b), (21c): gamma, gamma~, z = Proj((2 gamma~ + gamma)/3), v = (z + gamma)/2, dual updates
 // The factors stream from HBM every iteration (about 8.1 KB per stage-iteration at nu = 12): the method is
 // reported against the HBM roofline.
+//
+// pinmpc_split_solve_ex adds (oracle/split.py header):
+//   variable scaling   x = Sx x~, u = su u~: k_split_scale writes the scaled problem (A~ = Sx^-1 A Sx, B~ = su Sx^-1 B,
+//                      c~, references, xi_0) into the workspace once, Q~ = Sx^2 Q, R~ = su^2 R and the box bounds of
+//                      the wrench set / su go into the parameters, k_split_unscale scales xi and z back
+//   fast ADMM with restart on w = (z, v, theta, beta, lambda): (21a)/(21b) read the extrapolated point w^, (21b)
+//                      writes w_m into a ring of two buffers and the stage's share of the combined residual c_m;
+//                      k_split_decide (one thread per env, stages summed in order in double: deterministic) takes
+//                      the accept / restart decision, k_split_extrapolate forms w^_{m+1}
 #include "pinmpc_common.cuh"
+#include <cmath>
 
 namespace {
 
@@ -25,9 +35,14 @@ struct SplitPtrs {
     const uint8_t *contact;
     float *H, *G;                          // [st][n][n], [st][nu][nu]
     float *Tt;                             // [st][n][13]  [A_k B_k] transposed: column-major rows for coalesced reads in (21b)
-    float *xi, *du, *z, *v, *th, *be, *la; // [st][n] (du: [st][nu])
+    float *xi, *du;                        // [st][n], [st][nu]
+    const float *z, *v, *th, *be, *la;     // [st][n] the point the iteration starts from (w^ with acceleration)
+    float *nz, *nv, *nth, *nbe, *nla;      // [st][n] the point it produces (the same buffers without acceleration)
     float *rs;                             // [st] per-stage primal residual of the last iteration
+    float *cpart;                          // [st] per-stage share of the combined residual c_m (acceleration) or NULL
 };
+
+struct SplitScale { float sx[NX], isx[NX], su, isu; };
 
 // In-place Gauss-Jordan inverse of an SPD m x m matrix without pivoting: lane i holds row i in registers
 // (lanes >= m hold zero rows), the pivot row is broadcast with shuffles; everything is unrolled, so the rows
@@ -254,17 +269,90 @@ __global__ void __launch_bounds__(SPLIT_WARPS * 32) k_split_b(SolveParams P, Spl
     __syncwarp();
     const float z = isx ? w : (on ? uw[ju] : 0.0f);
     const float v = 0.5f * (z + gamma);
+    if (q.cpart) {
+        // c_m share of this stage: rho (|d theta|^2 + |d beta|^2 + |d lambda|^2 + |dz|^2 + |dv|^2 + |dz - dv|^2) against w^
+        float cs = 0.0f;
+        if (on) {
+            const float dth = xi - z, dbe = Bdu - v, dla = z - Axi - v - e;
+            const float dz = z - q.z[s * n + lane], dv = v - q.v[s * n + lane];
+            cs = dth * dth + dbe * dbe + dla * dla + dz * dz + dv * dv + (dz - dv) * (dz - dv);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) cs += __shfl_xor_sync(FULL, cs, o);
+        if (lane == 0) q.cpart[s] = P.rho * cs;
+    }
     if (on) {
-        q.z[s * n + lane] = z;
-        q.v[s * n + lane] = v;
-        q.th[s * n + lane] = th + xi - z;
-        q.be[s * n + lane] = be + Bdu - v;
-        q.la[s * n + lane] = la + z - Axi - v - e;
+        q.nz[s * n + lane] = z;
+        q.nv[s * n + lane] = v;
+        q.nth[s * n + lane] = th + xi - z;
+        q.nbe[s * n + lane] = be + Bdu - v;
+        q.nla[s * n + lane] = la + z - Axi - v - e;
     }
     if (last) {
         const float rmax = warp_max(on ? fabsf(xi - z) : 0.0f);
         if (lane == 0) q.rs[s] = rmax;
     }
+}
+
+// x = Sx x~, u = su u~: the scaled problem, written once.  One thread per element of the largest array (A or B).
+__global__ void k_split_scale(int B, int N, int nu, SplitScale S, const float *A, const float *Bm, const float *c, const float *x0,
+                              const float *u_prev, const float *x_ref, const float *u_ref, float *sA, float *sB, float *sc, float *sx0,
+                              float *sup, float *sxr, float *sur)
+{
+    const long st = (long)B * N, i = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < st * NX * NX) { const int r = (int)((i / NX) % NX), col = (int)(i % NX); sA[i] = A[i] * S.isx[r] * S.sx[col]; }
+    if (i < st * NX * nu) { const int r = (int)((i / nu) % NX); sB[i] = Bm[i] * S.isx[r] * S.su; }
+    if (i < st * NX) { const int r = (int)(i % NX); if (c) sc[i] = c[i] * S.isx[r]; sxr[i] = x_ref[i] * S.isx[r]; }
+    if (i < st * nu && u_ref) sur[i] = u_ref[i] * S.isu;
+    if (i < (long)B * NX) sx0[i] = x0[i] * S.isx[(int)(i % NX)];
+    if (i < (long)B * nu && u_prev) sup[i] = u_prev[i] * S.isu;
+}
+
+__global__ void k_split_unscale(long st, int n, SplitScale S, const float *in, float *out)
+{
+    const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= st * n) return;
+    const int j = (int)(i % n);
+    out[i] = in[i] * (j < NX ? S.sx[j] : S.su);
+}
+
+// Accept / restart decision of iteration m for every env (oracle/split.py header).  acc[b] = (alpha, c_prev, mom, restart).
+__global__ void k_split_decide(int B, int N, float eta, const float *cpart, float4 *acc, int *restarts)
+{
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= B) return;
+    double c = 0.0;
+    for (int k = 0; k < N; k++) c += (double)cpart[(long)b * N + k];
+    float4 a = acc[b];
+    const float cm = (float)c;
+    if (cm < eta * a.y) {
+        const float an = 0.5f * (1.0f + sqrtf(1.0f + 4.0f * a.x * a.x));
+        a.z = (a.x - 1.0f) / an; a.x = an; a.y = cm; a.w = 0.0f;
+    } else {
+        a.z = 0.0f; a.x = 1.0f; a.y = a.y / eta; a.w = 1.0f;
+        if (restarts) restarts[b] += 1;
+    }
+    acc[b] = a;
+}
+
+// w^_{m+1} = w_m + mom (w_m - w_{m-1}), or w_{m-1} after a restart; the five vectors z, v, theta, beta, lambda are
+// contiguous [5][st][n] in each buffer.
+__global__ void k_split_extrapolate(long st, int N, int n, const float4 *acc, const float *wm, const float *wp, float *hat)
+{
+    const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= 5 * st * n) return;
+    const long s = (i % (st * n)) / n;
+    const float4 a = acc[s / N];
+    const float m = wm[i], p = wp[i];
+    hat[i] = a.w != 0.0f ? p : fmaf(a.z, m - p, m);
+}
+
+__global__ void k_split_accel_init(int B, float4 *acc, int *restarts)
+{
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= B) return;
+    acc[b] = make_float4(1.0f, __int_as_float(0x7f800000), 0.0f, 0.0f);
+    if (restarts) restarts[b] = 0;
 }
 
 __global__ void k_split_residual(const float *rs, float *r_prim, int B, int N)
@@ -282,15 +370,43 @@ size_t split_floats(int nu, long st)
     return (size_t)st * (n * n + nu * nu + NX * n + 7 * n + nu + 1);
 }
 
-template <int NU>
-pinmpc_status run(const SolveParams &P, SplitPtrs q, int iters, float *r_prim, cudaStream_t stream)
+bool opt_scaled(const pinmpc_split_options *o) { return o && (o->h_scale_x != nullptr || (o->scale_u != 0.0f && o->scale_u != 1.0f)); }
+bool opt_accel(const pinmpc_split_options *o) { return o && o->accel != 0; }
+
+size_t split_floats_ex(int nu, long st, long B, const pinmpc_split_options *o)
 {
+    const long n = NX + nu;
+    size_t f = split_floats(nu, st);
+    if (opt_scaled(o)) f += (size_t)st * (NX * NX + NX * nu + 2 * NX + nu) + (size_t)B * n;
+    if (opt_accel(o)) f += (size_t)st * (10 * n + 1) + (size_t)B * 4 + 4;
+    return f;
+}
+
+template <int NU>
+pinmpc_status run(const SolveParams &P, SplitPtrs q, int iters, float *r_prim, bool accel, float eta, float *w1, float *hat, float4 *acc,
+                  int *restarts, cudaStream_t stream)
+{
+    constexpr int n = NX + NU;
     const long st = (long)P.B * P.N;
     const unsigned blocks = (unsigned)((st + SPLIT_WARPS - 1) / SPLIT_WARPS);
     k_split_factor<NU><<<blocks, SPLIT_WARPS * 32, 0, stream>>>(P, q);
+    float *w0 = q.nz;                                        // ring buffer 0 = the plain iteration's z, v, theta, beta, lambda
+    if (accel) {
+        k_split_accel_init<<<(P.B + 127) / 128, 128, 0, stream>>>(P.B, acc, restarts);
+        q.z = hat; q.v = hat + st * n; q.th = hat + 2 * st * n; q.be = hat + 3 * st * n; q.la = hat + 4 * st * n;
+    }
     for (int it = 0; it < iters; it++) {
+        if (accel) {
+            float *wm = (it & 1) ? w1 : w0;
+            q.nz = wm; q.nv = wm + st * n; q.nth = wm + 2 * st * n; q.nbe = wm + 3 * st * n; q.nla = wm + 4 * st * n;
+        }
         k_split_a<NU><<<blocks, SPLIT_WARPS * 32, 0, stream>>>(P, q);
         k_split_b<NU><<<blocks, SPLIT_WARPS * 32, 0, stream>>>(P, q, it == iters - 1 && r_prim != nullptr);
+        if (accel && it < iters - 1) {
+            k_split_decide<<<(P.B + 127) / 128, 128, 0, stream>>>(P.B, P.N, eta, q.cpart, acc, restarts);
+            const long tot = 5 * st * n;
+            k_split_extrapolate<<<(unsigned)((tot + 255) / 256), 256, 0, stream>>>(st, P.N, n, acc, (it & 1) ? w1 : w0, (it & 1) ? w0 : w1, hat);
+        }
     }
     if (r_prim) k_split_residual<<<(P.B + 127) / 128, 128, 0, stream>>>(q.rs, r_prim, P.B, P.N);
     return cudaGetLastError() == cudaSuccess ? PINMPC_OK : PINMPC_ECUDA;
@@ -298,30 +414,44 @@ pinmpc_status run(const SolveParams &P, SplitPtrs q, int iters, float *r_prim, c
 
 }   // namespace
 
-extern "C" size_t pinmpc_split_workspace_bytes(int nu, int N, int B)
+extern "C" size_t pinmpc_split_workspace_bytes_ex(int nu, int N, int B, const pinmpc_split_options *opts)
 {
     if ((nu != 12 && nu != 18) || N < 1 || N > PINMPC_SPLIT_N_MAX || B < 0) return 0;
-    return split_floats(nu, (long)B * N) * sizeof(float) + 256;
+    return split_floats_ex(nu, (long)B * N, B, opts) * sizeof(float) + 256;
 }
 
-extern "C" pinmpc_status pinmpc_split_solve(int nu, int N, int B, const pinmpc_layout *layout, const float *h_Qdiag, const float *h_Rdiag,
-                                            float rho, int iters, const pinmpc_split_problem *p, void *d_ws, size_t ws_bytes,
-                                            float *xi, float *z, float *r_prim, void *stream)
+extern "C" size_t pinmpc_split_workspace_bytes(int nu, int N, int B) { return pinmpc_split_workspace_bytes_ex(nu, N, B, nullptr); }
+
+extern "C" pinmpc_status pinmpc_split_solve_ex(int nu, int N, int B, const pinmpc_layout *layout, const float *h_Qdiag, const float *h_Rdiag,
+                                               float rho, int iters, const pinmpc_split_problem *p, const pinmpc_split_options *opts,
+                                               void *d_ws, size_t ws_bytes, float *xi, float *z, float *r_prim, void *stream)
 {
     if ((nu != 12 && nu != 18) || N < 1 || N > PINMPC_SPLIT_N_MAX) return PINMPC_EUNSUPPORTED;
     if (!layout || layout->n_wrench != 2 || 6 * layout->n_wrench + 3 * layout->n_force != nu) return PINMPC_EUNSUPPORTED;
     if (B < 0 || !(rho > 0.0f) || iters < 1 || !h_Qdiag || !h_Rdiag || !p) return PINMPC_EINVAL;
+    const bool scaled = opt_scaled(opts), accel = opt_accel(opts);
+    SplitScale S;
+    for (int i = 0; i < NX; i++) {
+        const float v = (opts && opts->h_scale_x) ? opts->h_scale_x[i] : 1.0f;
+        if (!(v > 0.0f) || !std::isfinite(v)) return PINMPC_EINVAL;
+        S.sx[i] = v; S.isx[i] = 1.0f / v;
+    }
+    S.su = (opts && opts->scale_u != 0.0f) ? opts->scale_u : 1.0f;
+    if (!(S.su > 0.0f) || !std::isfinite(S.su)) return PINMPC_EINVAL;
+    S.isu = 1.0f / S.su;
+    const float eta = (opts && opts->eta != 0.0f) ? opts->eta : 0.999f;
+    if (accel && !(eta > 0.0f && eta <= 1.0f)) return PINMPC_EINVAL;
     if (B == 0) return PINMPC_OK;
     if (!p->A || !p->Bm || !p->x0 || !p->x_ref || !p->contact || !d_ws) return PINMPC_EINVAL;
-    if (ws_bytes < pinmpc_split_workspace_bytes(nu, N, B)) return PINMPC_EALLOC;
+    if (ws_bytes < pinmpc_split_workspace_bytes_ex(nu, N, B, opts)) return PINMPC_EALLOC;
     cudaStream_t st_ = (cudaStream_t)stream;
     SolveParams P;
     memset(&P, 0, sizeof P);
     P.B = B; P.N = N; P.nu = nu; P.nw = layout->n_wrench; P.nf = layout->n_force; P.iters = iters; P.rho = rho;
-    P.mu = layout->mu; P.fz_max = layout->fz_max; P.cx = layout->mx_coef; P.cy = layout->my_coef; P.cz = layout->mz_coef;
-    P.hand_fmax = layout->hand_fmax;
-    for (int i = 0; i < NX; i++) { if (!(h_Qdiag[i] >= 0.0f)) return PINMPC_EINVAL; P.Qd[i] = h_Qdiag[i]; }
-    for (int i = 0; i < nu; i++) { if (!(h_Rdiag[i] >= 0.0f)) return PINMPC_EINVAL; P.Rd[i] = h_Rdiag[i]; }
+    P.mu = layout->mu; P.fz_max = layout->fz_max * S.isu; P.cx = layout->mx_coef; P.cy = layout->my_coef; P.cz = layout->mz_coef;
+    P.hand_fmax = layout->hand_fmax * S.isu;
+    for (int i = 0; i < NX; i++) { if (!(h_Qdiag[i] >= 0.0f)) return PINMPC_EINVAL; P.Qd[i] = h_Qdiag[i] * S.sx[i] * S.sx[i]; }
+    for (int i = 0; i < nu; i++) { if (!(h_Rdiag[i] >= 0.0f)) return PINMPC_EINVAL; P.Rd[i] = h_Rdiag[i] * S.su * S.su; }
     P.iw[0] = P.iw[1] = 1.0f / P.mu; P.iw[2] = 1.0f / P.cx; P.iw[3] = 1.0f / P.cy; P.iw[4] = 1.0f / P.cz;
     const long stg = (long)B * N, n = NX + nu;
     float *w = reinterpret_cast<float *>(((uintptr_t)d_ws + 255) & ~(uintptr_t)255);
@@ -330,15 +460,59 @@ extern "C" pinmpc_status pinmpc_split_solve(int nu, int N, int B, const pinmpc_l
     q.H = w; w += stg * n * n;
     q.G = w; w += stg * nu * nu;
     q.Tt = w; w += stg * NX * n;
-    q.xi = w; w += stg * n; q.z = w; w += stg * n; q.v = w; w += stg * n; q.th = w; w += stg * n; q.be = w; w += stg * n; q.la = w; w += stg * n;
+    q.xi = w; w += stg * n;
+    float *w0 = w; w += 5 * stg * n;
+    q.nz = w0; q.nv = w0 + stg * n; q.nth = w0 + 2 * stg * n; q.nbe = w0 + 3 * stg * n; q.nla = w0 + 4 * stg * n;
+    q.z = q.nz; q.v = q.nv; q.th = q.nth; q.be = q.nbe; q.la = q.nla;
     q.du = w; w += stg * nu;
     q.rs = w; w += stg;
+    q.cpart = nullptr;
+    if (scaled) {
+        float *sA = w; w += stg * NX * NX;
+        float *sB = w; w += stg * NX * nu;
+        float *sc = w; w += stg * NX;
+        float *sxr = w; w += stg * NX;
+        float *sur = w; w += stg * nu;
+        float *sx0 = w; w += (long)B * NX;
+        float *sup = w; w += (long)B * nu;
+        const long tot = stg * NX * (nu > NX ? nu : NX);
+        k_split_scale<<<(unsigned)((tot + 255) / 256), 256, 0, st_>>>(B, N, nu, S, p->A, p->Bm, p->c, p->x0, p->u_prev, p->x_ref, p->u_ref, sA, sB, sc,
+                                                                     sx0, sup, sxr, sur);
+        q.A = sA; q.Bm = sB; q.c = p->c ? sc : nullptr; q.x0 = sx0; q.u_prev = p->u_prev ? sup : nullptr; q.x_ref = sxr;
+        q.u_ref = p->u_ref ? sur : nullptr;
+    }
+    float *w1 = nullptr, *hat = nullptr;
+    float4 *acc = nullptr;
+    if (accel) {
+        w1 = w; w += 5 * stg * n;
+        hat = w; w += 5 * stg * n;
+        q.cpart = w; w += stg;
+        w = reinterpret_cast<float *>(((uintptr_t)w + 15) & ~(uintptr_t)15);
+        acc = reinterpret_cast<float4 *>(w); w += (long)B * 4;
+        if (cudaMemsetAsync(w1, 0, (size_t)stg * n * 10 * sizeof(float), st_) != cudaSuccess) return PINMPC_ECUDA;
+    }
     // all iterates start at 0 (z, v, theta, beta, lambda are contiguous)
-    if (cudaMemsetAsync(q.z, 0, (size_t)stg * n * 5 * sizeof(float), st_) != cudaSuccess) return PINMPC_ECUDA;
-    pinmpc_status rc = nu == 12 ? run<12>(P, q, iters, r_prim, st_) : run<18>(P, q, iters, r_prim, st_);
+    if (cudaMemsetAsync(w0, 0, (size_t)stg * n * 5 * sizeof(float), st_) != cudaSuccess) return PINMPC_ECUDA;
+    int *restarts = (accel && opts) ? opts->d_restarts : nullptr;
+    pinmpc_status rc = nu == 12 ? run<12>(P, q, iters, r_prim, accel, eta, w1, hat, acc, restarts, st_)
+                                : run<18>(P, q, iters, r_prim, accel, eta, w1, hat, acc, restarts, st_);
     if (rc != PINMPC_OK) return rc;
+    const float *zlast = (accel && ((iters - 1) & 1)) ? w1 : w0;
     const size_t bytes = (size_t)stg * n * sizeof(float);
+    if (scaled) {
+        const long tot = stg * n;
+        if (xi) k_split_unscale<<<(unsigned)((tot + 255) / 256), 256, 0, st_>>>(stg, (int)n, S, q.xi, xi);
+        if (z) k_split_unscale<<<(unsigned)((tot + 255) / 256), 256, 0, st_>>>(stg, (int)n, S, zlast, z);
+        return cudaGetLastError() == cudaSuccess ? PINMPC_OK : PINMPC_ECUDA;
+    }
     if (xi && cudaMemcpyAsync(xi, q.xi, bytes, cudaMemcpyDeviceToDevice, st_) != cudaSuccess) return PINMPC_ECUDA;
-    if (z && cudaMemcpyAsync(z, q.z, bytes, cudaMemcpyDeviceToDevice, st_) != cudaSuccess) return PINMPC_ECUDA;
+    if (z && cudaMemcpyAsync(z, zlast, bytes, cudaMemcpyDeviceToDevice, st_) != cudaSuccess) return PINMPC_ECUDA;
     return PINMPC_OK;
+}
+
+extern "C" pinmpc_status pinmpc_split_solve(int nu, int N, int B, const pinmpc_layout *layout, const float *h_Qdiag, const float *h_Rdiag,
+                                            float rho, int iters, const pinmpc_split_problem *p, void *d_ws, size_t ws_bytes,
+                                            float *xi, float *z, float *r_prim, void *stream)
+{
+    return pinmpc_split_solve_ex(nu, N, B, layout, h_Qdiag, h_Rdiag, rho, iters, p, nullptr, d_ws, ws_bytes, xi, z, r_prim, stream);
 }
