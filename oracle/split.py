@@ -23,8 +23,9 @@ One env, generic LTV data A[N,nx,nx], Bm[N,nx,nu], e[N,nx].  Notation of the pap
 
 Readings: the paper prints eb_k inside the Ab_{k+1}^T term of h_k; stationarity of the (20d)
 term of stage k+1 requires eb_{k+1} and that is what is used; xi_0 = [x_0 ; u_{-1}] is data and
-never updated (in the gamma terms of stage 0 it enters as a constant); all iterates start at 0; X_k = R^nx, so the
-projection acts on the u part only (the set of stage k, since xi_{k+1} carries u_k).
+never updated (in the gamma terms of stage 0 it enters as a constant); all iterates start at 0; X_k = R^nx unless a
+box is given (x_lo, x_hi), so the projection acts on the u part (the set of stage k, since xi_{k+1} carries u_k) and
+clips the x part to the box.
 
 Variable scaling (PAPER.md:L184 leaves rho and the units open; with one scalar rho the iteration stalls on
 the SRB problem's units).  `scale_x` (nx positive numbers) and `scale_u` (one positive number) define x = Sx x~,
@@ -74,11 +75,13 @@ def factors(Ab, Bb, Qb, rho):
 
 
 def solve_env(A, Bm, e, Qd, Rd, rho, iters, x0, u_prev, x_ref, u_ref, project_u, state=None, scale_x=None, scale_u=1.0,
-              accel=False, eta=0.999, trace=None):
+              accel=False, eta=0.999, trace=None, x_lo=None, x_hi=None):
     """project_u(k, v[nu]) -> Proj_{U_k}(v) in the caller's units.  Returns dict(xi[N,n], z[N,n], du[N,nu], v, theta, beta, lam, r_prim[, restarts, c]) in the caller's units.
 
     xi[k] = xi_{k+1} = [x_{k+1}; u_k].  r_prim = max_k |xi_{k+1} - z_{k+1}|_inf of the last iteration (scaled variables).
-    trace: optional list, receives (xi, z) in the caller's units after every iteration."""
+    trace: optional list, receives (xi, z) in the caller's units after every iteration.
+    x_lo, x_hi [nx] (caller's units, +-inf allowed): the state set X_k of (17) as a box, xi_{k+1} in X_k; the projection of
+    (21b) then clips the x part of z (Xb_k = X_k x U_k)."""
     A = np.asarray(A, dtype=np.float64); Bm = np.asarray(Bm, dtype=np.float64); e = np.asarray(e, dtype=np.float64)
     N, nx, nu = Bm.shape
     n = nx + nu
@@ -121,7 +124,7 @@ def solve_env(A, Bm, e, Qd, Rd, rho, iters, x0, u_prev, x_ref, u_ref, project_u,
             gamma = Bdu + beta[k] - Axi - eb[k] + lam[k]
             gammat = xi[k] + theta[k] + Axi + eb[k] - lam[k]
             w = (2.0 * gammat + gamma) / 3.0
-            zn[k, :nx] = w[:nx]
+            zn[k, :nx] = w[:nx] if x_lo is None else np.clip(w[:nx], np.asarray(x_lo, dtype=np.float64) / sx, np.asarray(x_hi, dtype=np.float64) / sx)
             zn[k, nx:] = proj(k, w[nx:])
             vn[k] = 0.5 * (zn[k] + gamma)
             theta[k] = theta[k] + xi[k] - zn[k]

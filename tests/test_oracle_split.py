@@ -252,3 +252,36 @@ def test_accelerated_iteration_on_an_unconstrained_problem_is_faster():
         return int(np.argmax(errs < 1e-6)) + 1
     n_plain, n_acc = iters_to(False), iters_to(True)
     assert n_acc < n_plain, (n_plain, n_acc)
+
+
+def test_state_box_limit_is_the_qp_optimum():
+    """xi_{k+1} in X_k (a box on the states, eq. (17)) next to the input box: the limit equals the optimum of the
+    condensed QP with linear inequality constraints on X = S U + d, solved by SLSQP and polished on its active set."""
+    from scipy.optimize import minimize
+    N, nx, nu = 5, 3, 2
+    A, Bm, e, Qd, Rd, x0, u_prev, x_ref, u_ref, lo, hi = _box_problem(31, N, nx, nu)
+    free = split.solve_env(A, Bm, e, Qd, Rd, 1.0, 20000, x0, u_prev, x_ref, u_ref, lambda k, v: np.clip(v, lo, hi))
+    xf = free["z"][:, :nx]
+    x_lo = np.array([xf[:, 0].min() + 0.3 * np.ptp(xf[:, 0]), -np.inf, -np.inf])           # cuts into the free optimum
+    x_hi = np.array([np.inf, xf[:, 1].max() - 0.3 * np.ptp(xf[:, 1]), np.inf])
+    out = split.solve_env(A, Bm, e, Qd, Rd, 1.0, 60000, x0, u_prev, x_ref, u_ref, lambda k, v: np.clip(v, lo, hi), x_lo=x_lo, x_hi=x_hi)
+    S, d = condense(A, Bm, e, x0)
+    Wq = np.kron(np.eye(N), np.diag(Qd)); Wr = np.kron(np.eye(N), np.diag(Rd))
+    cost = lambda U: 0.5 * (S @ U + d - x_ref.reshape(-1)) @ Wq @ (S @ U + d - x_ref.reshape(-1)) + 0.5 * (U - u_ref.reshape(-1)) @ Wr @ (U - u_ref.reshape(-1))
+    grad = lambda U: S.T @ Wq @ (S @ U + d - x_ref.reshape(-1)) + Wr @ (U - u_ref.reshape(-1))
+    cons = []
+    Xlo, Xhi = np.tile(x_lo, N), np.tile(x_hi, N)
+    for i in range(N * nx):
+        if np.isfinite(Xlo[i]):
+            cons.append(dict(type="ineq", fun=lambda U, i=i: S[i] @ U + d[i] - Xlo[i], jac=lambda U, i=i: S[i]))
+        if np.isfinite(Xhi[i]):
+            cons.append(dict(type="ineq", fun=lambda U, i=i: Xhi[i] - S[i] @ U - d[i], jac=lambda U, i=i: -S[i]))
+    res = minimize(cost, np.zeros(N * nu), jac=grad, bounds=list(zip(np.tile(lo, N), np.tile(hi, N))), constraints=cons, method="SLSQP",
+                   options=dict(ftol=1e-15, maxiter=2000))
+    U = res.x; X = (S @ U + d).reshape(N, nx)
+    assert res.success
+    assert np.sum(np.abs(X[:, 0] - x_lo[0]) < 1e-7) + np.sum(np.abs(X[:, 1] - x_hi[1]) < 1e-7) >= 2   # the state box is active
+    assert np.abs(out["z"][:, nx:] - U.reshape(N, nu)).max() < 2e-5
+    assert np.abs(out["z"][:, :nx] - X).max() < 2e-5
+    assert np.all(out["z"][:, 0] >= x_lo[0] - 1e-12) and np.all(out["z"][:, 1] <= x_hi[1] + 1e-12)
+    assert cost(out["z"][:, nx:].reshape(-1)) <= cost(U) + 1e-7
