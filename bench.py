@@ -97,6 +97,8 @@ def parse():
                     help="time the paper's own stage-local ADMM (pinmpc_split_solve) on the config instead (one JSON line)")
     ap.add_argument("--split-scaled", action="store_true", help="--split with the variable scaling Sx = Q^-1/2, su = 100 (DESIGN.md 7c)")
     ap.add_argument("--split-accel", action="store_true", help="--split with Nesterov acceleration and restart")
+    ap.add_argument("--centroidal", action="store_true",
+                    help="--split on the paper's own 9-state centroidal model (eq. (1)-(4)) with the state box of gen.centroidal_view, scaled")
     ap.add_argument("--converge", action="store_true",
                     help="iterations to tolerance x ms per iteration for the exact-dynamics path and the stage-local method (one JSON line per setting)")
     ap.add_argument("--split-sweep", action="store_true",
@@ -245,13 +247,20 @@ def run_split(args):
     d = lambda a, t=torch.float32: None if a is None else torch.from_numpy(np.ascontiguousarray(a)).to(dev, t)
     x0, x_ref, u_ref, contact = d(w.x0), d(w.x_ref), d(w.u_ref), d(w.contact, torch.uint8)
     opts = {}
-    if args.split_scaled:
+    Qd, nx = w.Qdiag, 13
+    if args.centroidal:
+        from paper_2606_05687_b200 import binding
+        v = gen.centroidal_view(w)
+        A, Bm, c = binding.assemble_centroidal(w.n_wrench, w.n_force, w.dt, d(w.mass), d(w.foot_r))
+        x0, x_ref, Qd, nx = d(v["x0"]), d(v["x_ref"]), v["Qdiag"], 9
+        opts.update(nx=9, x_lo=v["x_lo"], x_hi=v["x_hi"], scale_x=[1.0 / float(q) ** 0.5 for q in Qd], scale_u=100.0)
+    if args.split_scaled and not args.centroidal:
         opts.update(scale_x=split_scale_x(w), scale_u=100.0)
     if args.split_accel:
         opts.update(accel=True)
-    sp = SplitSolver(w.nu, w.N, w.B, lay, w.Qdiag, w.Rdiag, w.rho, w.iters, device=dev, **opts)
+    sp = SplitSolver(w.nu, w.N, w.B, lay, Qd, w.Rdiag, w.rho, w.iters, device=dev, **opts)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
-    run = lambda: sp.solve(A, Bm, c if w.ext_wrench is not None else None, x0, None, x_ref, u_ref, contact)
+    run = lambda: sp.solve(A, Bm, c if (w.ext_wrench is not None or args.centroidal) else None, x0, None, x_ref, u_ref, contact)
     for _ in range(max(args.warmup, 3)):
         run()
     torch.cuda.synchronize(dev)
@@ -263,11 +272,11 @@ def run_split(args):
         torch.cuda.synchronize(dev)
         ts.append(a.elapsed_time(b))
     ms = float(np.mean(ts))
-    n = 13 + w.nu
+    n = nx + w.nu
     st = w.B * w.N
-    # algorithmic bytes per stage-iteration: (21a) reads H_k (n^2), G_k (nu^2), B_k (13 nu), [A_{k+1} B_{k+1}] (13 n);
-    # (21b,c) reads [A_k B_k]^T (13 n); lifted vectors: 6 read + xi, du written in (21a), 5 read + 5 written in (21b,c)
-    per_stage_iter = 4 * (n * n + w.nu * w.nu + 13 * w.nu + 2 * 13 * n + 18 * n)
+    # algorithmic bytes per stage-iteration: (21a) reads H_k (n^2), G_k (nu^2), B_k (nx nu), [A_{k+1} B_{k+1}] (nx n);
+    # (21b,c) reads [A_k B_k]^T (nx n); lifted vectors: 6 read + xi, du written in (21a), 5 read + 5 written in (21b,c)
+    per_stage_iter = 4 * (n * n + w.nu * w.nu + nx * w.nu + 2 * nx * n + 18 * n)
     gbs = per_stage_iter * st * w.iters / (ms * 1e-3) / 1e9
     try:
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
@@ -276,13 +285,14 @@ def run_split(args):
     print(json.dumps({"metric": "stage-local ADMM (paper eq. 22) solves/s", "value": w.B / (ms * 1e-3), "unit": "solves/s",
                       "ms_per_step": ms, "steps": args.steps, "n_gpus": 1, "dtype": "f32", "data": "synthetic",
                       "config": {"workload": w.name, "B": w.B, "N": w.N, "iters": w.iters, "nu": w.nu, "method": "split",
-                                 "scaled": bool(args.split_scaled), "accel": bool(args.split_accel)},
+                                 "scaled": bool(args.split_scaled or args.centroidal), "accel": bool(args.split_accel),
+                                 "model": "centroidal 9-state (eq. 1-4), state box" if args.centroidal else "SRB 13-state"},
                       "stage_iters_per_s": st * w.iters / (ms * 1e-3), "gpu_launches": sp.launch_count(),
                       "roofline": {"bound": "hbm", "achieved": gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                                    "frac": gbs / peaks["hbm_gbs"],
                                    # dram read + write of one k_split_a plus one k_split_b launch (one iteration),
                                    # ncu --set full, profiles/r1_split_ncu.md; measured at config 2 only
-                                   "traffic": (1016841000 + 31662592 + 358631936 + 81859584) if w.name == "c2_long_horizon" else None,
+                                   "traffic": (1016841000 + 31662592 + 358631936 + 81859584) if (w.name == "c2_long_horizon" and not opts) else None,
                                    "traffic_unit": "bytes per iteration (both kernels)",
                                    "bytes_per_stage_iter": per_stage_iter, "scope": "whole solve (factorisation + all iterations)"},
                       "workspace_mb": sp.workspace_bytes / 1e6, "r_prim_max": float(sp.r_prim.max())}))
@@ -484,7 +494,7 @@ def main():
         return write_traffic(args.write_traffic, gen.make_config(args.config, B=args.B, N=args.N).name)
     if args.impl == "reference":
         return run_reference(args)
-    if args.split:
+    if args.split or args.centroidal:
         return run_split(args)
     if args.split_sweep:
         return run_split_sweep(args)

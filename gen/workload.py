@@ -213,3 +213,20 @@ def subset(w: Workload, env_idx) -> Workload:
         v = getattr(w, a)
         kw[a] = None if v is None else np.ascontiguousarray(v[env_idx])
     return replace(w, B=int(env_idx.size), name=f"{w.name}_sub{env_idx.size}", **kw)
+
+
+def centroidal_view(w: Workload) -> dict:
+    """Inputs of the paper's 9-state centroidal model (eq. (1): xi = [c ; l_G ; k_G]) for the same synthetic
+    episode: CoM position from the position entries of the 13-state arrays, momenta as mass x velocity entries and
+    body-inertia diagonal x angular-velocity entries (inputs only; the dynamics come from the assembly).  Adds fixed
+    weights of the momenta's units and a state box X_k (eq. (17)): a CoM height ceiling and a bound on the fore-aft
+    linear momentum, chosen so that both bind on part of the envs."""
+    m = w.mass.astype(np.float64)
+    Ib = np.diagonal(w.inertia.astype(np.float64), axis1=1, axis2=2)
+    x0 = np.concatenate([w.x0[:, 3:6], m[:, None] * w.x0[:, 9:12], Ib * w.x0[:, 6:9]], axis=-1)
+    x_ref = np.concatenate([w.x_ref[..., 3:6], m[:, None, None] * w.x_ref[..., 9:12], Ib[:, None, :] * w.x_ref[..., 6:9]], axis=-1)
+    Qd = np.array([50.0, 50.0, 200.0, 1e-2, 1e-2, 5e-3, 0.4, 0.4, 0.4])
+    x_lo = np.array([-np.inf, -np.inf, 0.80, -20.0, -np.inf, -np.inf, -np.inf, -np.inf, -np.inf])
+    x_hi = np.array([np.inf, np.inf, 0.905, 20.0, np.inf, np.inf, np.inf, np.inf, np.inf])
+    return dict(x0=x0.astype(np.float32), x_ref=x_ref.astype(np.float32), Qdiag=Qd.astype(np.float32),
+                x_lo=x_lo.astype(np.float32), x_hi=x_hi.astype(np.float32))

@@ -275,13 +275,19 @@ pinmpc_status pinmpc_split_solve(int nu, int N, int B, const pinmpc_layout *layo
  *    c_m = rho (|theta_m - theta^_m|^2 + |beta_m - beta^_m|^2 + |lambda_m - lambda^_m|^2 + |dz|^2 + |dv|^2 + |dz - dv|^2)
  *    summed over the env's stages; c_m < eta c_{m-1}: a_{m+1} = (1 + sqrt(1 + 4 a_m^2)) / 2, w^_{m+1} = w_m +
  *    (a_m - 1) / a_{m+1} (w_m - w_{m-1}); else restart: a_{m+1} = 1, w^_{m+1} = w_{m-1}, c_m <- c_{m-1} / eta.
- *    Every env decides for itself.  z is w_M of the last iteration. */
+ *    Every env decides for itself.  z is w_M of the last iteration.
+ *  - nx, h_x_lo, h_x_hi: the state dimension (all [..,13] shapes of pinmpc_split_problem become [..,nx], xi and z are
+ *    [B,N,nx+nu]) and the state box of eq. (17): the projection of (21b) clips the x part of z to it. */
 typedef struct {
     const float *h_scale_x;    /* HOST [13] positive, or NULL => 1                                    */
     float scale_u;             /* > 0; 0 => 1                                                         */
     int accel;                 /* 0 plain iteration, 1 accelerated with restart                       */
     float eta;                 /* restart threshold in (0, 1]; 0 => 0.999                             */
     int *d_restarts;           /* DEVICE [B] or NULL: restarts taken per env (accel only)             */
+    int nx;                    /* state dimension of A, Bm, c, x0, x_ref: 13 (0 => 13) or 9 (the      */
+                               /* centroidal model of eq. (1)-(4)); Qdiag, scale_x, x_lo, x_hi: [nx]  */
+    const float *h_x_lo;       /* HOST [nx] or NULL: the state set X_k of eq. (17) as a box on        */
+    const float *h_x_hi;       /* xi_{k+1} (caller's units, -INFINITY / INFINITY = free); NULL => R^nx */
 } pinmpc_split_options;
 
 /* Workspace of pinmpc_split_solve_ex for these options (scaling adds the scaled problem, about 1.5 KB per stage at
@@ -289,10 +295,18 @@ typedef struct {
 size_t pinmpc_split_workspace_bytes_ex(int nu, int N, int B, const pinmpc_split_options *opts);
 
 /* pinmpc_split_solve with options.  Extra errors: PINMPC_EINVAL for a non-positive or non-finite scale, eta outside
- * (0, 1]. */
+ * (0, 1], x_lo > x_hi; PINMPC_EUNSUPPORTED for nx not in {0, 9, 13}. */
 pinmpc_status pinmpc_split_solve_ex(int nu, int N, int B, const pinmpc_layout *layout, const float *h_Qdiag, const float *h_Rdiag,
                                     float rho, int iters, const pinmpc_split_problem *p, const pinmpc_split_options *opts,
                                     void *d_workspace, size_t workspace_bytes, float *xi, float *z, float *r_prim, void *stream);
+
+/* The paper's own 9-state centroidal model (eq. (1)-(4)): xi = [c ; l_G ; k_G] (CoM position, linear
+ * and angular centroidal momentum), forward Euler; the lever r_{i,k} = p_{i,k} - c_k of contact i is data.
+ * Writes the LTV system of eq. (16), xi_{k+1} = A xi_k + B_k u_k + e:  A [B,N,9,9], Bm [B,N,9,nu], e [B,N,9] with
+ * nu = 6 n_wrench + 3 n_force and the input layout above; mass [B], foot_r [B,N,n_wrench+n_force,3]; all DEVICE, float32.
+ * Feed them to pinmpc_split_solve_ex with options.nx = 9.  PINMPC_EINVAL: NULL pointer, dt <= 0, no contact; B = 0: no-op. */
+pinmpc_status pinmpc_assemble_centroidal(int B, int N, int n_wrench, int n_force, float dt, const float *mass, const float *foot_r,
+                                         float *A, float *Bm, float *e, void *stream);
 
 /* Human-readable description of the last error on this handle (owned by the handle; "" if none).
  * With h = NULL: the last pinmpc_create failure in this thread. */

@@ -27,7 +27,7 @@ EXPORTS = ("pinmpc_workspace_bytes", "pinmpc_workspace_bytes_method", "pinmpc_cr
            "pinmpc_destroy", "pinmpc_set_profiling", "pinmpc_get_kernel_ms",
            "pinmpc_set_warm_start", "pinmpc_shift_aux", "pinmpc_landmark_ring_bytes", "pinmpc_landmark_reset", "pinmpc_landmark_push",
            "pinmpc_landmark_push_solver", "pinmpc_landmark_reward", "pinmpc_split_workspace_bytes", "pinmpc_split_solve",
-           "pinmpc_split_workspace_bytes_ex", "pinmpc_split_solve_ex")
+           "pinmpc_split_workspace_bytes_ex", "pinmpc_split_solve_ex", "pinmpc_assemble_centroidal")
 MAX_LANDMARKS = 8
 
 
@@ -52,7 +52,8 @@ class SplitProblem(ctypes.Structure):
 
 
 class SplitOptions(ctypes.Structure):
-    _fields_ = [("h_scale_x", POINTER(c_float)), ("scale_u", c_float), ("accel", c_int), ("eta", c_float), ("d_restarts", c_void_p)]
+    _fields_ = [("h_scale_x", POINTER(c_float)), ("scale_u", c_float), ("accel", c_int), ("eta", c_float), ("d_restarts", c_void_p),
+                ("nx", c_int), ("h_x_lo", POINTER(c_float)), ("h_x_hi", POINTER(c_float))]
 
 
 class LandmarkCfg(ctypes.Structure):
@@ -138,6 +139,8 @@ def load():
     lib.pinmpc_split_solve_ex.argtypes = [c_int, c_int, c_int, POINTER(Layout), POINTER(c_float), POINTER(c_float), c_float, c_int,
                                           POINTER(SplitProblem), POINTER(SplitOptions), c_void_p, c_size_t, c_void_p, c_void_p, c_void_p,
                                           c_void_p]
+    lib.pinmpc_assemble_centroidal.restype = c_int
+    lib.pinmpc_assemble_centroidal.argtypes = [c_int, c_int, c_int, c_int, c_float] + [c_void_p] * 6
     lib.pinmpc_destroy.restype = None
     lib.pinmpc_destroy.argtypes = [c_void_p]
     _lib = lib
@@ -474,22 +477,27 @@ class SplitSolver:
     """Owns the workspace and the output tensors of pinmpc_split_solve_ex; solve() is one asynchronous C-ABI call.
     scale_x (13 positive numbers) / scale_u: variable scaling; accel: Nesterov acceleration with restart (include/pinmpc.h)."""
 
-    def __init__(self, nu, N, B, layout, Qdiag, Rdiag, rho, iters, device="cuda:0", scale_x=None, scale_u=1.0, accel=False, eta=0.999):
+    def __init__(self, nu, N, B, layout, Qdiag, Rdiag, rho, iters, device="cuda:0", scale_x=None, scale_u=1.0, accel=False, eta=0.999,
+                 nx=NX, x_lo=None, x_hi=None):
         import torch
         self.torch, self.device = torch, torch.device(device)
         self.nu, self.N, self.B, self.layout, self.rho, self.iters = int(nu), int(N), int(B), layout, float(rho), int(iters)
+        self.nx = int(nx)
         self.restarts = torch.zeros(self.B, dtype=torch.int32, device=self.device) if accel else None
-        self._sx = None if scale_x is None else (c_float * NX)(*[float(v) for v in scale_x])
-        self.opts = SplitOptions(self._sx if self._sx is not None else ctypes.cast(None, POINTER(c_float)), float(scale_u), int(bool(accel)),
-                                 float(eta), None if self.restarts is None else self.restarts.data_ptr())
+        arr = lambda a: None if a is None else (c_float * self.nx)(*[float(v) for v in a])
+        null = ctypes.cast(None, POINTER(c_float))
+        self._sx, self._lo, self._hi = arr(scale_x), arr(x_lo), arr(x_hi)
+        self.opts = SplitOptions(self._sx if self._sx is not None else null, float(scale_u), int(bool(accel)),
+                                 float(eta), None if self.restarts is None else self.restarts.data_ptr(), self.nx,
+                                 self._lo if self._lo is not None else null, self._hi if self._hi is not None else null)
         self.workspace_bytes = load().pinmpc_split_workspace_bytes_ex(self.nu, self.N, self.B, ctypes.byref(self.opts))
         if self.workspace_bytes == 0:
             raise PinmpcError(EUNSUPPORTED, "unsupported sizes")
         self.ws = torch.empty(self.workspace_bytes, dtype=torch.uint8, device=self.device)
-        self.xi = torch.empty((self.B, self.N, NX + self.nu), dtype=torch.float32, device=self.device)
+        self.xi = torch.empty((self.B, self.N, self.nx + self.nu), dtype=torch.float32, device=self.device)
         self.z = torch.empty_like(self.xi)
         self.r_prim = torch.empty(self.B, dtype=torch.float32, device=self.device)
-        self.Qd = (c_float * NX)(*[float(v) for v in Qdiag]); self.Rd = (c_float * self.nu)(*[float(v) for v in Rdiag])
+        self.Qd = (c_float * NX)(*([float(v) for v in Qdiag] + [0.0] * (NX - len(Qdiag)))); self.Rd = (c_float * self.nu)(*[float(v) for v in Rdiag])
 
     def launch_count(self):
         """Kernel launches of one solve (factorisation + iterations + outputs)."""
@@ -506,13 +514,29 @@ class SplitSolver:
         return self.xi, self.z, self.r_prim
 
 
+def assemble_centroidal(n_wrench, n_force, dt, mass, foot_r, stream=None):
+    """pinmpc_assemble_centroidal on torch CUDA tensors: mass [B], foot_r [B,N,nc,3] -> A [B,N,9,9], Bm [B,N,9,nu], e [B,N,9]."""
+    import torch
+    B, N = foot_r.shape[:2]
+    nu = 6 * n_wrench + 3 * n_force
+    A = torch.empty((B, N, 9, 9), dtype=torch.float32, device=foot_r.device)
+    Bm = torch.empty((B, N, 9, nu), dtype=torch.float32, device=foot_r.device)
+    e = torch.empty((B, N, 9), dtype=torch.float32, device=foot_r.device)
+    st = c_void_p(torch.cuda.current_stream(foot_r.device).cuda_stream if stream is None else stream.cuda_stream)
+    rc = load().pinmpc_assemble_centroidal(B, N, n_wrench, n_force, float(dt), _ptr(mass), _ptr(foot_r), _ptr(A), _ptr(Bm), _ptr(e), st)
+    if rc != OK:
+        raise PinmpcError(rc, "pinmpc_assemble_centroidal")
+    return A, Bm, e
+
+
 def split_solve(A, Bm, c, x0, u_prev, x_ref, u_ref, contact, layout, Qdiag, Rdiag, rho, iters, stream=None, scale_x=None, scale_u=1.0,
-                accel=False, eta=0.999, return_restarts=False):
+                accel=False, eta=0.999, return_restarts=False, x_lo=None, x_hi=None):
     """One pinmpc_split_solve_ex call on torch CUDA tensors (float32, contiguous; c, u_prev, u_ref may be None).
     Returns (xi [B,N,13+nu], z [B,N,13+nu], r_prim [B]) (+ restarts [B] int32 when asked for); synchronises the stream."""
     import torch
-    B, N, _, nu = Bm.shape
-    s = SplitSolver(nu, N, B, layout, Qdiag, Rdiag, rho, iters, device=Bm.device, scale_x=scale_x, scale_u=scale_u, accel=accel, eta=eta)
+    B, N, nx, nu = Bm.shape
+    s = SplitSolver(nu, N, B, layout, Qdiag, Rdiag, rho, iters, device=Bm.device, scale_x=scale_x, scale_u=scale_u, accel=accel, eta=eta,
+                    nx=nx, x_lo=x_lo, x_hi=x_hi)
     out = s.solve(A, Bm, c, x0, u_prev, x_ref, u_ref, contact, stream)
     torch.cuda.current_stream(Bm.device).synchronize()
     return out + (s.restarts,) if return_restarts else out

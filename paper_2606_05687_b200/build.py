@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpinmpc.so")
-SOURCES = ["pinmpc_api.cu", "pinmpc_dense.cu", "pinmpc_srb.cu", "pinmpc_tmem.cu", "pinmpc_landmarks.cu", "pinmpc_split.cu"]
+SOURCES = ["pinmpc_api.cu", "pinmpc_dense.cu", "pinmpc_srb.cu", "pinmpc_tmem.cu", "pinmpc_landmarks.cu", "pinmpc_split.cu", "pinmpc_centroidal.cu"]
 # bench-only helper (a register-resident FMA loop that measures the FP32 peak): its own library, not part of the product ABI
 PROBE_SRC = "bench_probe.cu"
 PROBE_LIB = os.path.join(HERE, "libpinmpc_benchprobe.so")

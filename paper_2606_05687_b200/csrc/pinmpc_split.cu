@@ -1,6 +1,7 @@
 // The paper's own stage-local ADMM (pi^n MPC proper), eq. (18)-(22); SURVEY 8(f) rank 1.
 // Second method next to the exact-dynamics solver: no recursion over the horizon, every update is local to a
-// stage and reads at most the neighbouring stage.  Generic dense LTV data (A_k, B_k, c_k), nx = 13.
+// stage and reads at most the neighbouring stage.  Generic dense LTV data (A_k, B_k, c_k), nx = 13 (the SRB model)
+// or nx = 9 (the paper's centroidal model, eq. (1)-(4)); a box X_k on the states (eq. (17)) is part of the projection.
 //
 // Lifted state xi_k = [x_k ; u_{k-1}] (n = 13 + nu <= 31), Ab = [[A, B],[0, I]], Bb = [B ; I], eb = [c ; 0].
 // One warp per stage, lane i = component i of the lifted vectors; matrices are read so that consecutive lanes
@@ -40,6 +41,7 @@ struct SplitPtrs {
     float *nz, *nv, *nth, *nbe, *nla;      // [st][n] the point it produces (the same buffers without acceleration)
     float *rs;                             // [st] per-stage primal residual of the last iteration
     float *cpart;                          // [st] per-stage share of the combined residual c_m (acceleration) or NULL
+    float x_lo[NX], x_hi[NX];              // the state box X_k in scaled units (+-inf = free)
 };
 
 struct SplitScale { float sx[NX], isx[NX], su, isu; };
@@ -62,11 +64,11 @@ template <int m> __device__ __forceinline__ void spd_inverse_regs(float (&row)[m
     }
 }
 
-template <int NU>
+template <int NXT, int NU>
 __global__ void __launch_bounds__(SPLIT_WARPS * 32) k_split_factor(SolveParams P, SplitPtrs q)
 {
-    constexpr int n = NX + NU;
-    __shared__ float sT[SPLIT_WARPS][NX * n];
+    constexpr int n = NXT + NU;
+    __shared__ float sT[SPLIT_WARPS][NXT * n];
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     const long s = (long)blockIdx.x * SPLIT_WARPS + wib, st = (long)P.B * P.N;
     if (s >= st) return;
@@ -74,18 +76,18 @@ __global__ void __launch_bounds__(SPLIT_WARPS * 32) k_split_factor(SolveParams P
     float *T = sT[wib];
     // ---- G = (B^T B + I)^-1 : B_k staged in shared memory, lane i keeps column i
     {
-        const float *Bk = q.Bm + s * NX * NU;
-        for (int i = lane; i < NX * NU; i += 32) T[i] = Bk[i];
+        const float *Bk = q.Bm + s * NXT * NU;
+        for (int i = lane; i < NXT * NU; i += 32) T[i] = Bk[i];
         __syncwarp();
         const int lu = lane < NU ? lane : 0;
-        float col[NX], g[NU];
+        float col[NXT], g[NU];
 #pragma unroll
-        for (int a = 0; a < NX; a++) col[a] = lane < NU ? T[a * NU + lu] : 0.0f;
+        for (int a = 0; a < NXT; a++) col[a] = lane < NU ? T[a * NU + lu] : 0.0f;
 #pragma unroll
         for (int j = 0; j < NU; j++) {
             float acc = lane == j ? 1.0f : 0.0f;
 #pragma unroll
-            for (int a = 0; a < NX; a++) acc = fmaf(col[a], T[a * NU + j], acc);
+            for (int a = 0; a < NXT; a++) acc = fmaf(col[a], T[a * NU + j], acc);
             g[j] = acc;
         }
         spd_inverse_regs<NU>(g, lane);
@@ -97,39 +99,39 @@ __global__ void __launch_bounds__(SPLIT_WARPS * 32) k_split_factor(SolveParams P
     }
     // ---- Tt_k = [A_k B_k]^T for (21b)
     {
-        const float *Ak = q.A + s * NX * NX, *Bk = q.Bm + s * NX * NU;
-        for (int i = lane; i < NX * n; i += 32) {
+        const float *Ak = q.A + s * NXT * NXT, *Bk = q.Bm + s * NXT * NU;
+        for (int i = lane; i < NXT * n; i += 32) {
             const int a = i / n, j = i - a * n;
-            T[i] = j < NX ? Ak[a * NX + j] : Bk[a * NU + j - NX];
+            T[i] = j < NXT ? Ak[a * NXT + j] : Bk[a * NU + j - NXT];
         }
         __syncwarp();
-        for (int i = lane; i < NX * n; i += 32) {
-            const int c = i / NX, r = i - c * NX;
-            q.Tt[s * NX * n + i] = T[r * n + c];
+        for (int i = lane; i < NXT * n; i += 32) {
+            const int c = i / NXT, r = i - c * NXT;
+            q.Tt[s * NXT * n + i] = T[r * n + c];
         }
         __syncwarp();
     }
     // ---- H = (Qb + rho I [+ rho Ab_{k+1}^T Ab_{k+1}])^-1 ;  Ab^T Ab = T^T T + [[0, 0],[0, I]],  T = [A_{k+1} B_{k+1}] (13 x n)
     const bool nxt = k < P.N - 1;
     if (nxt) {
-        const float *A1 = q.A + (s + 1) * NX * NX, *B1 = q.Bm + (s + 1) * NX * NU;
-        for (int i = lane; i < NX * n; i += 32) {
+        const float *A1 = q.A + (s + 1) * NXT * NXT, *B1 = q.Bm + (s + 1) * NXT * NU;
+        for (int i = lane; i < NXT * n; i += 32) {
             const int a = i / n, j = i - a * n;
-            T[i] = j < NX ? A1[a * NX + j] : B1[a * NU + j - NX];
+            T[i] = j < NXT ? A1[a * NXT + j] : B1[a * NU + j - NXT];
         }
     }
     __syncwarp();
     const int ln = lane < n ? lane : 0;
-    const float qd = lane < NX ? P.Qd[lane] : (lane < n ? P.Rd[lane - NX] : 0.0f);
-    float h[n], col[NX];
+    const float qd = lane < NXT ? P.Qd[lane] : (lane < n ? P.Rd[lane - NXT] : 0.0f);
+    float h[n], col[NXT];
 #pragma unroll
-    for (int a = 0; a < NX; a++) col[a] = (nxt && lane < n) ? T[a * n + ln] : 0.0f;
+    for (int a = 0; a < NXT; a++) col[a] = (nxt && lane < n) ? T[a * n + ln] : 0.0f;
 #pragma unroll
     for (int j = 0; j < n; j++) {
-        float acc = (lane == j && lane >= NX && nxt) ? 1.0f : 0.0f;
+        float acc = (lane == j && lane >= NXT && nxt) ? 1.0f : 0.0f;
         if (nxt) {
 #pragma unroll
-            for (int a = 0; a < NX; a++) acc = fmaf(col[a], T[a * n + j], acc);
+            for (int a = 0; a < NXT; a++) acc = fmaf(col[a], T[a * n + j], acc);
         }
         h[j] = fmaf(P.rho, acc, lane == j ? qd + P.rho : 0.0f);
     }
@@ -141,26 +143,26 @@ __global__ void __launch_bounds__(SPLIT_WARPS * 32) k_split_factor(SolveParams P
 }
 
 // (21a)
-template <int NU>
+template <int NXT, int NU>
 __global__ void __launch_bounds__(SPLIT_WARPS * 32, 5) k_split_a(SolveParams P, SplitPtrs q)
 {
-    constexpr int n = NX + NU;
+    constexpr int n = NXT + NU;
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     const long s = (long)blockIdx.x * SPLIT_WARPS + wib, st = (long)P.B * P.N;
     if (s >= st) return;
     const int k = (int)(s % P.N);
-    const bool on = lane < n, isx = lane < NX;
-    const int ju = isx ? 0 : (on ? lane - NX : 0);
+    const bool on = lane < n, isx = lane < NXT;
+    const int ju = isx ? 0 : (on ? lane - NXT : 0);
     // The kernel is bound by memory latency, so the matrix elements a lane needs (column `lane` of B_k, G_k,
     // Ab_{k+1}, H_k) are requested in batches of independent loads before they are used.
     const bool nxt = k < P.N - 1;
     const long s1 = nxt ? s + 1 : s;
-    const float *Bk = q.Bm + s * NX * NU, *Gk = q.G + s * NU * NU, *Hk = q.H + s * n * n;
-    const float *A1 = q.A + s1 * NX * NX, *B1 = q.Bm + s1 * NX * NU;
+    const float *Bk = q.Bm + s * NXT * NU, *Gk = q.G + s * NU * NU, *Hk = q.H + s * n * n;
+    const float *A1 = q.A + s1 * NXT * NXT, *B1 = q.Bm + s1 * NXT * NU;
     const int lu = lane < NU ? lane : 0, ln = on ? lane : 0;
-    float bb[NX], gb[NU];
+    float bb[NXT], gb[NU];
 #pragma unroll
-    for (int a = 0; a < NX; a++) bb[a] = Bk[a * NU + lu];
+    for (int a = 0; a < NXT; a++) bb[a] = Bk[a * NU + lu];
 #pragma unroll
     for (int l = 0; l < NU; l++) gb[l] = Gk[l * NU + lu];
     const float vv = on ? q.v[s * n + lane] : 0.0f, bv = on ? q.be[s * n + lane] : 0.0f;
@@ -168,17 +170,17 @@ __global__ void __launch_bounds__(SPLIT_WARPS * 32, 5) k_split_a(SolveParams P, 
     float w = 0.0f;
     if (on && nxt) {
         w = q.z[s1 * n + lane] - q.v[s1 * n + lane] + q.la[s1 * n + lane];
-        if (isx && q.c) w -= q.c[s1 * NX + lane];
+        if (isx && q.c) w -= q.c[s1 * NXT + lane];
     }
-    const float ref = on ? (isx ? q.x_ref[s * NX + lane] : (q.u_ref ? q.u_ref[s * NU + ju] : 0.0f)) : 0.0f;
+    const float ref = on ? (isx ? q.x_ref[s * NXT + lane] : (q.u_ref ? q.u_ref[s * NU + ju] : 0.0f)) : 0.0f;
     // du = G (B^T r_x + r_u),  r = v - beta
     const float r = vv - bv;
-    float t = __shfl_sync(FULL, r, NX + lu);                               // r_u[lane] on lanes < NU
+    float t = __shfl_sync(FULL, r, NXT + lu);                               // r_u[lane] on lanes < NU
 #pragma unroll
-    for (int a = 0; a < NX; a++) t = fmaf(bb[a], __shfl_sync(FULL, r, a), t);
-    float ab[NX];
+    for (int a = 0; a < NXT; a++) t = fmaf(bb[a], __shfl_sync(FULL, r, a), t);
+    float ab[NXT];
 #pragma unroll
-    for (int a = 0; a < NX; a++) ab[a] = isx ? A1[a * NX + lane] : B1[a * NU + ju];
+    for (int a = 0; a < NXT; a++) ab[a] = isx ? A1[a * NXT + lane] : B1[a * NU + ju];
     float du = 0.0f;
 #pragma unroll
     for (int l = 0; l < NU; l++) du = fmaf(gb[l], __shfl_sync(FULL, t, l), du);
@@ -193,7 +195,7 @@ __global__ void __launch_bounds__(SPLIT_WARPS * 32, 5) k_split_a(SolveParams P, 
     if (nxt) {
         float acc = isx ? 0.0f : w;
 #pragma unroll
-        for (int a = 0; a < NX; a++) acc = fmaf(ab[a], __shfl_sync(FULL, w, a), acc);
+        for (int a = 0; a < NXT; a++) acc = fmaf(ab[a], __shfl_sync(FULL, w, a), acc);
         if (on) h = fmaf(P.rho, acc, h);
     }
     float hb[n - H1];
@@ -209,23 +211,23 @@ __global__ void __launch_bounds__(SPLIT_WARPS * 32, 5) k_split_a(SolveParams P, 
 }
 
 // (21b), (21c)
-template <int NU>
+template <int NXT, int NU>
 __global__ void __launch_bounds__(SPLIT_WARPS * 32) k_split_b(SolveParams P, SplitPtrs q, int last)
 {
-    constexpr int n = NX + NU, NC = 2 + (NU - 12) / 3;
+    constexpr int n = NXT + NU, NC = 2 + (NU - 12) / 3;
     __shared__ float su[SPLIT_WARPS][NU_MAX + 2];
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     const long s = (long)blockIdx.x * SPLIT_WARPS + wib, st = (long)P.B * P.N;
     if (s >= st) return;
     const long b = s / P.N;
     const int k = (int)(s - b * P.N);
-    const bool on = lane < n, isx = lane < NX;
-    const int ju = isx ? 0 : (on ? lane - NX : 0);
-    const float *Tt = q.Tt + s * NX * n + (isx ? lane : 0);      // column-major [A_k B_k]: Tt[a * 13 + row]
+    const bool on = lane < n, isx = lane < NXT;
+    const int ju = isx ? 0 : (on ? lane - NXT : 0);
+    const float *Tt = q.Tt + s * NXT * n + (isx ? lane : 0);      // column-major [A_k B_k]: Tt[a * 13 + row]
     // xi_k (the lifted state entering stage k): data for k = 0
     float xp = 0.0f;
     if (on) {
-        if (k == 0) xp = isx ? q.x0[b * NX + lane] : (q.u_prev ? q.u_prev[b * NU + ju] : 0.0f);
+        if (k == 0) xp = isx ? q.x0[b * NXT + lane] : (q.u_prev ? q.u_prev[b * NU + ju] : 0.0f);
         else xp = q.xi[(s - 1) * n + lane];
     }
     const float du = (on && !isx) ? q.du[s * NU + ju] : 0.0f;
@@ -234,17 +236,17 @@ __global__ void __launch_bounds__(SPLIT_WARPS * 32) k_split_b(SolveParams P, Spl
 #pragma unroll
     for (int a = 0; a < n; a++) {
         const float xa = __shfl_sync(FULL, xp, a);
-        if (isx) Axi = fmaf(Tt[a * NX], xa, Axi);
+        if (isx) Axi = fmaf(Tt[a * NXT], xa, Axi);
     }
 #pragma unroll
     for (int j = 0; j < NU; j++) {
-        const float dj = __shfl_sync(FULL, du, NX + j);
-        if (isx) Bdu = fmaf(Tt[(NX + j) * NX], dj, Bdu);
+        const float dj = __shfl_sync(FULL, du, NXT + j);
+        if (isx) Bdu = fmaf(Tt[(NXT + j) * NXT], dj, Bdu);
     }
     float xi = 0.0f, th = 0.0f, be = 0.0f, la = 0.0f, e = 0.0f;
     if (on) {
         xi = q.xi[s * n + lane]; th = q.th[s * n + lane]; be = q.be[s * n + lane]; la = q.la[s * n + lane];
-        if (isx && q.c) e = q.c[s * NX + lane];
+        if (isx && q.c) e = q.c[s * NXT + lane];
     }
     const float gamma = Bdu + be - Axi - e + la;
     const float gammat = xi + th + Axi + e - la;
@@ -267,7 +269,7 @@ __global__ void __launch_bounds__(SPLIT_WARPS * 32) k_split_b(SolveParams P, Spl
         }
     }
     __syncwarp();
-    const float z = isx ? w : (on ? uw[ju] : 0.0f);
+    const float z = isx ? fminf(fmaxf(w, q.x_lo[isx ? lane : 0]), q.x_hi[isx ? lane : 0]) : (on ? uw[ju] : 0.0f);      // X_k: a box (+-inf = free)
     const float v = 0.5f * (z + gamma);
     if (q.cpart) {
         // c_m share of this stage: rho (|d theta|^2 + |d beta|^2 + |d lambda|^2 + |dz|^2 + |dv|^2 + |dz - dv|^2) against w^
@@ -295,25 +297,25 @@ __global__ void __launch_bounds__(SPLIT_WARPS * 32) k_split_b(SolveParams P, Spl
 }
 
 // x = Sx x~, u = su u~: the scaled problem, written once.  One thread per element of the largest array (A or B).
-__global__ void k_split_scale(int B, int N, int nu, SplitScale S, const float *A, const float *Bm, const float *c, const float *x0,
+__global__ void k_split_scale(int B, int N, int nx, int nu, SplitScale S, const float *A, const float *Bm, const float *c, const float *x0,
                               const float *u_prev, const float *x_ref, const float *u_ref, float *sA, float *sB, float *sc, float *sx0,
                               float *sup, float *sxr, float *sur)
 {
     const long st = (long)B * N, i = (long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < st * NX * NX) { const int r = (int)((i / NX) % NX), col = (int)(i % NX); sA[i] = A[i] * S.isx[r] * S.sx[col]; }
-    if (i < st * NX * nu) { const int r = (int)((i / nu) % NX); sB[i] = Bm[i] * S.isx[r] * S.su; }
-    if (i < st * NX) { const int r = (int)(i % NX); if (c) sc[i] = c[i] * S.isx[r]; sxr[i] = x_ref[i] * S.isx[r]; }
+    if (i < st * nx * nx) { const int r = (int)((i / nx) % nx), col = (int)(i % nx); sA[i] = A[i] * S.isx[r] * S.sx[col]; }
+    if (i < st * nx * nu) { const int r = (int)((i / nu) % nx); sB[i] = Bm[i] * S.isx[r] * S.su; }
+    if (i < st * nx) { const int r = (int)(i % nx); if (c) sc[i] = c[i] * S.isx[r]; sxr[i] = x_ref[i] * S.isx[r]; }
     if (i < st * nu && u_ref) sur[i] = u_ref[i] * S.isu;
-    if (i < (long)B * NX) sx0[i] = x0[i] * S.isx[(int)(i % NX)];
+    if (i < (long)B * nx) sx0[i] = x0[i] * S.isx[(int)(i % nx)];
     if (i < (long)B * nu && u_prev) sup[i] = u_prev[i] * S.isu;
 }
 
-__global__ void k_split_unscale(long st, int n, SplitScale S, const float *in, float *out)
+__global__ void k_split_unscale(long st, int nx, int n, SplitScale S, const float *in, float *out)
 {
     const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= st * n) return;
     const int j = (int)(i % n);
-    out[i] = in[i] * (j < NX ? S.sx[j] : S.su);
+    out[i] = in[i] * (j < nx ? S.sx[j] : S.su);
 }
 
 // Accept / restart decision of iteration m for every env (oracle/split.py header).  acc[b] = (alpha, c_prev, mom, restart).
@@ -364,32 +366,34 @@ __global__ void k_split_residual(const float *rs, float *r_prim, int B, int N)
     r_prim[b] = m;
 }
 
-size_t split_floats(int nu, long st)
+size_t split_floats(int nx, int nu, long st)
 {
-    const long n = NX + nu;
-    return (size_t)st * (n * n + nu * nu + NX * n + 7 * n + nu + 1);
+    const long n = nx + nu;
+    return (size_t)st * (n * n + nu * nu + nx * n + 7 * n + nu + 1);
 }
 
 bool opt_scaled(const pinmpc_split_options *o) { return o && (o->h_scale_x != nullptr || (o->scale_u != 0.0f && o->scale_u != 1.0f)); }
 bool opt_accel(const pinmpc_split_options *o) { return o && o->accel != 0; }
 
+int opt_nx(const pinmpc_split_options *o) { return (o && o->nx != 0) ? o->nx : NX; }
+
 size_t split_floats_ex(int nu, long st, long B, const pinmpc_split_options *o)
 {
-    const long n = NX + nu;
-    size_t f = split_floats(nu, st);
-    if (opt_scaled(o)) f += (size_t)st * (NX * NX + NX * nu + 2 * NX + nu) + (size_t)B * n;
+    const long nx = opt_nx(o), n = nx + nu;
+    size_t f = split_floats((int)nx, nu, st);
+    if (opt_scaled(o)) f += (size_t)st * (nx * nx + nx * nu + 2 * nx + nu) + (size_t)B * n;
     if (opt_accel(o)) f += (size_t)st * (10 * n + 1) + (size_t)B * 4 + 4;
     return f;
 }
 
-template <int NU>
+template <int NXT, int NU>
 pinmpc_status run(const SolveParams &P, SplitPtrs q, int iters, float *r_prim, bool accel, float eta, float *w1, float *hat, float4 *acc,
                   int *restarts, cudaStream_t stream)
 {
-    constexpr int n = NX + NU;
+    constexpr int n = NXT + NU;
     const long st = (long)P.B * P.N;
     const unsigned blocks = (unsigned)((st + SPLIT_WARPS - 1) / SPLIT_WARPS);
-    k_split_factor<NU><<<blocks, SPLIT_WARPS * 32, 0, stream>>>(P, q);
+    k_split_factor<NXT, NU><<<blocks, SPLIT_WARPS * 32, 0, stream>>>(P, q);
     float *w0 = q.nz;                                        // ring buffer 0 = the plain iteration's z, v, theta, beta, lambda
     if (accel) {
         k_split_accel_init<<<(P.B + 127) / 128, 128, 0, stream>>>(P.B, acc, restarts);
@@ -400,8 +404,8 @@ pinmpc_status run(const SolveParams &P, SplitPtrs q, int iters, float *r_prim, b
             float *wm = (it & 1) ? w1 : w0;
             q.nz = wm; q.nv = wm + st * n; q.nth = wm + 2 * st * n; q.nbe = wm + 3 * st * n; q.nla = wm + 4 * st * n;
         }
-        k_split_a<NU><<<blocks, SPLIT_WARPS * 32, 0, stream>>>(P, q);
-        k_split_b<NU><<<blocks, SPLIT_WARPS * 32, 0, stream>>>(P, q, it == iters - 1 && r_prim != nullptr);
+        k_split_a<NXT, NU><<<blocks, SPLIT_WARPS * 32, 0, stream>>>(P, q);
+        k_split_b<NXT, NU><<<blocks, SPLIT_WARPS * 32, 0, stream>>>(P, q, it == iters - 1 && r_prim != nullptr);
         if (accel && it < iters - 1) {
             k_split_decide<<<(P.B + 127) / 128, 128, 0, stream>>>(P.B, P.N, eta, q.cpart, acc, restarts);
             const long tot = 5 * st * n;
@@ -417,6 +421,7 @@ pinmpc_status run(const SolveParams &P, SplitPtrs q, int iters, float *r_prim, b
 extern "C" size_t pinmpc_split_workspace_bytes_ex(int nu, int N, int B, const pinmpc_split_options *opts)
 {
     if ((nu != 12 && nu != 18) || N < 1 || N > PINMPC_SPLIT_N_MAX || B < 0) return 0;
+    if (opt_nx(opts) != NX && opt_nx(opts) != 9) return 0;
     return split_floats_ex(nu, (long)B * N, B, opts) * sizeof(float) + 256;
 }
 
@@ -429,10 +434,12 @@ extern "C" pinmpc_status pinmpc_split_solve_ex(int nu, int N, int B, const pinmp
     if ((nu != 12 && nu != 18) || N < 1 || N > PINMPC_SPLIT_N_MAX) return PINMPC_EUNSUPPORTED;
     if (!layout || layout->n_wrench != 2 || 6 * layout->n_wrench + 3 * layout->n_force != nu) return PINMPC_EUNSUPPORTED;
     if (B < 0 || !(rho > 0.0f) || iters < 1 || !h_Qdiag || !h_Rdiag || !p) return PINMPC_EINVAL;
+    const int nx = opt_nx(opts);
+    if (nx != NX && nx != 9) return PINMPC_EUNSUPPORTED;
     const bool scaled = opt_scaled(opts), accel = opt_accel(opts);
     SplitScale S;
     for (int i = 0; i < NX; i++) {
-        const float v = (opts && opts->h_scale_x) ? opts->h_scale_x[i] : 1.0f;
+        const float v = (opts && opts->h_scale_x && i < nx) ? opts->h_scale_x[i] : 1.0f;
         if (!(v > 0.0f) || !std::isfinite(v)) return PINMPC_EINVAL;
         S.sx[i] = v; S.isx[i] = 1.0f / v;
     }
@@ -450,16 +457,16 @@ extern "C" pinmpc_status pinmpc_split_solve_ex(int nu, int N, int B, const pinmp
     P.B = B; P.N = N; P.nu = nu; P.nw = layout->n_wrench; P.nf = layout->n_force; P.iters = iters; P.rho = rho;
     P.mu = layout->mu; P.fz_max = layout->fz_max * S.isu; P.cx = layout->mx_coef; P.cy = layout->my_coef; P.cz = layout->mz_coef;
     P.hand_fmax = layout->hand_fmax * S.isu;
-    for (int i = 0; i < NX; i++) { if (!(h_Qdiag[i] >= 0.0f)) return PINMPC_EINVAL; P.Qd[i] = h_Qdiag[i] * S.sx[i] * S.sx[i]; }
+    for (int i = 0; i < nx; i++) { if (!(h_Qdiag[i] >= 0.0f)) return PINMPC_EINVAL; P.Qd[i] = h_Qdiag[i] * S.sx[i] * S.sx[i]; }
     for (int i = 0; i < nu; i++) { if (!(h_Rdiag[i] >= 0.0f)) return PINMPC_EINVAL; P.Rd[i] = h_Rdiag[i] * S.su * S.su; }
     P.iw[0] = P.iw[1] = 1.0f / P.mu; P.iw[2] = 1.0f / P.cx; P.iw[3] = 1.0f / P.cy; P.iw[4] = 1.0f / P.cz;
-    const long stg = (long)B * N, n = NX + nu;
+    const long stg = (long)B * N, n = nx + nu;
     float *w = reinterpret_cast<float *>(((uintptr_t)d_ws + 255) & ~(uintptr_t)255);
     SplitPtrs q;
     q.A = p->A; q.Bm = p->Bm; q.c = p->c; q.x0 = p->x0; q.u_prev = p->u_prev; q.x_ref = p->x_ref; q.u_ref = p->u_ref; q.contact = p->contact;
     q.H = w; w += stg * n * n;
     q.G = w; w += stg * nu * nu;
-    q.Tt = w; w += stg * NX * n;
+    q.Tt = w; w += stg * nx * n;
     q.xi = w; w += stg * n;
     float *w0 = w; w += 5 * stg * n;
     q.nz = w0; q.nv = w0 + stg * n; q.nth = w0 + 2 * stg * n; q.nbe = w0 + 3 * stg * n; q.nla = w0 + 4 * stg * n;
@@ -467,16 +474,21 @@ extern "C" pinmpc_status pinmpc_split_solve_ex(int nu, int N, int B, const pinmp
     q.du = w; w += stg * nu;
     q.rs = w; w += stg;
     q.cpart = nullptr;
+    for (int i = 0; i < NX; i++) {
+        const float lo = (opts && opts->h_x_lo && i < nx) ? opts->h_x_lo[i] : -INFINITY, hi = (opts && opts->h_x_hi && i < nx) ? opts->h_x_hi[i] : INFINITY;
+        if (!(lo <= hi)) return PINMPC_EINVAL;
+        q.x_lo[i] = lo * S.isx[i]; q.x_hi[i] = hi * S.isx[i];
+    }
     if (scaled) {
-        float *sA = w; w += stg * NX * NX;
-        float *sB = w; w += stg * NX * nu;
-        float *sc = w; w += stg * NX;
-        float *sxr = w; w += stg * NX;
+        float *sA = w; w += stg * nx * nx;
+        float *sB = w; w += stg * nx * nu;
+        float *sc = w; w += stg * nx;
+        float *sxr = w; w += stg * nx;
         float *sur = w; w += stg * nu;
-        float *sx0 = w; w += (long)B * NX;
+        float *sx0 = w; w += (long)B * nx;
         float *sup = w; w += (long)B * nu;
-        const long tot = stg * NX * (nu > NX ? nu : NX);
-        k_split_scale<<<(unsigned)((tot + 255) / 256), 256, 0, st_>>>(B, N, nu, S, p->A, p->Bm, p->c, p->x0, p->u_prev, p->x_ref, p->u_ref, sA, sB, sc,
+        const long tot = stg * nx * (nu > nx ? nu : nx);
+        k_split_scale<<<(unsigned)((tot + 255) / 256), 256, 0, st_>>>(B, N, nx, nu, S, p->A, p->Bm, p->c, p->x0, p->u_prev, p->x_ref, p->u_ref, sA, sB, sc,
                                                                      sx0, sup, sxr, sur);
         q.A = sA; q.Bm = sB; q.c = p->c ? sc : nullptr; q.x0 = sx0; q.u_prev = p->u_prev ? sup : nullptr; q.x_ref = sxr;
         q.u_ref = p->u_ref ? sur : nullptr;
@@ -494,15 +506,18 @@ extern "C" pinmpc_status pinmpc_split_solve_ex(int nu, int N, int B, const pinmp
     // all iterates start at 0 (z, v, theta, beta, lambda are contiguous)
     if (cudaMemsetAsync(w0, 0, (size_t)stg * n * 5 * sizeof(float), st_) != cudaSuccess) return PINMPC_ECUDA;
     int *restarts = (accel && opts) ? opts->d_restarts : nullptr;
-    pinmpc_status rc = nu == 12 ? run<12>(P, q, iters, r_prim, accel, eta, w1, hat, acc, restarts, st_)
-                                : run<18>(P, q, iters, r_prim, accel, eta, w1, hat, acc, restarts, st_);
+    pinmpc_status rc;
+    if (nx == NX) rc = nu == 12 ? run<NX, 12>(P, q, iters, r_prim, accel, eta, w1, hat, acc, restarts, st_)
+                                : run<NX, 18>(P, q, iters, r_prim, accel, eta, w1, hat, acc, restarts, st_);
+    else rc = nu == 12 ? run<9, 12>(P, q, iters, r_prim, accel, eta, w1, hat, acc, restarts, st_)
+                       : run<9, 18>(P, q, iters, r_prim, accel, eta, w1, hat, acc, restarts, st_);
     if (rc != PINMPC_OK) return rc;
     const float *zlast = (accel && ((iters - 1) & 1)) ? w1 : w0;
     const size_t bytes = (size_t)stg * n * sizeof(float);
     if (scaled) {
         const long tot = stg * n;
-        if (xi) k_split_unscale<<<(unsigned)((tot + 255) / 256), 256, 0, st_>>>(stg, (int)n, S, q.xi, xi);
-        if (z) k_split_unscale<<<(unsigned)((tot + 255) / 256), 256, 0, st_>>>(stg, (int)n, S, zlast, z);
+        if (xi) k_split_unscale<<<(unsigned)((tot + 255) / 256), 256, 0, st_>>>(stg, nx, (int)n, S, q.xi, xi);
+        if (z) k_split_unscale<<<(unsigned)((tot + 255) / 256), 256, 0, st_>>>(stg, nx, (int)n, S, zlast, z);
         return cudaGetLastError() == cudaSuccess ? PINMPC_OK : PINMPC_ECUDA;
     }
     if (xi && cudaMemcpyAsync(xi, q.xi, bytes, cudaMemcpyDeviceToDevice, st_) != cudaSuccess) return PINMPC_ECUDA;

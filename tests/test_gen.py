@@ -57,3 +57,13 @@ def test_loco_manipulation_extras_and_subset():
 
 def test_different_configs_use_different_seeds():
     assert not np.array_equal(gen.make_config(1, B=8, N=10).mass, gen.make_config(2, B=8, N=10).mass)
+
+
+def test_centroidal_view_is_the_same_episode_in_nine_states():
+    w = gen.make_config(3, B=5, N=8)
+    v = gen.centroidal_view(w)
+    assert v["x0"].shape == (5, 9) and v["x_ref"].shape == (5, 8, 9) and v["Qdiag"].shape == (9,)
+    assert np.allclose(v["x0"][:, 0:3], w.x0[:, 3:6])
+    assert np.allclose(v["x_ref"][..., 3:6], w.mass[:, None, None] * w.x_ref[..., 9:12], rtol=1e-6)
+    assert np.all(v["Qdiag"] > 0) and np.all(v["x_lo"] <= v["x_hi"])
+    assert np.isinf(v["x_lo"]).sum() == 7 and np.isinf(v["x_hi"]).sum() == 7
