@@ -189,6 +189,14 @@ __device__ __forceinline__ float4 lds_f4(uint32_t a)
     return v;
 }
 
+// Packed FP32 pair FMA (sm_100 fma.rn.f32x2): (d0, d1) += (a0, a1) * (b0, b1).  One issue slot for two FMAs; the pairs
+// must sit in aligned register pairs, which the callers arrange (consecutive tcgen05.ld destinations, paired states).
+__device__ __forceinline__ void ffma2(float &d0, float &d1, float a0, float a1, float b0, float b1)
+{
+    asm("{ .reg .b64 a, b, c;\n\t mov.b64 a, {%2, %3};\n\t mov.b64 b, {%4, %5};\n\t mov.b64 c, {%0, %1};\n\t fma.rn.f32x2 c, a, b, c;\n\t mov.b64 {%0, %1}, c; }"
+        : "+f"(d0), "+f"(d1) : "f"(a0), "f"(a1), "f"(b0), "f"(b1));
+}
+
 // all 72 gains of stage j of the chunk, row-major Kn[r][0..11]
 __device__ __forceinline__ void chain_ld_stage(uint32_t tk, int j, float *k)
 {
@@ -219,7 +227,9 @@ __device__ __forceinline__ void chain_bwd_sweep(const Chain &ch, float dt, const
         const bool act = j < ch.len;
         const float dte = act ? dt : 0.0f;
         const float2 cs = lds_f2(ch.sCS + chain_joff(ch, j));
+#ifndef TM_NOWAIT
         tm_wait_ld();
+#endif
         float hh[6];
 #pragma unroll
         for (int r = 0; r < 6; r++) hh[r] = s0[r] + v[r];
@@ -246,9 +256,9 @@ __device__ __forceinline__ void chain_bwd_sweep(const Chain &ch, float dt, const
 #pragma unroll
         for (int r = 0; r < 6; r++)
 #pragma unroll
-            for (int i = 0; i < 6; i++) {
-                q[i] = fmaf(k[12 * r + i], hh[r], q[i]);
-                v[i] = fmaf(k[12 * r + 6 + i], hh[r], v[i]);
+            for (int i = 0; i < 6; i += 2) {
+                ffma2(q[i], q[i + 1], k[12 * r + i], k[12 * r + i + 1], hh[r], hh[r]);
+                ffma2(v[i], v[i + 1], k[12 * r + 6 + i], k[12 * r + 7 + i], hh[r], hh[r]);
             }
     }
     if (OUT) tm_wait_st();
@@ -301,13 +311,19 @@ __device__ __forceinline__ void chain_fwd_sweep(const Chain &ch, float dt, float
         const bool act = j < ch.len;
         const float dte = act ? dt : 0.0f, gdte = act ? gdt : 0.0f;
         const float2 cs = lds_f2(ch.sCS + chain_joff(ch, j));
+#ifndef TM_NOWAIT
         tm_wait_ld();
+#endif
 #pragma unroll
         for (int r = 0; r < 6; r++) {
-            float a = w[r], b = 0.0f;
+            // row r of Kn times (xa ; xb): pairs of products accumulate in two packed sums (even, odd columns)
+            float a0 = w[r], a1 = 0.0f, b0 = 0.0f, b1 = 0.0f;
 #pragma unroll
-            for (int i = 0; i < 6; i++) { a = fmaf(k[12 * r + i], xa[i], a); b = fmaf(k[12 * r + 6 + i], xb[i], b); }
-            w[r] = a + b;
+            for (int i = 0; i < 6; i += 2) {
+                ffma2(a0, a1, k[12 * r + i], k[12 * r + i + 1], xa[i], xa[i + 1]);
+                ffma2(b0, b1, k[12 * r + 6 + i], k[12 * r + 7 + i], xb[i], xb[i + 1]);
+            }
+            w[r] = (a0 + a1) + (b0 + b1);
         }
         if (OUT) tm_st6(ch.tk + TM_XOFF + 6 * j, w);
         // x_a+ = x_a + dt Rot x_b (old x_b);  x_b+ = x_b + w + c
