@@ -294,7 +294,7 @@ __device__ __forceinline__ void chain_kappa(const Chain &ch)
 // Forward sweep over the chunk, stages 0 .. nsteps-1:  w = kappa + Kn x ;  x+ = A x + E (w + c).
 // OUT: w replaces kappa in the exchange vector; ox != nullptr (with OUT): x+ -> ox (x_{k+1} of the output).
 // init: the start state (12 floats in shared memory; nullptr = 0); fin: where the end state goes (nullptr = nowhere).
-template <bool OUT>
+template <bool OUT, bool OX = false>
 __device__ __forceinline__ void chain_fwd_sweep(const Chain &ch, float dt, float gdt, float x12, int has_ext, const float *init, float *fin, float *ox)
 {
     float xa[6], xb[6];
@@ -316,14 +316,14 @@ __device__ __forceinline__ void chain_fwd_sweep(const Chain &ch, float dt, float
 #endif
 #pragma unroll
         for (int r = 0; r < 6; r++) {
-            // row r of Kn times (xa ; xb): pairs of products accumulate in two packed sums (even, odd columns)
-            float a0 = w[r], a1 = 0.0f, b0 = 0.0f, b1 = 0.0f;
+            // row r of Kn times (xa ; xb): the products accumulate in one packed sum (even, odd columns); the six rows
+            // are independent chains
+            float a0 = w[r], a1 = 0.0f;
 #pragma unroll
-            for (int i = 0; i < 6; i += 2) {
-                ffma2(a0, a1, k[12 * r + i], k[12 * r + i + 1], xa[i], xa[i + 1]);
-                ffma2(b0, b1, k[12 * r + 6 + i], k[12 * r + 7 + i], xb[i], xb[i + 1]);
-            }
-            w[r] = (a0 + a1) + (b0 + b1);
+            for (int i = 0; i < 6; i += 2) ffma2(a0, a1, k[12 * r + i], k[12 * r + i + 1], xa[i], xa[i + 1]);
+#pragma unroll
+            for (int i = 0; i < 6; i += 2) ffma2(a0, a1, k[12 * r + 6 + i], k[12 * r + 7 + i], xb[i], xb[i + 1]);
+            w[r] = a0 + a1;
         }
         if (OUT) tm_st6(ch.tk + TM_XOFF + 6 * j, w);
         // x_a+ = x_a + dt Rot x_b (old x_b);  x_b+ = x_b + w + c
@@ -336,7 +336,7 @@ __device__ __forceinline__ void chain_fwd_sweep(const Chain &ch, float dt, float
 #pragma unroll
         for (int i = 0; i < 6; i++) xb[i] += w[i] + cv[i];
         xb[5] += gdte;
-        if (ox != nullptr && act) {
+        if (OX && ox != nullptr && act) {
             float *o = ox + j * NX;
 #pragma unroll
             for (int i = 0; i < 6; i++) { o[i] = xa[i]; o[6 + i] = xb[i]; }
@@ -554,15 +554,20 @@ struct ChainArgs {
 template <int RBW>
 __device__ __noinline__ void tm_chain_main(ChainArgs A)
 {
-    const Chain ch = A.ch;
+    Chain ch = A.ch;
+    // Warp-uniform by construction; the broadcast from lane 0 tells the compiler, which then keeps the tensor-memory
+    // addresses and the loop counters of the sweeps in uniform registers (no R2UR per tcgen05.ld: 6-13 per step before).
+    ch.tk = __shfl_sync(FULL, ch.tk, 0);
+    ch.nsteps = __shfl_sync(FULL, ch.nsteps, 0);
     const float dt = A.dt, gdt = A.gdt, x12 = A.x12;
-    const int has_ext = A.has_ext, C = A.C, cc = A.cc;
+    const int has_ext = __shfl_sync(FULL, A.has_ext, 0), C = __shfl_sync(FULL, A.C, 0), cc = A.cc;
+    A.iters = __shfl_sync(FULL, A.iters, 0); A.tol_mode = __shfl_sync(FULL, A.tol_mode, 0); A.check_every = __shfl_sync(FULL, A.check_every, 0);
     const bool cvalid = A.cvalid != 0;
     float *slot_lo = A.slot_lo, *slot_hi = A.slot_lo + 12, *oxe = A.oxe;
     int *ndone = A.ndone;
     for (int it = 0; it < A.iters; it++) {
         const bool is_check = A.tol_mode && ((it + 1) % A.check_every == 0);
-        const bool emit = (it == A.iters - 1) || is_check;
+        const bool emit = __shfl_sync(FULL, (int)((it == A.iters - 1) || is_check), 0) != 0;   // (the modulo hides its uniformity)
         tm_sync();                                          // (1) sigma0 of every stage is in the exchange vectors
         TM_TICK(0)
         // ---- backward sweep A: zero terminal costate -> b_c (the last chunk: its true costate)
@@ -582,7 +587,10 @@ __device__ __noinline__ void tm_chain_main(ChainArgs A)
         __syncthreads();                                    // (5) true start states in the slots
         TM_TICK(5)
         // ---- forward sweep B: true start state; w -> exchange, x -> output
-        if (TM_ABL != 4) chain_fwd_sweep<true>(ch, dt, gdt, x12, has_ext, slot_lo, nullptr, (emit && cvalid && !*A.done_e) ? oxe : nullptr);
+        if (TM_ABL != 4) {
+            if (emit) chain_fwd_sweep<true, true>(ch, dt, gdt, x12, has_ext, slot_lo, nullptr, (cvalid && !*A.done_e) ? oxe : nullptr);
+            else chain_fwd_sweep<true, false>(ch, dt, gdt, x12, has_ext, slot_lo, nullptr, nullptr);     // no state output code in the common step
+        }
         TM_TICK(6)
         tm_sync();                                          // (6) w of every stage is in the exchange vectors
         if (emit) {
