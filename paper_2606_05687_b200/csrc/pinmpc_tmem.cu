@@ -704,7 +704,8 @@ __global__ void __launch_bounds__(tm_threads(NU), 1) k_iterate_tm(SolveParams P,
     constexpr int NC = NW + (NU - 12) / 3, RBW = tm_rbw(NU), GRBW = pinmpc_rb_width(NU), TM_THREADS = tm_threads(NU);
     extern __shared__ __align__(16) float smem[];
     __shared__ uint32_t tmem_slot;
-    const int N = P.N, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int N = P.N, tid = threadIdx.x, lane = tid & 31;
+    const int warp = tid >> 5;
     const long st = (long)P.B * N;
     const TmLay L = tm_layout(N, G, C, NU);
     const int b0 = blockIdx.x * G;
@@ -807,7 +808,8 @@ __global__ void __launch_bounds__(tm_threads(NU), 1) k_iterate_tm(SolveParams P,
         bool frozen = false;
 
         for (int it = 0; it < P.iters; it++) {
-            const bool is_check = tol_mode && ((it + 1) % P.check_every == 0);
+            // (uniform by construction; the modulo hides it from the compiler, the broadcast restores it)
+            const bool is_check = __shfl_sync(FULL, (int)(tol_mode && ((it + 1) % P.check_every == 0)), 0) != 0;
             const bool emit = (it == P.iters - 1) || is_check;
             if (emit)
                 for (int i = tid - 128; i < 5 * TM_GMAX; i += TM_THREADS - 128) red[i] = 0u;
