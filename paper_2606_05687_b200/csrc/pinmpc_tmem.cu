@@ -691,10 +691,10 @@ __device__ __noinline__ void tm_cta_load(SrbWs W, const float *__restrict__ Psi,
 }
 
 // ---------------------------------------------------------------------------------------------
-// S3-S6: all ADMM iterations of G envs per CTA.  12 warps: warps 0-3 are the CHAIN warps (lane t of warp q =
-// chain 32 q + t = TMEM lane), warps 4-7 and 8-11 the WORKER warps: worker (slot s = 0, 1; quarter q; lane t)
-// shares the TMEM lane of chain 32 q + t and owns stages 3 s .. 3 s + 2 of its chunk (z, y in registers).
-// 168 registers per thread: the chain threads hold two half-stage operand buffers, the workers three stages.
+// S3-S6: all ADMM iterations of G envs per CTA.  Warps 0-3 are the CHAIN warps (lane t of warp q = chain 32 q + t =
+// TMEM lane), the others the WORKER warps: worker (slot s, quarter q, lane t) shares the TMEM lane of chain 32 q + t and
+// owns stages WS s .. WS s + WS - 1 of its chunk with z, y in registers (nu = 12: three workers per chain, two stages
+// each, 512 threads at 128 registers; nu = 18: two workers per chain, two stages each, 384 threads at 168 registers).
 // ---------------------------------------------------------------------------------------------
 template <int NU, bool WARM>
 __global__ void __launch_bounds__(tm_threads(NU), 1) k_iterate_tm(SolveParams P, SrbWs W, const float *__restrict__ Psi, const float *__restrict__ x0g,
