@@ -318,12 +318,12 @@ __device__ __forceinline__ void chain_fwd_sweep(const Chain &ch, float dt, float
         for (int r = 0; r < 6; r++) {
             // row r of Kn times (xa ; xb): the products accumulate in one packed sum (even, odd columns); the six rows
             // are independent chains
-            float a0 = w[r], a1 = 0.0f;
+            float a0 = 0.0f, a1 = 0.0f;
 #pragma unroll
             for (int i = 0; i < 6; i += 2) ffma2(a0, a1, k[12 * r + i], k[12 * r + i + 1], xa[i], xa[i + 1]);
 #pragma unroll
             for (int i = 0; i < 6; i += 2) ffma2(a0, a1, k[12 * r + 6 + i], k[12 * r + 7 + i], xb[i], xb[i + 1]);
-            w[r] = a0 + a1;
+            w[r] += a0 + a1;
         }
         if (OUT) tm_st6(ch.tk + TM_XOFF + 6 * j, w);
         // x_a+ = x_a + dt Rot x_b (old x_b);  x_b+ = x_b + w + c
@@ -334,7 +334,11 @@ __device__ __forceinline__ void chain_fwd_sweep(const Chain &ch, float dt, float
             for (int i = 2; i < 6; i++) xa[i] = fmaf(dte, xb[i], xa[i]);
         }
 #pragma unroll
-        for (int i = 0; i < 6; i++) xb[i] += w[i] + cv[i];
+        for (int i = 0; i < 6; i++) xb[i] += w[i];
+        if (has_ext) {                                      // (uniform)
+#pragma unroll
+            for (int i = 0; i < 6; i++) xb[i] += cv[i];
+        }
         xb[5] += gdte;
         if (OX && ox != nullptr && act) {
             float *o = ox + j * NX;
