@@ -197,6 +197,12 @@ __device__ __forceinline__ void ffma2(float &d0, float &d1, float a0, float a1, 
         : "+f"(d0), "+f"(d1) : "f"(a0), "f"(a1), "f"(b0), "f"(b1));
 }
 
+__device__ __forceinline__ void fadd2(float &d0, float &d1, float a0, float a1, float b0, float b1)      // (d0, d1) = (a0, a1) + (b0, b1)
+{
+    asm("{ .reg .b64 a, b, c;\n\t mov.b64 a, {%2, %3};\n\t mov.b64 b, {%4, %5};\n\t add.rn.f32x2 c, a, b;\n\t mov.b64 {%0, %1}, c; }"
+        : "=f"(d0), "=f"(d1) : "f"(a0), "f"(a1), "f"(b0), "f"(b1));
+}
+
 // all 72 gains of stage j of the chunk, row-major Kn[r][0..11]
 __device__ __forceinline__ void chain_ld_stage(uint32_t tk, int j, float *k)
 {
@@ -232,7 +238,7 @@ __device__ __forceinline__ void chain_bwd_sweep(const Chain &ch, float dt, const
 #endif
         float hh[6];
 #pragma unroll
-        for (int r = 0; r < 6; r++) hh[r] = s0[r] + v[r];
+        for (int r = 0; r < 6; r += 2) fadd2(hh[r], hh[r + 1], s0[r], s0[r + 1], v[r], v[r + 1]);
         if (OUT) {
             float Mi[28], kp[6];
             const uint32_t a = ch.sA + chain_joff(ch, j);
@@ -249,9 +255,9 @@ __device__ __forceinline__ void chain_bwd_sweep(const Chain &ch, float dt, const
         // (A^T p)_v = pv + dt Rot^T pq  (old pq)
         {
             const float t0 = cs.x * q[0] - cs.y * q[1], t1 = cs.x * q[1] + cs.y * q[0];
-            v[0] = fmaf(dte, t0, v[0]); v[1] = fmaf(dte, t1, v[1]);
+            ffma2(v[0], v[1], t0, t1, dte, dte);
 #pragma unroll
-            for (int i = 2; i < 6; i++) v[i] = fmaf(dte, q[i], v[i]);
+            for (int i = 2; i < 6; i += 2) ffma2(v[i], v[i + 1], q[i], q[i + 1], dte, dte);
         }
 #pragma unroll
         for (int r = 0; r < 6; r++)
@@ -329,15 +335,15 @@ __device__ __forceinline__ void chain_fwd_sweep(const Chain &ch, float dt, float
         // x_a+ = x_a + dt Rot x_b (old x_b);  x_b+ = x_b + w + c
         {
             const float t0 = fmaf(cs.x, xb[0], cs.y * xb[1]), t1 = fmaf(cs.x, xb[1], -cs.y * xb[0]);
-            xa[0] = fmaf(dte, t0, xa[0]); xa[1] = fmaf(dte, t1, xa[1]);
+            ffma2(xa[0], xa[1], t0, t1, dte, dte);
 #pragma unroll
-            for (int i = 2; i < 6; i++) xa[i] = fmaf(dte, xb[i], xa[i]);
+            for (int i = 2; i < 6; i += 2) ffma2(xa[i], xa[i + 1], xb[i], xb[i + 1], dte, dte);
         }
 #pragma unroll
-        for (int i = 0; i < 6; i++) xb[i] += w[i];
+        for (int i = 0; i < 6; i += 2) fadd2(xb[i], xb[i + 1], xb[i], xb[i + 1], w[i], w[i + 1]);
         if (has_ext) {                                      // (uniform)
 #pragma unroll
-            for (int i = 0; i < 6; i++) xb[i] += cv[i];
+            for (int i = 0; i < 6; i += 2) fadd2(xb[i], xb[i + 1], xb[i], xb[i + 1], cv[i], cv[i + 1]);
         }
         xb[5] += gdte;
         if (OX && ox != nullptr && act) {
