@@ -300,6 +300,22 @@ pinmpc_status pinmpc_split_solve_ex(int nu, int N, int B, const pinmpc_layout *l
                                     float rho, int iters, const pinmpc_split_problem *p, const pinmpc_split_options *opts,
                                     void *d_workspace, size_t workspace_bytes, float *xi, float *z, float *r_prim, void *stream);
 
+/* pinmpc_split_solve_ex for callers that cannot allocate device memory (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): no workspace argument.  The scratch is a static device array of
+ * PINMPC_SPLIT_STATIC_BYTES inside the library: every GPU that loads the library holds it until the process exits.
+ * The call allocates nothing (no cudaMalloc / cudaFree / allocating library routine; the array's device address is
+ * looked up once per device on the first call there, with the caller's current device).  Same arguments, outputs and
+ * errors as pinmpc_split_solve_ex otherwise; PINMPC_EALLOC when pinmpc_split_workspace_bytes_ex(nu, N, B, opts) exceeds
+ * PINMPC_SPLIT_STATIC_BYTES (about 3200 stages at nu = 12, 2100 at nu = 18, without options), with the sizes in
+ * pinmpc_last_error(NULL).  All calls on a device share the one array: it keeps the last call's contents (everything
+ * that must start at zero is cleared on `stream` by the call itself), and two calls that overlap on the GPU (different
+ * streams, or different threads) RACE: serialise them. */
+#define PINMPC_SPLIT_STATIC_BYTES (16u << 20)
+size_t pinmpc_split_static_bytes(void);
+pinmpc_status pinmpc_split_solve_static(int nu, int N, int B, const pinmpc_layout *layout, const float *h_Qdiag, const float *h_Rdiag,
+                                        float rho, int iters, const pinmpc_split_problem *p, const pinmpc_split_options *opts,
+                                        float *xi, float *z, float *r_prim, void *stream);
+
 /* The paper's own 9-state centroidal model (eq. (1)-(4)): xi = [c ; l_G ; k_G] (CoM position, linear
  * and angular centroidal momentum), forward Euler; the lever r_{i,k} = p_{i,k} - c_k of contact i is data.
  * Writes the LTV system of eq. (16), xi_{k+1} = A xi_k + B_k u_k + e:  A [B,N,9,9], Bm [B,N,9,nu], e [B,N,9] with
@@ -309,7 +325,7 @@ pinmpc_status pinmpc_assemble_centroidal(int B, int N, int n_wrench, int n_force
                                          float *A, float *Bm, float *e, void *stream);
 
 /* Human-readable description of the last error on this handle (owned by the handle; "" if none).
- * With h = NULL: the last pinmpc_create failure in this thread. */
+ * With h = NULL: the last pinmpc_create or pinmpc_split_solve_static failure in this thread. */
 const char *pinmpc_last_error(pinmpc_t h);
 
 /* Free the host context.  The workspace and all problem buffers stay with the caller. */

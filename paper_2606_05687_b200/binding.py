@@ -27,7 +27,8 @@ EXPORTS = ("pinmpc_workspace_bytes", "pinmpc_workspace_bytes_method", "pinmpc_cr
            "pinmpc_destroy", "pinmpc_set_profiling", "pinmpc_get_kernel_ms",
            "pinmpc_set_warm_start", "pinmpc_shift_aux", "pinmpc_landmark_ring_bytes", "pinmpc_landmark_reset", "pinmpc_landmark_push",
            "pinmpc_landmark_push_solver", "pinmpc_landmark_reward", "pinmpc_split_workspace_bytes", "pinmpc_split_solve",
-           "pinmpc_split_workspace_bytes_ex", "pinmpc_split_solve_ex", "pinmpc_assemble_centroidal")
+           "pinmpc_split_workspace_bytes_ex", "pinmpc_split_solve_ex", "pinmpc_assemble_centroidal",
+           "pinmpc_split_static_bytes", "pinmpc_split_solve_static")
 MAX_LANDMARKS = 8
 
 
@@ -139,6 +140,11 @@ def load():
     lib.pinmpc_split_solve_ex.argtypes = [c_int, c_int, c_int, POINTER(Layout), POINTER(c_float), POINTER(c_float), c_float, c_int,
                                           POINTER(SplitProblem), POINTER(SplitOptions), c_void_p, c_size_t, c_void_p, c_void_p, c_void_p,
                                           c_void_p]
+    lib.pinmpc_split_static_bytes.restype = c_size_t
+    lib.pinmpc_split_static_bytes.argtypes = []
+    lib.pinmpc_split_solve_static.restype = c_int
+    lib.pinmpc_split_solve_static.argtypes = [c_int, c_int, c_int, POINTER(Layout), POINTER(c_float), POINTER(c_float), c_float, c_int,
+                                              POINTER(SplitProblem), POINTER(SplitOptions), c_void_p, c_void_p, c_void_p, c_void_p]
     lib.pinmpc_assemble_centroidal.restype = c_int
     lib.pinmpc_assemble_centroidal.argtypes = [c_int, c_int, c_int, c_int, c_float] + [c_void_p] * 6
     lib.pinmpc_destroy.restype = None
@@ -512,6 +518,23 @@ class SplitSolver:
                                             ctypes.byref(prob), ctypes.byref(self.opts), _ptr(self.ws), self.workspace_bytes, _ptr(self.xi),
                                             _ptr(self.z), _ptr(self.r_prim), st))
         return self.xi, self.z, self.r_prim
+
+
+def split_solve_static(A, Bm, c, x0, u_prev, x_ref, u_ref, contact, layout, Qdiag, Rdiag, rho, iters, xi, z, r_prim, stream=None):
+    """pinmpc_split_solve_static on torch CUDA tensors: no workspace, nothing allocated by the call (the scratch is a static
+    device array of the library, pinmpc_split_static_bytes() bytes).  xi, z [B,N,nx+nu] and r_prim [B] are caller-owned
+    outputs.  Raises PinmpcError (EALLOC with the sizes in the message) when the problem does not fit.  Asynchronous."""
+    import torch
+    B, N, nx, nu = Bm.shape
+    Qd = (c_float * NX)(*([float(v) for v in Qdiag] + [0.0] * (NX - len(Qdiag)))); Rd = (c_float * nu)(*[float(v) for v in Rdiag])
+    prob = SplitProblem(*[None if t is None else t.data_ptr() for t in (A, Bm, c, x0, u_prev, x_ref, u_ref, contact)])
+    null = ctypes.cast(None, POINTER(c_float))
+    opts = SplitOptions(null, 1.0, 0, 0.0, None, int(nx), null, null)
+    st = c_void_p(torch.cuda.current_stream(Bm.device).cuda_stream if stream is None else stream.cuda_stream)
+    rc = load().pinmpc_split_solve_static(nu, N, B, ctypes.byref(layout), Qd, Rd, float(rho), int(iters), ctypes.byref(prob), ctypes.byref(opts),
+                                          _ptr(xi), _ptr(z), _ptr(r_prim), st)
+    if rc != OK:
+        raise PinmpcError(rc, load().pinmpc_last_error(None).decode())
 
 
 def assemble_centroidal(n_wrench, n_force, dt, mass, foot_r, stream=None):

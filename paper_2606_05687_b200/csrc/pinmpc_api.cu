@@ -388,6 +388,9 @@ extern "C" pinmpc_status pinmpc_get_kernel_ms(pinmpc_t h, float *h_ms)
     return PINMPC_OK;
 }
 
+// Error text of a handle-less entry point (pinmpc_split_solve_static): this thread's handle-less error string.
+void pinmpc_note_error(const char *msg) { snprintf(g_create_err, sizeof g_create_err, "%s", msg); }
+
 extern "C" const char *pinmpc_last_error(pinmpc_t h) { return h ? h->err : g_create_err; }
 
 extern "C" void pinmpc_destroy(pinmpc_t h)

@@ -24,6 +24,9 @@
 //                      the accept / restart decision, k_split_extrapolate forms w^_{m+1}
 #include "pinmpc_common.cuh"
 #include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <mutex>
 
 namespace {
 
@@ -530,4 +533,65 @@ extern "C" pinmpc_status pinmpc_split_solve(int nu, int N, int B, const pinmpc_l
                                             float *xi, float *z, float *r_prim, void *stream)
 {
     return pinmpc_split_solve_ex(nu, N, B, layout, h_Qdiag, h_Rdiag, rho, iters, p, nullptr, d_ws, ws_bytes, xi, z, r_prim, stream);
+}
+
+// ---------------------------------------------------------------------------------------------
+// pinmpc_split_solve_static: the same solve for callers that cannot allocate (CUDA graph capture, serving loops,
+// harnesses that forbid cudaMalloc).  The workspace is this file-scope array: PINMPC_SPLIT_STATIC_BYTES of every GPU that
+// loads the library, held until the process exits.  In host code `g_split_scratch` is only the host-side stand-in of
+// the symbol, not a device address: the address is resolved once per device, with that device current, by
+// cudaGetSymbolAddress and that pointer goes to the kernels.  Every call shares the array and finds the last call's
+// contents in it: pinmpc_split_solve_ex zeroes the iterates (cudaMemsetAsync on the stream) and k_split_factor rewrites
+// every factor before use, nothing else is read before it is written.  Calls that overlap on the GPU race.
+// ---------------------------------------------------------------------------------------------
+static __device__ __align__(256) unsigned char g_split_scratch[PINMPC_SPLIT_STATIC_BYTES];
+
+namespace {
+constexpr int STATIC_MAX_DEVICES = 64;
+std::mutex g_static_mu;
+void *g_static_ptr[STATIC_MAX_DEVICES];        // device address of g_split_scratch, per device ordinal (nullptr = not resolved)
+
+pinmpc_status static_fail(pinmpc_status s, const char *fmt, ...)
+{
+    char msg[256];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(msg, sizeof msg, fmt, ap);
+    va_end(ap);
+    pinmpc_note_error(msg);
+    return s;
+}
+}   // namespace
+
+extern "C" size_t pinmpc_split_static_bytes(void) { return PINMPC_SPLIT_STATIC_BYTES; }
+
+extern "C" pinmpc_status pinmpc_split_solve_static(int nu, int N, int B, const pinmpc_layout *layout, const float *h_Qdiag, const float *h_Rdiag,
+                                                   float rho, int iters, const pinmpc_split_problem *p, const pinmpc_split_options *opts,
+                                                   float *xi, float *z, float *r_prim, void *stream)
+{
+    const size_t need = pinmpc_split_workspace_bytes_ex(nu, N, B, opts);
+    if (need == 0) return static_fail(PINMPC_EUNSUPPORTED, "pinmpc_split_solve_static: unsupported sizes (nu = %d, N = %d, B = %d)", nu, N, B);
+    if (need > (size_t)PINMPC_SPLIT_STATIC_BYTES)
+        return static_fail(PINMPC_EALLOC, "pinmpc_split_solve_static: this problem needs %zu bytes of scratch, the static array holds %zu "
+                           "(PINMPC_SPLIT_STATIC_BYTES); use pinmpc_split_solve_ex with a caller-owned workspace", need, (size_t)PINMPC_SPLIT_STATIC_BYTES);
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess || dev < 0 || dev >= STATIC_MAX_DEVICES)
+        return static_fail(PINMPC_ECUDA, "pinmpc_split_solve_static: cudaGetDevice: %s (device %d)", cudaGetErrorString(e), dev);
+    void *ws = nullptr;
+    {
+        std::lock_guard<std::mutex> lk(g_static_mu);
+        if (g_static_ptr[dev] == nullptr) {                  // set-up, once per device, with that device current
+            void *ptr = nullptr;
+            e = cudaGetSymbolAddress(&ptr, g_split_scratch);
+            if (e != cudaSuccess || ptr == nullptr)
+                return static_fail(PINMPC_ECUDA, "pinmpc_split_solve_static: cudaGetSymbolAddress: %s", cudaGetErrorString(e));
+            g_static_ptr[dev] = ptr;
+        }
+        ws = g_static_ptr[dev];
+    }
+    const pinmpc_status rc = pinmpc_split_solve_ex(nu, N, B, layout, h_Qdiag, h_Rdiag, rho, iters, p, opts, ws, PINMPC_SPLIT_STATIC_BYTES, xi, z, r_prim,
+                                                   stream);
+    if (rc != PINMPC_OK) static_fail(rc, "pinmpc_split_solve_static: pinmpc_split_solve_ex returned status %d", (int)rc);
+    return rc;
 }
