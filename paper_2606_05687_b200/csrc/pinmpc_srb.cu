@@ -189,27 +189,35 @@ __global__ void __launch_bounds__(128) k_assemble_srb(SolveParams P, ProblemPtrs
 }
 
 // ---------------------------------------------------------------------------------------------
-// S2  factorisation: one warp per env, sequential over stages.  Lane i < 13 owns row i of the 13x13
-// matrices P and X = P A (rows padded to 16 floats in shared memory, float4 accesses, no index
-// arithmetic in the loop); lanes 0..20 own one packed element of the symmetric 6x6 Mh each.
+// S2  factorisation: TWO envs per warp (lanes 0-15 and 16-31), sequential over stages.  Lane hl < 13 of a half owns
+// row hl of the 13x13 matrices P and X = P A of its env (rows 20 floats apart in shared memory, float4 accesses, no
+// index arithmetic in the loop).  The symmetric 6x6 Mh is inverted by sweeps on the packed 21 elements, one element
+// per lane 0..20 of the whole warp, for one env after the other (the only part that is not packed).  With one env per
+// warp 13 of 32 lanes worked: the kernel is bound by issue slots and shared-memory wavefronts, so packing halves it.
 // ---------------------------------------------------------------------------------------------
-constexpr int FAC_WARPS = 4;                        // warps (envs) per CTA
+constexpr int FAC_WARPS = 4;                        // warps per CTA (8 envs)
+constexpr int FAC_EPW = 2;                          // envs per warp
 constexpr int FAC_LD = 20;                          // padded row length: rows 80 B apart, the float4 row accesses of eight lanes hit distinct banks
-constexpr int FAC_SMEM = 13 * FAC_LD + 13 * FAC_LD + 6 * FAC_LD + 24;   // floats per warp: P, X, Kh, Mh^-1
+constexpr int FAC_SMEM = 13 * FAC_LD + 13 * FAC_LD + 6 * FAC_LD + 24;   // floats per env: P, X, Kh, Mh^-1
 
-__global__ void __launch_bounds__(FAC_WARPS * 32, 7) k_factor_srb(SolveParams P, const float *__restrict__ x0, SrbWs W, int has_ext)
+__global__ void __launch_bounds__(FAC_WARPS * 32, 4) k_factor_srb(SolveParams P, const float *__restrict__ x0, SrbWs W, int has_ext)
 {
-    __shared__ __align__(16) float sm_all[FAC_WARPS * FAC_SMEM];
+    __shared__ __align__(16) float sm_all[FAC_WARPS * FAC_EPW * FAC_SMEM];
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
-    const int b = blockIdx.x * FAC_WARPS + wib;
-    if (b >= P.B) return;
-    float *sP = sm_all + wib * FAC_SMEM, *sX = sP + 13 * FAC_LD, *sK = sX + 13 * FAC_LD, *sM = sK + 6 * FAC_LD;
+    const int hf = lane >> 4, hl = lane & 15, hb = 16 * hf;          // half of the warp, lane inside it, its first lane
+    const int bw = (blockIdx.x * FAC_WARPS + wib) * FAC_EPW;         // first env of the warp
+    if (bw >= P.B) return;
+    const bool pair = bw + 1 < P.B;                                  // a last odd env: half 1 shadows it (no stores)
+    const int b = bw + (pair ? hf : 0);
+    const bool live = hf == 0 || pair;
+    float *sE[FAC_EPW] = { sm_all + (wib * FAC_EPW) * FAC_SMEM, sm_all + (wib * FAC_EPW + 1) * FAC_SMEM };
+    float *sP = sE[hf], *sX = sP + 13 * FAC_LD, *sK = sX + 13 * FAC_LD, *sM = sK + 6 * FAC_LD;
     const int N = P.N;
     const long st = (long)P.B * N;
     const float dt = P.dt;
     const float x12 = x0[(long)b * NX + 12];
-    const int row = lane < NX ? lane : 0;             // lanes >= 13 shadow row 0 (no stores)
-    const bool rown = lane < NX;
+    const int row = hl < NX ? hl : 0;                 // lanes >= 13 of a half shadow row 0 (no stores)
+    const bool rown = hl < NX;
 
     // lane <-> (i,j) of the packed symmetric 6x6 (lanes >= 21 shadow element (0,0))
     int mi = 0, mj = 0;
@@ -236,23 +244,28 @@ __global__ void __launch_bounds__(FAC_WARPS * 32, 7) k_factor_srb(SolveParams P,
         }
     }
     __syncwarp();
-    const int jl = lane < 12 ? lane : 0;
+    const int jl = hl < 12 ? hl : 0;
     float pc = W.qv[((long)b * (N + 1) + N) * 12 + jl];     // pc_N = q_N
+    const long sq[FAC_EPW] = { (long)bw * N, (long)(bw + (pair ? 1 : 0)) * N };     // stage 0 of the warp's two envs
 
     // prefetch stage N-1
     long s = (long)b * N + N - 1;
     float cs_n = W.cs[s * 2], sn_n = W.cs[s * 2 + 1];
-    float S_n = W.MI[(long)(lane < 21 ? lane : 0) * st + s];
-    float ch_n = (has_ext && lane < 6) ? W.c6[s * 6 + lane] : 0.0f;
+    float S_n[FAC_EPW];
+#pragma unroll
+    for (int q = 0; q < FAC_EPW; q++) S_n[q] = W.MI[(long)(lane < 21 ? lane : 0) * st + sq[q] + N - 1];
+    float ch_n = (has_ext && hl < 6) ? W.c6[s * 6 + hl] : 0.0f;
     float q_n = N >= 2 ? W.qv[((long)b * (N + 1) + N - 1) * 12 + jl] : 0.0f;      // q_k of the stage being processed
     for (int k = N - 1; k >= 0; k--) {
         s = (long)b * N + k;
-        const float cs = cs_n, sn = sn_n, Sl = S_n, chl = ch_n, qk12 = k >= 1 ? q_n : 0.0f;
+        const float cs = cs_n, sn = sn_n, chl = ch_n, qk12 = k >= 1 ? q_n : 0.0f;
+        const float Sl[FAC_EPW] = { S_n[0], S_n[1] };
         if (k > 1) q_n = W.qv[((long)b * (N + 1) + k - 1) * 12 + jl];
         if (k > 0) {
             cs_n = W.cs[(s - 1) * 2]; sn_n = W.cs[(s - 1) * 2 + 1];
-            S_n = W.MI[(long)(lane < 21 ? lane : 0) * st + s - 1];
-            ch_n = (has_ext && lane < 6) ? W.c6[(s - 1) * 6 + lane] : 0.0f;
+#pragma unroll
+            for (int q = 0; q < FAC_EPW; q++) S_n[q] = W.MI[(long)(lane < 21 ? lane : 0) * st + sq[q] + k - 1];
+            ch_n = (has_ext && hl < 6) ? W.c6[(s - 1) * 6 + hl] : 0.0f;
         }
         // ---- X = P A, row `row`:  columns 6..12 pick up dt * (R_z^T | I | e_11) combinations of columns 0..5, 11
         float xr[16];
@@ -272,26 +285,33 @@ __global__ void __launch_bounds__(FAC_WARPS * 32, 7) k_factor_srb(SolveParams P,
                 Xr[2] = make_float4(xr[8], xr[9], xr[10], xr[11]); Xr[3] = make_float4(xr[12], 0.0f, 0.0f, 0.0f);
             }
         }
-        // ---- Mh = S + P[6:12,6:12] (one packed element per lane) ;  s_k = P (E ch)
-        float M = Sl + sP[(6 + mi) * FAC_LD + 6 + mj];
+        // ---- s_k = P (E ch)
         float sk = 0.0f;
         if (has_ext) {
 #pragma unroll
-            for (int a = 0; a < 6; a++) sk = fmaf(sP[row * FAC_LD + 6 + a], __shfl_sync(FULL, chl, a), sk);
+            for (int a = 0; a < 6; a++) sk = fmaf(sP[row * FAC_LD + 6 + a], __shfl_sync(FULL, chl, hb + a), sk);
         }
-        // Mh^-1 by symmetric sweeps (-Mh^-1 after six pivots), all in registers
+        // ---- Mh = S + P[6:12,6:12], one packed element per lane 0..20, and Mh^-1 by symmetric sweeps (-Mh^-1 after six
+        // pivots), all in registers: one env of the warp after the other
 #pragma unroll
-        for (int p = 0; p < 6; p++) {
-            float d = __shfl_sync(FULL, M, sidx(p, p));
-            float a = __shfl_sync(FULL, M, la[p]);
-            float c = __shfl_sync(FULL, M, lb[p]);
-            float id = 1.0f / d;
-            if (mi == p && mj == p) M = -id;
-            else if (mi == p || mj == p) M = M * id;
-            else M = fmaf(-a * id, c, M);
+        for (int q = 0; q < FAC_EPW; q++) {
+            float M = Sl[q] + sE[q][(6 + mi) * FAC_LD + 6 + mj];
+#pragma unroll
+            for (int p = 0; p < 6; p++) {
+                float d = __shfl_sync(FULL, M, sidx(p, p));
+                float a = __shfl_sync(FULL, M, la[p]);
+                float c = __shfl_sync(FULL, M, lb[p]);
+                float id = 1.0f / d;
+                if (mi == p && mj == p) M = -id;
+                else if (mi == p || mj == p) M = M * id;
+                else M = fmaf(-a * id, c, M);
+            }
+            M = -M;
+            if (lane < 21) {
+                sE[q][13 * FAC_LD + 13 * FAC_LD + 6 * FAC_LD + lane] = M;
+                if (q == 0 || pair) W.RA[pinmpc_rec_index(lane, st, sq[q] + k)] = M;
+            }
         }
-        M = -M;
-        if (lane < 21) { sM[lane] = M; W.RA[pinmpc_rec_index(lane, st, s)] = M; }
         __syncwarp();
         // ---- Kh = Mh^-1 X[6:12,:], column `row`;  xc = X[6..11][row] = G[:, row] is reused for the P update
         float xc[6], kc[6];
@@ -309,7 +329,7 @@ __global__ void __launch_bounds__(FAC_WARPS * 32, 7) k_factor_srb(SolveParams P,
         if (rown) {
 #pragma unroll
             for (int r = 0; r < 6; r++) sK[r * FAC_LD + row] = kc[r];
-            if (row < 12) {
+            if (row < 12 && live) {
                 const int pos = row < 6 ? 2 * row : 2 * (row - 6) + 1;
 #pragma unroll
                 for (int r = 0; r < 6; r++) W.Kh[s * 72 + r * 12 + pos] = kc[r];
@@ -317,26 +337,26 @@ __global__ void __launch_bounds__(FAC_WARPS * 32, 7) k_factor_srb(SolveParams P,
         }
         __syncwarp();
         // ---- iteration-invariant part of the backward vector pass (response to q and s, sigma0 = 0):
-        //   g = pc - s_k ; hq_k = E^T g ; pc <- q_k + A^T g - Kh^T hq_k        (lane j < 12 holds pc_j)
+        //   g = pc - s_k ; hq_k = E^T g ; pc <- q_k + A^T g - Kh^T hq_k        (lane hl < 12 of the half holds pc_j)
         // The iteration kernel runs the sigma0-driven part only; hq_k enters kappa_k through kg_k.
         {
             const float g = pc - sk;
-            const float g_lo = __shfl_sync(FULL, g, lane >= 6 ? lane - 6 : lane);
-            const float g_nb = __shfl_sync(FULL, g, lane >= 6 ? (lane - 6) ^ 1 : lane);
+            const float g_lo = __shfl_sync(FULL, g, hb + (hl >= 6 ? hl - 6 : hl));
+            const float g_nb = __shfl_sync(FULL, g, hb + (hl >= 6 ? (hl - 6) ^ 1 : hl));
             float acc = 0.0f, mh = 0.0f;
-            const int il = lane < 6 ? lane : 0;
+            const int il = hl < 6 ? hl : 0;
 #pragma unroll
             for (int r = 0; r < 6; r++) {
-                const float hr = __shfl_sync(FULL, g, 6 + r);
-                acc = fmaf(kc[r], hr, acc);                 // kc = Kh[:, lane] for lane < 13
+                const float hr = __shfl_sync(FULL, g, hb + 6 + r);
+                acc = fmaf(kc[r], hr, acc);                 // kc = Kh[:, hl] for hl < 13
                 mh = fmaf(sM[sidx(il, r)], hr, mh);
             }
             // constant part of kappa_k = Mh^-1 hh_k - Kh[:,12] x_12 :  kg_k = Kh[:,12] x_12 - Mh^-1 hq_k
-            if (lane < 6) W.RA[pinmpc_rec_index(21 + lane, st, s)] = fmaf(sK[lane * FAC_LD + 12], x12, -mh);
+            if (hl < 6 && live) W.RA[pinmpc_rec_index(21 + hl, st, s)] = fmaf(sK[hl * FAC_LD + 12], x12, -mh);
             float atg = g;
-            if (lane == 6) atg = fmaf(dt, cs * g_lo - sn * g_nb, g);
-            else if (lane == 7) atg = fmaf(dt, cs * g_lo + sn * g_nb, g);
-            else if (lane >= 8 && lane < 12) atg = fmaf(dt, g_lo, g);
+            if (hl == 6) atg = fmaf(dt, cs * g_lo - sn * g_nb, g);
+            else if (hl == 7) atg = fmaf(dt, cs * g_lo + sn * g_nb, g);
+            else if (hl >= 8 && hl < 12) atg = fmaf(dt, g_lo, g);
             pc = qk12 + atg - acc;
         }
         // ---- P <- [k>=1] Q + A^T X - G^T Kh, row `row`, four columns at a time
@@ -1026,7 +1046,7 @@ int launch_t(pinmpc_ctx *h, cudaStream_t st)
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(h, "k_assemble_srb launch", e);
     if (prof) cudaEventRecord(h->ev[1], st);
-    k_factor_srb<<<(unsigned)((h->B + FAC_WARPS - 1) / FAC_WARPS), FAC_WARPS * 32, 0, st>>>(P, q.x0, h->srb, ext);
+    k_factor_srb<<<(unsigned)((h->B + FAC_WARPS * FAC_EPW - 1) / (FAC_WARPS * FAC_EPW)), FAC_WARPS * 32, 0, st>>>(P, q.x0, h->srb, ext);
     e = cudaGetLastError();
     if (e != cudaSuccess) return fail(h, "k_factor_srb launch", e);
     if (prof) cudaEventRecord(h->ev[2], st);
