@@ -301,10 +301,11 @@ __global__ void __launch_bounds__(FAC_WARPS * 32, 4) k_factor_srb(SolveParams P,
                 float d = __shfl_sync(FULL, M, sidx(p, p));
                 float a = __shfl_sync(FULL, M, la[p]);
                 float c = __shfl_sync(FULL, M, lb[p]);
-                float id = 1.0f / d;
-                if (mi == p && mj == p) M = -id;
-                else if (mi == p || mj == p) M = M * id;
-                else M = fmaf(-a * id, c, M);
+                // (branch-free, and the reciprocal without the slow path of an IEEE division: this is the longest
+                // dependent chain of a stage; d > 0 is a pivot of an SPD matrix, 1 ulp is far inside the parity budget)
+                const float id = __fdividef(1.0f, d);
+                const float t = fmaf(-a * id, c, M);
+                M = (mi == p && mj == p) ? -id : ((mi == p || mj == p) ? M * id : t);
             }
             M = -M;
             if (lane < 21) {
@@ -377,7 +378,8 @@ __global__ void __launch_bounds__(FAC_WARPS * 32, 4) k_factor_srb(SolveParams P,
                     o.x = fmaf(-xc[l], kv.x, o.x); o.y = fmaf(-xc[l], kv.y, o.y);
                     o.z = fmaf(-xc[l], kv.z, o.z); o.w = fmaf(-xc[l], kv.w, o.w);
                 }
-                if (row == 4 * c) o.x += qk; else if (row == 4 * c + 1) o.y += qk; else if (row == 4 * c + 2) o.z += qk; else if (row == 4 * c + 3) o.w += qk;
+                o.x += row == 4 * c ? qk : 0.0f; o.y += row == 4 * c + 1 ? qk : 0.0f;
+                o.z += row == 4 * c + 2 ? qk : 0.0f; o.w += row == 4 * c + 3 ? qk : 0.0f;
                 // upper triangle (j >= row), mirrored: P stays exactly symmetric over long horizons
                 const float ov[4] = { o.x, o.y, o.z, o.w };
 #pragma unroll
