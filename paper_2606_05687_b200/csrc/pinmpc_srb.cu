@@ -219,16 +219,6 @@ __global__ void __launch_bounds__(FAC_WARPS * 32, 4) k_factor_srb(SolveParams P,
     const int row = hl < NX ? hl : 0;                 // lanes >= 13 of a half shadow row 0 (no stores)
     const bool rown = hl < NX;
 
-    // lane <-> (i,j) of the packed symmetric 6x6 (lanes >= 21 shadow element (0,0))
-    int mi = 0, mj = 0;
-    {
-        int l = lane < 21 ? lane : 0, r = 0;
-        while (l >= 6 - r) { l -= 6 - r; r++; }
-        mi = r; mj = r + l;
-    }
-    int la[6], lb[6];
-#pragma unroll
-    for (int p = 0; p < 6; p++) { la[p] = sidx(mi, p); lb[p] = sidx(p, mj); }
     // A^T X: row i of A^T X = X[i] + ea X[ra] + eb X[rb]  (rows 6..12 pick up dt * rows of X)
     const int ra = row == 6 || row == 7 ? 0 : (row == 8 ? 2 : (row >= 9 && row <= 11 ? row - 6 : (row == 12 ? 11 : 0)));
     const int rb = row == 6 || row == 7 ? 1 : ra;
@@ -251,20 +241,29 @@ __global__ void __launch_bounds__(FAC_WARPS * 32, 4) k_factor_srb(SolveParams P,
     // prefetch stage N-1
     long s = (long)b * N + N - 1;
     float cs_n = W.cs[s * 2], sn_n = W.cs[s * 2 + 1];
-    float S_n[FAC_EPW];
+    float S_n[21];                                    // S_k of the own env, all 21 packed elements in every lane (broadcast loads)
 #pragma unroll
-    for (int q = 0; q < FAC_EPW; q++) S_n[q] = W.MI[(long)(lane < 21 ? lane : 0) * st + sq[q] + N - 1];
+    for (int i = 0; i < 21; i++) S_n[i] = W.MI[(long)i * st + s];
     float ch_n = (has_ext && hl < 6) ? W.c6[s * 6 + hl] : 0.0f;
     float q_n = N >= 2 ? W.qv[((long)b * (N + 1) + N - 1) * 12 + jl] : 0.0f;      // q_k of the stage being processed
     for (int k = N - 1; k >= 0; k--) {
         s = (long)b * N + k;
         const float cs = cs_n, sn = sn_n, chl = ch_n, qk12 = k >= 1 ? q_n : 0.0f;
-        const float Sl[FAC_EPW] = { S_n[0], S_n[1] };
+        // ---- Mh = S + P[6:12,6:12], packed upper triangle, in every lane of the half (rows 6..11 of P, columns 4..11: two
+        // aligned float4 per row, the block starts at column 6)
+        float M[21];
+#pragma unroll
+        for (int i = 0; i < 6; i++) {
+            const float4 lo = *reinterpret_cast<const float4 *>(sP + (6 + i) * FAC_LD + 4), hi = *reinterpret_cast<const float4 *>(sP + (6 + i) * FAC_LD + 8);
+            const float pr[6] = { lo.z, lo.w, hi.x, hi.y, hi.z, hi.w };
+#pragma unroll
+            for (int j = i; j < 6; j++) M[sidx(i, j)] = S_n[sidx(i, j)] + pr[j];
+        }
         if (k > 1) q_n = W.qv[((long)b * (N + 1) + k - 1) * 12 + jl];
         if (k > 0) {
             cs_n = W.cs[(s - 1) * 2]; sn_n = W.cs[(s - 1) * 2 + 1];
 #pragma unroll
-            for (int q = 0; q < FAC_EPW; q++) S_n[q] = W.MI[(long)(lane < 21 ? lane : 0) * st + sq[q] + k - 1];
+            for (int i = 0; i < 21; i++) S_n[i] = W.MI[(long)i * st + s - 1];
             ch_n = (has_ext && hl < 6) ? W.c6[(s - 1) * 6 + hl] : 0.0f;
         }
         // ---- X = P A, row `row`:  columns 6..12 pick up dt * (R_z^T | I | e_11) combinations of columns 0..5, 11
@@ -291,41 +290,41 @@ __global__ void __launch_bounds__(FAC_WARPS * 32, 4) k_factor_srb(SolveParams P,
 #pragma unroll
             for (int a = 0; a < 6; a++) sk = fmaf(sP[row * FAC_LD + 6 + a], __shfl_sync(FULL, chl, hb + a), sk);
         }
-        // ---- Mh = S + P[6:12,6:12], one packed element per lane 0..20, and Mh^-1 by symmetric sweeps (-Mh^-1 after six
-        // pivots), all in registers: one env of the warp after the other
+        // ---- Mh^-1 by symmetric sweeps (-Mh^-1 after six pivots), redundantly in the registers of every lane: no exchange
+        // between lanes inside this chain, the longest of a stage (with one element per lane and three shuffles per pivot
+        // it was 40 % of the kernel's time).  The reciprocal without the slow path of an IEEE division: d > 0 is a pivot
+        // of an SPD matrix, 1 ulp is far inside the parity budget.
 #pragma unroll
-        for (int q = 0; q < FAC_EPW; q++) {
-            float M = Sl[q] + sE[q][(6 + mi) * FAC_LD + 6 + mj];
+        for (int p = 0; p < 6; p++) {
+            const float id = __fdividef(1.0f, M[sidx(p, p)]);
+            float t[6], Mn[21];
 #pragma unroll
-            for (int p = 0; p < 6; p++) {
-                float d = __shfl_sync(FULL, M, sidx(p, p));
-                float a = __shfl_sync(FULL, M, la[p]);
-                float c = __shfl_sync(FULL, M, lb[p]);
-                // (branch-free, and the reciprocal without the slow path of an IEEE division: this is the longest
-                // dependent chain of a stage; d > 0 is a pivot of an SPD matrix, 1 ulp is far inside the parity budget)
-                const float id = __fdividef(1.0f, d);
-                const float t = fmaf(-a * id, c, M);
-                M = (mi == p && mj == p) ? -id : ((mi == p || mj == p) ? M * id : t);
-            }
-            M = -M;
-            if (lane < 21) {
-                sE[q][13 * FAC_LD + 13 * FAC_LD + 6 * FAC_LD + lane] = M;
-                if (q == 0 || pair) W.RA[pinmpc_rec_index(lane, st, sq[q] + k)] = M;
-            }
+            for (int i = 0; i < 6; i++) t[i] = M[sidx(i, p)] * id;
+#pragma unroll
+            for (int i = 0; i < 6; i++)
+#pragma unroll
+                for (int j = i; j < 6; j++)
+                    Mn[sidx(i, j)] = (i == p && j == p) ? -id : (i == p ? t[j] : (j == p ? t[i] : fmaf(-t[i], M[sidx(p, j)], M[sidx(i, j)])));
+#pragma unroll
+            for (int i = 0; i < 21; i++) M[i] = Mn[i];
+        }
+#pragma unroll
+        for (int i = 0; i < 21; i++) M[i] = -M[i];
+        if (hl == 0) {                                       // one lane per env publishes Mh^-1 (for the record and the vector pass)
+#pragma unroll
+            for (int c = 0; c < 5; c++) *reinterpret_cast<float4 *>(sM + 4 * c) = make_float4(M[4 * c], M[4 * c + 1], M[4 * c + 2], M[4 * c + 3]);
+            sM[20] = M[20];
         }
         __syncwarp();
         // ---- Kh = Mh^-1 X[6:12,:], column `row`;  xc = X[6..11][row] = G[:, row] is reused for the P update
         float xc[6], kc[6];
 #pragma unroll
         for (int l = 0; l < 6; l++) xc[l] = sX[(6 + l) * FAC_LD + row];
-        {
-            float Mi[24];
+        symv6(M, xc, kc);
+        if (lane < 21) {                                     // the packed Mh^-1 of both envs -> stage records
 #pragma unroll
-            for (int c = 0; c < 6; c++) {
-                const float4 v = *reinterpret_cast<const float4 *>(sM + 4 * c);
-                Mi[4 * c] = v.x; Mi[4 * c + 1] = v.y; Mi[4 * c + 2] = v.z; Mi[4 * c + 3] = v.w;
-            }
-            symv6(Mi, xc, kc);
+            for (int q = 0; q < FAC_EPW; q++)
+                if (q == 0 || pair) W.RA[pinmpc_rec_index(lane, st, sq[q] + k)] = sE[q][13 * FAC_LD + 13 * FAC_LD + 6 * FAC_LD + lane];
         }
         if (rown) {
 #pragma unroll
