@@ -21,7 +21,7 @@ static const int SRB_NARR = 8;
 static void srb_sizes(int nu, int N, int B, size_t *f)
 {
     size_t st = (size_t)B * N;
-    f[0] = st * 72; f[1] = (size_t)B * (N + 1) * 12; f[2] = st * 6; f[3] = st * 2; f[4] = st * 21;
+    f[0] = st * 72; f[1] = (size_t)B * (N + 1) * 12; f[2] = st * 6; f[3] = st * 2; f[4] = st * 24;
     f[5] = st * PINMPC_RA_W; f[6] = st * (size_t)pinmpc_rb_width(nu);
     f[7] = (size_t)B * pinmpc_psi_cap(N, nu) * 144;
 }

@@ -51,7 +51,7 @@ struct SrbWs {
     float *qv;     // [B][N+1][12]   q_k = Q xbar_k (k = 1..N), q_0 = 0
     float *c6;     // [st][6]        ch = (dt I_w^-1 tau_ext ; dt/m F_ext)   (zeros without ext_wrench)
     float *cs;     // [st][2]        cos, sin of the linearisation yaw
-    float *MI;     // [21][st]       S_k = D^-1 Lam^-1 D^-1 (packed symmetric): assembly -> factorisation
+    float *MI;     // [6][st][4]     S_k = D^-1 Lam^-1 D^-1 (packed symmetric, 21 of 24 words): assembly -> factorisation
     // Stage constants streamed by the stage threads of the iteration kernel every iteration: float4
     // component-major, so that thread = stage reads them with coalesced LDG.128 (word w of stage s is
     // at [(w / 4) * st + s] * 4 + w % 4).

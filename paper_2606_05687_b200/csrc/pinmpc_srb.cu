@@ -164,8 +164,15 @@ __global__ void __launch_bounds__(128) k_assemble_srb(SolveParams P, ProblemPtrs
         for (int x = 0; x < 3; x++)
 #pragma unroll
             for (int y = x; y < 3; y++) S[sidx(3 + x, 3 + y)] = Lam[sidx(3 + x, 3 + y)] * m_dt * m_dt;
+        // S_k as six float4 groups, group-major (the layout of the stage records): coalesced here, six 16-byte loads per
+        // stage in the factorisation
+        {
+            float4 *MI4 = reinterpret_cast<float4 *>(W.MI);
 #pragma unroll
-        for (int i = 0; i < 21; i++) W.MI[i * st + s] = S[i];
+            for (int g = 0; g < 6; g++)
+                MI4[(long)g * st + s] = make_float4(S[4 * g], 4 * g + 1 < 21 ? S[4 * g + 1] : 0.0f, 4 * g + 2 < 21 ? S[4 * g + 2] : 0.0f,
+                                                    4 * g + 3 < 21 ? S[4 * g + 3] : 0.0f);
+        }
     }
     // the stage record of the iteration kernel: float4 component-major
     {
@@ -241,9 +248,10 @@ __global__ void __launch_bounds__(FAC_WARPS * 32, 4) k_factor_srb(SolveParams P,
     // prefetch stage N-1
     long s = (long)b * N + N - 1;
     float cs_n = W.cs[s * 2], sn_n = W.cs[s * 2 + 1];
-    float S_n[21];                                    // S_k of the own env, all 21 packed elements in every lane (broadcast loads)
+    const float4 *MI4 = reinterpret_cast<const float4 *>(W.MI);
+    float4 S_n[6];                                    // S_k of the own env, all 21 packed elements in every lane (broadcast loads)
 #pragma unroll
-    for (int i = 0; i < 21; i++) S_n[i] = W.MI[(long)i * st + s];
+    for (int g = 0; g < 6; g++) S_n[g] = MI4[(long)g * st + s];
     float ch_n = (has_ext && hl < 6) ? W.c6[s * 6 + hl] : 0.0f;
     float q_n = N >= 2 ? W.qv[((long)b * (N + 1) + N - 1) * 12 + jl] : 0.0f;      // q_k of the stage being processed
     for (int k = N - 1; k >= 0; k--) {
@@ -257,13 +265,17 @@ __global__ void __launch_bounds__(FAC_WARPS * 32, 4) k_factor_srb(SolveParams P,
             const float4 lo = *reinterpret_cast<const float4 *>(sP + (6 + i) * FAC_LD + 4), hi = *reinterpret_cast<const float4 *>(sP + (6 + i) * FAC_LD + 8);
             const float pr[6] = { lo.z, lo.w, hi.x, hi.y, hi.z, hi.w };
 #pragma unroll
-            for (int j = i; j < 6; j++) M[sidx(i, j)] = S_n[sidx(i, j)] + pr[j];
+            for (int j = i; j < 6; j++) {
+                const float4 sg = S_n[sidx(i, j) >> 2];
+                const int w = sidx(i, j) & 3;
+                M[sidx(i, j)] = (w == 0 ? sg.x : (w == 1 ? sg.y : (w == 2 ? sg.z : sg.w))) + pr[j];
+            }
         }
         if (k > 1) q_n = W.qv[((long)b * (N + 1) + k - 1) * 12 + jl];
         if (k > 0) {
             cs_n = W.cs[(s - 1) * 2]; sn_n = W.cs[(s - 1) * 2 + 1];
 #pragma unroll
-            for (int i = 0; i < 21; i++) S_n[i] = W.MI[(long)i * st + s - 1];
+            for (int g = 0; g < 6; g++) S_n[g] = MI4[(long)g * st + s - 1];
             ch_n = (has_ext && hl < 6) ? W.c6[(s - 1) * 6 + hl] : 0.0f;
         }
         // ---- X = P A, row `row`:  columns 6..12 pick up dt * (R_z^T | I | e_11) combinations of columns 0..5, 11
@@ -1154,7 +1166,7 @@ __global__ void __launch_bounds__(128) k_srb_expand(SolveParams P, SrbWs W, cons
             for (int i = 0; i < 6; i++) cc[6 + i] = W.c6[s * 6 + i];
     }
     if (S)
-        for (int i = 0; i < 21; i++) S[s * 21 + i] = W.MI[(long)i * st + s];
+        for (int i = 0; i < 21; i++) S[s * 21 + i] = W.MI[((long)(i >> 2) * st + s) * 4 + (i & 3)];
     if (Tinv)
         for (int i = 0; i < 6; i++) Tinv[s * 6 + i] = rec[i];
 }

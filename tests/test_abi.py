@@ -38,9 +38,9 @@ def test_host_only_entry_points_without_a_gpu(lib):
     base = binding.pinmpc_workspace_bytes(13, 12, 50, 4096, lay)
     dense = binding.pinmpc_workspace_bytes(13, 12, 50, 4096, lay, binding.METHOD_DENSE)
     st = 4096 * 50
-    # outputs x,u,z,y (13 + 36 floats per stage) + the structured solver's factors (175 per stage + q_0) + the chunk
+    # outputs x,u,z,y (13 + 36 floats per stage) + the structured solver's factors (178 per stage + q_0) + the chunk
     # operators of the chunked iteration kernel (ceil(N / 5) - 2 = 8 matrices of 144 floats per env)
-    per_stage = (13 + 36) + (72 + 12 + 6 + 2 + 21 + 28 + 32)
+    per_stage = (13 + 36) + (72 + 12 + 6 + 2 + 24 + 28 + 32)
     lo = (st * per_stage + 4096 * 12 + 4096 * 8 * 144) * 4
     assert base >= lo and base < lo + 20 * 256 + 3 * 4096 * 4
     assert dense > base + st * (169 + 156 + 156 + 144) * 4
