@@ -217,8 +217,9 @@ __global__ void __launch_bounds__(FAC_WARPS * 32, 4) k_factor_srb(SolveParams P,
     const bool pair = bw + 1 < P.B;                                  // a last odd env: half 1 shadows it (no stores)
     const int b = bw + (pair ? hf : 0);
     const bool live = hf == 0 || pair;
-    float *sE[FAC_EPW] = { sm_all + (wib * FAC_EPW) * FAC_SMEM, sm_all + (wib * FAC_EPW + 1) * FAC_SMEM };
-    float *sP = sE[hf], *sX = sP + 13 * FAC_LD, *sK = sX + 13 * FAC_LD, *sM = sK + 6 * FAC_LD;
+    // (plain arithmetic on the __shared__ array, so that the accesses compile to LDS / STS: a pointer picked from an array
+    // of pointers made them generic loads, which go through the global-memory queue)
+    float *sP = sm_all + (wib * FAC_EPW + hf) * FAC_SMEM, *sX = sP + 13 * FAC_LD, *sK = sX + 13 * FAC_LD, *sM = sK + 6 * FAC_LD;
     const int N = P.N;
     const long st = (long)P.B * N;
     const float dt = P.dt;
@@ -336,7 +337,7 @@ __global__ void __launch_bounds__(FAC_WARPS * 32, 4) k_factor_srb(SolveParams P,
         if (lane < 21) {                                     // the packed Mh^-1 of both envs -> stage records
 #pragma unroll
             for (int q = 0; q < FAC_EPW; q++)
-                if (q == 0 || pair) W.RA[pinmpc_rec_index(lane, st, sq[q] + k)] = sE[q][13 * FAC_LD + 13 * FAC_LD + 6 * FAC_LD + lane];
+                if (q == 0 || pair) W.RA[pinmpc_rec_index(lane, st, sq[q] + k)] = sm_all[(wib * FAC_EPW + q) * FAC_SMEM + 32 * FAC_LD + lane];
         }
         if (rown) {
 #pragma unroll
