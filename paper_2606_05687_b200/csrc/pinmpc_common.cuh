@@ -110,6 +110,14 @@ size_t pinmpc_ws_srb_bytes(int nu, int N, int B);
 bool pinmpc_tm_config(const pinmpc_ctx *h, int *G, int *C);
 int pinmpc_launch_iterate_tm(pinmpc_ctx *h, int G, int C, cudaStream_t st);
 // chunk operators of up to ceil(N / 5) chunks (nu = 12: 5 or 6 stages per chunk), ceil(N / 3) chunks (nu = 18: 3 or 4)
+// chunk c of C over N stages (the chunked iteration kernel): the first N % C chunks hold one stage more
+__host__ __device__ inline void tm_chunk(int N, int C, int c, int &k0, int &len)
+{
+    const int base = N / C, rem = N - base * C;
+    k0 = c * base + (c < rem ? c : rem);
+    len = base + (c < rem ? 1 : 0);
+}
+
 void pinmpc_note_error(const char *msg);   // pinmpc_api.cu: sets what pinmpc_last_error(NULL) returns in this thread
 inline int pinmpc_psi_cap(int N, int nu) { int c = (nu == 12 ? (N + 4) / 5 : (N + 2) / 3) - 2; return c > 0 ? c : 0; }
 

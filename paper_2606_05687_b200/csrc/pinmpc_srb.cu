@@ -207,7 +207,7 @@ constexpr int FAC_EPW = 2;                          // envs per warp
 constexpr int FAC_LD = 20;                          // padded row length: rows 80 B apart, the float4 row accesses of eight lanes hit distinct banks
 constexpr int FAC_SMEM = 13 * FAC_LD + 13 * FAC_LD + 6 * FAC_LD + 24;   // floats per env: P, X, Kh, Mh^-1
 
-__global__ void __launch_bounds__(FAC_WARPS * 32, 4) k_factor_srb(SolveParams P, const float *__restrict__ x0, SrbWs W, int has_ext)
+__global__ void __launch_bounds__(FAC_WARPS * 32, 4) k_factor_srb(SolveParams P, const float *__restrict__ x0, SrbWs W, int has_ext, int C, float *__restrict__ Psi)
 {
     __shared__ __align__(16) float sm_all[FAC_WARPS * FAC_EPW * FAC_SMEM];
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
@@ -255,6 +255,15 @@ __global__ void __launch_bounds__(FAC_WARPS * 32, 4) k_factor_srb(SolveParams P,
     for (int g = 0; g < 6; g++) S_n[g] = MI4[(long)g * st + s];
     float ch_n = (has_ext && hl < 6) ? W.c6[s * 6 + hl] : 0.0f;
     float q_n = N >= 2 ? W.qv[((long)b * (N + 1) + N - 1) * 12 + jl] : 0.0f;      // q_k of the stage being processed
+    // chunk operators of the chunked iteration kernel, formed on the way (C > 2): lane hl < 12 carries row hl of
+    // Psi_c = Phi_{k0+len-1} ... Phi_{k0} of the chunk the walk is in, row <- row Phi_k, and stores it at the chunk's first
+    // stage.  Psi [B][C-2][12][12] for the inner chunks c = 1 .. C-2.  (This chain is independent of the Riccati chain and
+    // fills issue slots the latter leaves empty; as a kernel of its own it took 43 us.)
+    int pc_c = C - 1, pc_k0 = 0, pc_len = 0;
+    if (C > 2) tm_chunk(N, C, pc_c, pc_k0, pc_len);
+    float pa[6], pb[6];
+#pragma unroll
+    for (int j = 0; j < 6; j++) { pa[j] = 0.0f; pb[j] = 0.0f; }
     for (int k = N - 1; k >= 0; k--) {
         s = (long)b * N + k;
         const float cs = cs_n, sn = sn_n, chl = ch_n, qk12 = k >= 1 ? q_n : 0.0f;
@@ -349,6 +358,38 @@ __global__ void __launch_bounds__(FAC_WARPS * 32, 4) k_factor_srb(SolveParams P,
             }
         }
         __syncwarp();
+        if (C > 2) {                                         // (uniform)
+            if (k < pc_k0) { pc_c--; tm_chunk(N, C, pc_c, pc_k0, pc_len); }
+            if (pc_c >= 1 && pc_c <= C - 2) {
+                if (k == pc_k0 + pc_len - 1) {
+#pragma unroll
+                    for (int j = 0; j < 6; j++) { pa[j] = (hl == j) ? 1.0f : 0.0f; pb[j] = (hl == 6 + j) ? 1.0f : 0.0f; }
+                }
+                //   (row Phi)_a = row_a + row_b Kn_a ;  (row Phi)_b = dt row_a Rot + row_b + row_b Kn_b,  Kn = -Kh
+                float na[6], nb[6];
+                nb[0] = fmaf(dt, cs * pa[0] - sn * pa[1], pb[0]);
+                nb[1] = fmaf(dt, sn * pa[0] + cs * pa[1], pb[1]);
+#pragma unroll
+                for (int j = 2; j < 6; j++) nb[j] = fmaf(dt, pa[j], pb[j]);
+#pragma unroll
+                for (int j = 0; j < 6; j++) na[j] = pa[j];
+#pragma unroll
+                for (int r = 0; r < 6; r++) {
+                    const float4 k0v = *reinterpret_cast<const float4 *>(sK + r * FAC_LD), k1v = *reinterpret_cast<const float4 *>(sK + r * FAC_LD + 4),
+                                 k2v = *reinterpret_cast<const float4 *>(sK + r * FAC_LD + 8);
+                    const float m = -pb[r];
+                    na[0] = fmaf(m, k0v.x, na[0]); na[1] = fmaf(m, k0v.y, na[1]); na[2] = fmaf(m, k0v.z, na[2]); na[3] = fmaf(m, k0v.w, na[3]);
+                    na[4] = fmaf(m, k1v.x, na[4]); na[5] = fmaf(m, k1v.y, na[5]); nb[0] = fmaf(m, k1v.z, nb[0]); nb[1] = fmaf(m, k1v.w, nb[1]);
+                    nb[2] = fmaf(m, k2v.x, nb[2]); nb[3] = fmaf(m, k2v.y, nb[3]); nb[4] = fmaf(m, k2v.z, nb[4]); nb[5] = fmaf(m, k2v.w, nb[5]);
+                }
+#pragma unroll
+                for (int j = 0; j < 6; j++) { pa[j] = na[j]; pb[j] = nb[j]; }
+                if (k == pc_k0 && hl < 12 && live) {
+                    float4 *o = reinterpret_cast<float4 *>(Psi + (((long)b * (C - 2) + pc_c - 1) * 12 + hl) * 12);
+                    o[0] = make_float4(pa[0], pa[1], pa[2], pa[3]); o[1] = make_float4(pa[4], pa[5], pb[0], pb[1]); o[2] = make_float4(pb[2], pb[3], pb[4], pb[5]);
+                }
+            }
+        }
         // ---- iteration-invariant part of the backward vector pass (response to q and s, sigma0 = 0):
         //   g = pc - s_k ; hq_k = E^T g ; pc <- q_k + A^T g - Kh^T hq_k        (lane hl < 12 of the half holds pc_j)
         // The iteration kernel runs the sigma0-driven part only; hq_k enters kappa_k through kg_k.
@@ -1060,7 +1101,11 @@ int launch_t(pinmpc_ctx *h, cudaStream_t st)
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(h, "k_assemble_srb launch", e);
     if (prof) cudaEventRecord(h->ev[1], st);
-    k_factor_srb<<<(unsigned)((h->B + FAC_WARPS * FAC_EPW - 1) / (FAC_WARPS * FAC_EPW)), FAC_WARPS * 32, 0, st>>>(P, q.x0, h->srb, ext);
+    // which iteration kernel will run is known before the factorisation, which forms the chunk operators of the chunked one
+    int tmG = 0, tmC = 0;
+    const bool chunked = h->chunks != 1 && (h->chunks > 1 || h->N >= PINMPC_CHUNKED_MIN_N) && pinmpc_tm_config(h, &tmG, &tmC);
+    k_factor_srb<<<(unsigned)((h->B + FAC_WARPS * FAC_EPW - 1) / (FAC_WARPS * FAC_EPW)), FAC_WARPS * 32, 0, st>>>(P, q.x0, h->srb, ext,
+                                                                                                                chunked ? tmC : 0, h->psi);
     e = cudaGetLastError();
     if (e != cudaSuccess) return fail(h, "k_factor_srb launch", e);
     if (prof) cudaEventRecord(h->ev[2], st);
@@ -1070,8 +1115,7 @@ int launch_t(pinmpc_ctx *h, cudaStream_t st)
     // the chunked kernel wins from N = 20 on (1.05x at N = 20, 1.2x at N = 50, 1.35x at N = 100) and loses below (0.7-0.9x
     // at N = 10, where two chunks of five stages leave nothing to run in parallel).
     int nk = 2;
-    int tmG = 0, tmC = 0;
-    if (h->chunks != 1 && (h->chunks > 1 || h->N >= PINMPC_CHUNKED_MIN_N) && pinmpc_tm_config(h, &tmG, &tmC)) {
+    if (chunked) {
         const int n = pinmpc_launch_iterate_tm(h, tmG, tmC, st);
         if (n < 0) return -1;
         nk += n;

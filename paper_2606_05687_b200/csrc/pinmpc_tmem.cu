@@ -11,7 +11,7 @@
 //               backward from the zero terminal costate): gives the chunk's affine offset d_c / b_c
 //     boundary  x_{k_{c+1}} = Psi_c x_{k_c} + d_c  (backward: p_{k_c} = Psi_c^T p_{k_{c+1}} + b_c), C - 2 dependent
 //               12 x 12 steps with the chunk operators Psi_c = Phi_{k_c + L - 1} ... Phi_{k_c} formed once per
-//               solve by k_chunk_ops
+//               solve by the factorisation kernel on its backward walk
 //     sweep B   every chunk concurrently from its true boundary vector, producing hh -> kappa (backward) and
 //               w, x (forward)
 // so the dependent depth of a pass drops from N to 2 L + C - 2 (50 -> 19 at N = 50, C = 9).
@@ -102,62 +102,8 @@ __device__ __forceinline__ void tm_sync()
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 }
 
-// chunk c of C over N stages: the first N % C chunks hold one stage more
-__host__ __device__ inline void tm_chunk(int N, int C, int c, int &k0, int &len)
-{
-    const int base = N / C, rem = N - base * C;
-    k0 = c * base + (c < rem ? c : rem);
-    len = base + (c < rem ? 1 : 0);
-}
-
-// ---------------------------------------------------------------------------------------------
-// chunk operators Psi_c = Phi_{k0+len-1} ... Phi_{k0} for the inner chunks c = 1 .. C-2, once per solve.
-// One thread per (env, chunk, row): row <- row Phi_k from the last stage of the chunk to the first.
-//   (row Phi)_a = row_a + row_b Kn_a ;  (row Phi)_b = dt row_a Rot + row_b + row_b Kn_b
-// Psi [B][C-2][12][12] row-major.
-// ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(192) k_chunk_ops(int B, int N, int C, float dt, const float *__restrict__ Kh, const float *__restrict__ cs,
-                                                   float *__restrict__ Psi)
-{
-    const long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
-    const long rows = (long)B * (C - 2) * 12;
-    if (t >= rows) return;
-    const int i = (int)(t % 12);
-    const long bc = t / 12;
-    const int c = (int)(bc % (C - 2)) + 1, b = (int)(bc / (C - 2));
-    int k0, len;
-    tm_chunk(N, C, c, k0, len);
-    float ra[6], rb[6];
-#pragma unroll
-    for (int j = 0; j < 6; j++) { ra[j] = (i == j) ? 1.0f : 0.0f; rb[j] = (i == 6 + j) ? 1.0f : 0.0f; }
-    for (int k = k0 + len - 1; k >= k0; k--) {
-        const long s = (long)b * N + k;
-        const float4 *kp = reinterpret_cast<const float4 *>(Kh + s * 72);
-        const float co = cs[s * 2], sn = cs[s * 2 + 1];
-        float na[6], nb[6];
-        // dt row_a Rot:  Rot = [[c, s], [-s, c]] (+) I_4   (Theta+ = Theta + dt R_z^T omega, p+ = p + dt v)
-        nb[0] = fmaf(dt, co * ra[0] - sn * ra[1], rb[0]);
-        nb[1] = fmaf(dt, sn * ra[0] + co * ra[1], rb[1]);
-#pragma unroll
-        for (int j = 2; j < 6; j++) nb[j] = fmaf(dt, ra[j], rb[j]);
-#pragma unroll
-        for (int j = 0; j < 6; j++) na[j] = ra[j];
-#pragma unroll
-        for (int r = 0; r < 6; r++) {
-            // Kh row r as pairs (Kh[r][j], Kh[r][6+j]);  Kn = -Kh
-            const float4 v0 = __ldg(kp + 3 * r), v1 = __ldg(kp + 3 * r + 1), v2 = __ldg(kp + 3 * r + 2);
-            const float m = -rb[r];
-            na[0] = fmaf(m, v0.x, na[0]); nb[0] = fmaf(m, v0.y, nb[0]); na[1] = fmaf(m, v0.z, na[1]); nb[1] = fmaf(m, v0.w, nb[1]);
-            na[2] = fmaf(m, v1.x, na[2]); nb[2] = fmaf(m, v1.y, nb[2]); na[3] = fmaf(m, v1.z, na[3]); nb[3] = fmaf(m, v1.w, nb[3]);
-            na[4] = fmaf(m, v2.x, na[4]); nb[4] = fmaf(m, v2.y, nb[4]); na[5] = fmaf(m, v2.z, na[5]); nb[5] = fmaf(m, v2.w, nb[5]);
-        }
-#pragma unroll
-        for (int j = 0; j < 6; j++) { ra[j] = na[j]; rb[j] = nb[j]; }
-    }
-    float *o = Psi + t * 12;
-#pragma unroll
-    for (int j = 0; j < 6; j++) { o[j] = ra[j]; o[6 + j] = rb[j]; }
-}
+// The chunk operators Psi_c = Phi_{k0+len-1} ... Phi_{k0} of the inner chunks c = 1 .. C-2 (Psi [B][C-2][12][12] row-major) are
+// formed by the factorisation kernel on its backward walk (k_factor_srb in pinmpc_srb.cu), once per solve.
 
 // ---------------------------------------------------------------------------------------------
 // chain sweeps (one thread = one chunk of one env).  A sweep is software-pipelined over half stages: while
@@ -1035,14 +981,6 @@ template <int NU>
 static int tm_launch_t(pinmpc_ctx *h, const SolveParams &P, const ProblemPtrs &q, int G, int C, cudaStream_t st)
 {
     const int ext = q.ext != nullptr;
-    int n = 0;
-    if (C > 2) {
-        const long rows = (long)h->B * (C - 2) * 12;
-        k_chunk_ops<<<(unsigned)((rows + 191) / 192), 192, 0, st>>>(h->B, h->N, C, h->dt, h->srb.Kh, h->srb.cs, h->psi);
-        cudaError_t e = cudaGetLastError();
-        if (e != cudaSuccess) return tm_fail(h, "k_chunk_ops launch", e);
-        n++;
-    }
     auto kern = q.z0 ? k_iterate_tm<NU, true> : k_iterate_tm<NU, false>;
     const size_t smem = pinmpc_tm_smem_bytes(h->N, G, C, h->nu);
     static std::once_flag once[2];                             // process-global attribute: set once, not per solve
@@ -1054,10 +992,10 @@ static int tm_launch_t(pinmpc_ctx *h, const SolveParams &P, const ProblemPtrs &q
     kern<<<(unsigned)((h->B + G - 1) / G), tm_threads(NU), smem, st>>>(P, h->srb, h->psi, q.x0, q.mass, h->out, G, C, ext, q.z0, q.y0);
     e = cudaGetLastError();
     if (e != cudaSuccess) return tm_fail(h, "k_iterate_tm launch", e);
-    return n + 1;
+    return 1;
 }
 
-// Launch the chunk-operator kernel and the chunked iteration kernel (after assembly and factorisation).
+// Launch the chunked iteration kernel (after assembly and factorisation, which also forms the chunk operators).
 // Returns the number of kernels enqueued, or -1.
 int pinmpc_launch_iterate_tm(pinmpc_ctx *h, int G, int C, cudaStream_t st)
 {
