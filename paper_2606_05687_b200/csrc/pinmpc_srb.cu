@@ -1123,9 +1123,13 @@ int launch_t(pinmpc_ctx *h, cudaStream_t st)
     } else {
         // the cold-start kernel carries no warm-start code (same registers and schedule as without the feature)
         auto kern = q.z0 ? k_iterate_srb<NU, true> : k_iterate_srb<NU, false>;
-        cudaFuncAttributes fa;
-        e = cudaFuncGetAttributes(&fa, kern);
-        if (e != cudaSuccess) return fail(h, "k_iterate_srb attributes", e);
+        static std::once_flag fa_once[2];                          // per kernel variant (and per NU: launch_t is a template)
+        static cudaFuncAttributes fa_cache[2];
+        static cudaError_t fa_err[2];
+        const int fi = q.z0 ? 1 : 0;
+        std::call_once(fa_once[fi], [&] { fa_err[fi] = cudaFuncGetAttributes(&fa_cache[fi], kern); });
+        if (fa_err[fi] != cudaSuccess) return fail(h, "k_iterate_srb attributes", fa_err[fi]);
+        const cudaFuncAttributes &fa = fa_cache[fi];
         int G = h->envs_per_cta;
         if (G > G_MAX || (G > 0 && iterate_threads(h->N, G) > ITER_MAX_THREADS) || (G > 0 && iterate_smem_bytes(h->N, G, ext, h->nu) > (size_t)h->smem_optin)) G = 0;
         if (G == 0) G = choose_G(h, fa.numRegs, ext);
